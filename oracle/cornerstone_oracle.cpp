@@ -1,0 +1,382 @@
+// =====================================================================================
+// cornerstone_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, single-threaded CPU restatement of what the hot path of
+// arXiv 2307.06345 ("Cornerstone", PAPER.md) computes.  It exists only so that the
+// CUDA library can be checked against it bit for bit.  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// load it.  It shares no code, header, table or helper with
+// paper_2307_06345_b200/csrc/ and neither side includes the other.
+//
+// Build: g++ -std=c++17 -O2 -ffp-contract=off -fno-fast-math -shared -fPIC
+//        (see oracle/build.py).  -ffp-contract=off keeps (c-lo)/e*2^21 as three
+//        separately rounded IEEE-754 binary64 operations (reading A2).
+//
+// Every function cites the PAPER.md passage it follows; readings of silent or garbled
+// passages are the "A<n>" items of DESIGN.md ("Readings of the paper").
+// Parity pins: tests/test_oracle_*.py (all functions here are pinned; nothing is
+// "parity unpinned").
+// =====================================================================================
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <utility>
+#include <vector>
+
+namespace {
+
+constexpr int L = 21;                       // octree depth of a 64-bit key
+constexpr uint64_t KEY_END = 1ull << 63;    // 8^L, PAPER.md:66 (Eq. 2)
+
+// length of the key range of a node at division level l: 8^(L-l)
+inline uint64_t nodeRange(int level) { return 1ull << (3 * (L - level)); }
+
+}  // namespace
+
+extern "C" {
+
+// -------------------------------------------------------------------------------------
+// O1  bounding box.  The paper is silent (it starts from grid coordinates,
+// PAPER.md:54); north_star defines the key through (xmin, xmax).  Reading A1: closed
+// per-dimension [min, max] over the particles; a zero result is returned as +0.0.
+// box6 = {xmin, xmax, ymin, ymax, zmin, zmax}.  Returns 0, or 1 if n == 0.
+// -------------------------------------------------------------------------------------
+int orc_box(const double* x, const double* y, const double* z, uint64_t n, double* box6)
+{
+    if (n == 0) return 1;
+    const double* c[3] = {x, y, z};
+    for (int d = 0; d < 3; ++d) {
+        double mn = c[d][0], mx = c[d][0];
+        for (uint64_t i = 1; i < n; ++i) {
+            if (c[d][i] < mn) mn = c[d][i];
+            if (c[d][i] > mx) mx = c[d][i];
+        }
+        box6[2 * d]     = mn + 0.0;   // -0.0 -> +0.0 (round-to-nearest), A1
+        box6[2 * d + 1] = mx + 0.0;
+    }
+    return 0;
+}
+
+// -------------------------------------------------------------------------------------
+// O2  64-bit Morton keys, 21 bits per dimension.  PAPER.md:54-60 (Sec. 3, Eq. 1): the
+// key is L octal digits, digit i selecting the octant at division level i.
+// Grid coordinate (north_star; readings A2, A3):
+//     g = clamp(floor(((c - lo) / (hi - lo)) * 2^21), 0, 2^21 - 1)
+// evaluated in binary64, one rounding per operation, in exactly this order.
+// Octal digit = 4*xbit + 2*ybit + zbit; key bit 62 is x bit 20; bit 63 is 0.
+// -------------------------------------------------------------------------------------
+static uint32_t gridCoordinate(double c, double lo, double e)
+{
+    double t = (c - lo) / e;
+    t = t * 2097152.0;
+    double g = std::floor(t);
+    if (!(g >= 0.0)) g = 0.0;            // negatives and NaN (0/0 for a flat box, A1)
+    if (g > 2097151.0) g = 2097151.0;    // c == hi gives exactly 2^21
+    return (uint32_t)g;
+}
+
+void orc_keys(const double* x, const double* y, const double* z, uint64_t n, const double* box6,
+              uint64_t* keys)
+{
+    const double ex = box6[1] - box6[0];
+    const double ey = box6[3] - box6[2];
+    const double ez = box6[5] - box6[4];
+    for (uint64_t i = 0; i < n; ++i) {
+        uint32_t gx = gridCoordinate(x[i], box6[0], ex);
+        uint32_t gy = gridCoordinate(y[i], box6[2], ey);
+        uint32_t gz = gridCoordinate(z[i], box6[4], ez);
+        uint64_t k = 0;
+        for (int b = 0; b < L; ++b) {     // literal bit interleave, one octal digit per bit plane
+            uint64_t digit = 4ull * ((gx >> b) & 1u) + 2ull * ((gy >> b) & 1u) + ((gz >> b) & 1u);
+            k |= digit << (3 * b);
+        }
+        keys[i] = k;
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O3  sort.  PAPER.md:70 ("encoding ... followed by a radix-sort"), PAPER.md:168 ("the
+// particle SFC keys provided as keys and the identity permutation as values").
+// Reading A5: stable; perm[j] = original index of the particle at sorted slot j.
+// -------------------------------------------------------------------------------------
+void orc_sort(const uint64_t* keysIn, uint64_t n, uint64_t* keysOut, uint32_t* perm)
+{
+    std::vector<std::pair<uint64_t, uint32_t>> kv(n);
+    for (uint64_t i = 0; i < n; ++i) kv[i] = {keysIn[i], (uint32_t)i};
+    std::stable_sort(kv.begin(), kv.end(),
+                     [](const std::pair<uint64_t, uint32_t>& a, const std::pair<uint64_t, uint32_t>& b) {
+                         return a.first < b.first;
+                     });
+    for (uint64_t i = 0; i < n; ++i) {
+        keysOut[i] = kv[i].first;
+        perm[i]    = kv[i].second;
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O5  one f + g round, a literal sequential transcription of Sec. 4.
+//   f  (Eq. 3): N_i = number of keys of P in [K_i, K_{i+1}); counted
+//      here literally with a moving cursor over the sorted P (reading A6: lower bound).
+//   g1 (Eq. 5): O_i = 8 (split), 0 (merged away) or 1 (keep).
+//      Readings: A7 (no split at depth L), A8 (merge iff combined count <= Ncrit),
+//      A9 (the root never merges; 8*delta is formed only below the root).
+//   g2 (Eq. 6): exclusive prefix sum O'.
+//   g3 (Eqs. 7-9; reading A10): K'[O'_i] = K_i if O_i = 1;
+//      K'[O'_i + j] = K_i + j*delta_i/8, j = 0..7, if O_i = 8; A11: K'[O'_{n_l}] = 8^L.
+// K has nl+1 entries.  N (nl), O (nl), Oprime (nl+1) are outputs (may be null).
+// Kout must hold capOut+1 entries.  Returns the new leaf count, or -1 if > capOut.
+// -------------------------------------------------------------------------------------
+int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl, uint32_t bucketSize,
+                  uint32_t* N, uint32_t* O, uint32_t* Oprime, uint64_t* Kout, uint32_t capOut)
+{
+    std::vector<uint32_t> Nv(nl), Ov(nl), Op(nl + 1);
+    // f: literal per-leaf counting
+    uint64_t cur = 0;
+    for (uint32_t i = 0; i < nl; ++i) {
+        while (cur < n && P[cur] < K[i]) ++cur;    // keys below K_0 = 0 do not exist
+        uint64_t c = 0;
+        while (cur < n && P[cur] < K[i + 1]) { ++cur; ++c; }
+        Nv[i] = (uint32_t)c;
+    }
+    // g1
+    for (uint32_t i = 0; i < nl; ++i) {
+        uint64_t delta = K[i + 1] - K[i];
+        if (Nv[i] > bucketSize && delta > 1) { Ov[i] = 8; continue; }
+        Ov[i] = 1;
+        if (delta == KEY_END) continue;             // root leaf: nothing to merge into (A9)
+        uint64_t pd = 8 * delta;
+        uint32_t j  = (uint32_t)((K[i] % pd) / delta);
+        if (j == 0) continue;                       // "K_i is not the first octant"
+        if (i < j || (uint64_t)i - j + 8 > nl) continue;
+        if (K[i - j] + pd != K[i - j + 8]) continue;   // all 8 siblings are leaves
+        uint64_t sum = 0;
+        for (uint32_t s = 0; s < 8; ++s) sum += Nv[i - j + s];
+        if (sum <= bucketSize) Ov[i] = 0;           // A8
+    }
+    // g2
+    uint64_t run = 0;
+    for (uint32_t i = 0; i < nl; ++i) { Op[i] = (uint32_t)run; run += Ov[i]; }
+    Op[nl] = (uint32_t)run;
+    if (N) std::copy(Nv.begin(), Nv.end(), N);
+    if (O) std::copy(Ov.begin(), Ov.end(), O);
+    if (Oprime) std::copy(Op.begin(), Op.end(), Oprime);
+    if (run > capOut) return -1;
+    // g3
+    for (uint32_t i = 0; i < nl; ++i) {
+        if (Ov[i] == 1) Kout[Op[i]] = K[i];
+        else if (Ov[i] == 8) {
+            uint64_t delta = K[i + 1] - K[i];
+            for (uint32_t j = 0; j < 8; ++j) Kout[Op[i] + j] = K[i] + j * (delta / 8);
+        }
+    }
+    Kout[run] = KEY_END;
+    return (int64_t)run;
+}
+
+// -------------------------------------------------------------------------------------
+// O5b  iterate f, g (reading A12): start from Kstart (nlStart leaves),
+// repeat rounds until a round has O_i = 1 for all i, or maxRounds rounds were done
+// (maxRounds = 0: until converged).  The returned K is the output of the last round
+// performed (identical to its input when that round was all ones); *rounds counts the
+// rounds including the confirming one; *converged says whether the last round was all
+// ones.  counts (cap entries) receives N of the returned K.
+// Returns the leaf count or -1 on capacity overflow.
+// -------------------------------------------------------------------------------------
+int64_t orc_leaves_iterative(const uint64_t* P, uint64_t n, uint32_t bucketSize, const uint64_t* Kstart,
+                             uint32_t nlStart, uint32_t maxRounds, uint64_t* Kout, uint32_t* counts,
+                             uint32_t cap, uint32_t* rounds, int* converged)
+{
+    std::vector<uint64_t> K(Kstart, Kstart + nlStart + 1), Kn(cap + 1);
+    std::vector<uint32_t> O;
+    uint32_t r = 0;
+    int conv = 0;
+    for (;;) {
+        uint32_t nl = (uint32_t)K.size() - 1;
+        O.assign(nl, 0);
+        int64_t nn = orc_round(P, n, K.data(), nl, bucketSize, nullptr, O.data(), nullptr, Kn.data(), cap);
+        ++r;
+        if (nn < 0) return -1;
+        conv = 1;
+        for (uint32_t i = 0; i < nl; ++i) if (O[i] != 1) { conv = 0; break; }
+        K.assign(Kn.begin(), Kn.begin() + nn + 1);
+        if (conv || (maxRounds && r >= maxRounds)) break;
+    }
+    uint32_t nl = (uint32_t)K.size() - 1;
+    std::copy(K.begin(), K.end(), Kout);
+    uint64_t cur = 0;                               // f on the returned array
+    for (uint32_t i = 0; i < nl; ++i) {
+        uint64_t c = 0;
+        while (cur < n && P[cur] < K[i + 1]) { ++cur; ++c; }
+        counts[i] = (uint32_t)c;
+    }
+    *rounds = r;
+    *converged = conv;
+    return nl;
+}
+
+// -------------------------------------------------------------------------------------
+// O4  converged leaves by the plain definition: PAPER.md:68 and :120 define "balanced"
+// (leaf counts <= Ncrit, internal-node counts > Ncrit), which is the result of a
+// conventional top-down construction: node [s, s+8^(L-l)) is split iff
+// it holds more than bucketSize particles and l < L (A7).  Counting is literal: every
+// node walks its own particles with a cursor.
+// -------------------------------------------------------------------------------------
+namespace {
+struct TopDown {
+    const uint64_t* P; uint64_t n; uint32_t bucket;
+    std::vector<uint64_t>* K; std::vector<uint32_t>* cnt;
+    // a = index of the first key >= s; returns the index of the first key >= s + range
+    uint64_t node(uint64_t s, int level, uint64_t a)
+    {
+        const uint64_t len = nodeRange(level);
+        const uint64_t e = s + len;                 // level 0: 2^63, fits
+        uint64_t b = a;
+        while (b < n && P[b] < e) ++b;              // literal count of [s, e)
+        if (b - a > bucket && level < L) {
+            uint64_t cur = a;
+            for (int c = 0; c < 8; ++c) cur = node(s + c * (len / 8), level + 1, cur);
+            return cur;
+        }
+        K->push_back(s);
+        cnt->push_back((uint32_t)(b - a));
+        return b;
+    }
+};
+}  // namespace
+
+int64_t orc_leaves_topdown(const uint64_t* P, uint64_t n, uint32_t bucketSize, uint64_t* Kout,
+                           uint32_t* counts, uint32_t cap)
+{
+    std::vector<uint64_t> K;
+    std::vector<uint32_t> cnt;
+    TopDown td{P, n, bucketSize, &K, &cnt};
+    td.node(0, 0, 0);
+    if (K.size() > cap) return -(int64_t)K.size();   // tells the caller the capacity it needs
+    std::copy(K.begin(), K.end(), Kout);
+    Kout[K.size()] = KEY_END;
+    std::copy(cnt.begin(), cnt.end(), counts);
+    return (int64_t)K.size();
+}
+
+// -------------------------------------------------------------------------------------
+// O6  fully linked octree in the format of Sec. 5: node keys NK in
+// Warren-Salmon placeholder-bit format (a 1 bit followed by l octal digits, PAPER.md:
+// 146,152), connectivity CO = index of the first child (0 => leaf), level offsets
+// LO[L+2].  The node order is the one PAPER.md:158 produces ("radix sort NK to yield a
+// breadth-first node ordering", reading A16): by level, SFC order inside a level.
+// Built here the plain way: explicit node objects by recursive descent over K (every
+// internal node has exactly 8 children), then numbered breadth-first.
+// parents[] is reading A20 (parent[0] = 0); leafToNode / nodeToLeaf are reading A23
+// (nodeToLeaf = 0xFFFFFFFF for internal nodes); levelRange is reading A19.
+// Arrays must hold nl + (nl-1)/7 entries.  Returns the node count or -1 if K is not a
+// cornerstone array whose leaves close into an octree.
+// -------------------------------------------------------------------------------------
+namespace {
+struct BuildNode { uint64_t start; int level; int64_t child[8]; int64_t leaf; };
+struct Linker {
+    const uint64_t* K = nullptr; uint32_t nl = 0; uint32_t cursor = 0; bool bad = false;
+    std::vector<BuildNode> nodes;
+    int64_t build(uint64_t start, int level)
+    {
+        int64_t id = (int64_t)nodes.size();
+        nodes.push_back(BuildNode{start, level, {-1, -1, -1, -1, -1, -1, -1, -1}, -1});
+        if (bad || cursor >= nl) { bad = true; return id; }
+        const uint64_t len = nodeRange(level);
+        if (K[cursor] == start && K[cursor + 1] == start + len) {
+            nodes[id].leaf = cursor++;
+            return id;
+        }
+        if (level == L || K[cursor] != start || K[cursor + 1] > start + len) { bad = true; return id; }
+        for (int c = 0; c < 8; ++c) {
+            int64_t ch = build(start + c * (len / 8), level + 1);
+            nodes[id].child[c] = ch;
+        }
+        return id;
+    }
+};
+}  // namespace
+
+int64_t orc_link(const uint64_t* K, uint32_t nl, uint64_t* prefixes, uint32_t* levels, uint32_t* childOffsets,
+                 uint32_t* parents, uint32_t* levelRange, uint32_t* leafToNode, uint32_t* nodeToLeaf)
+{
+    if (nl == 0 || K[0] != 0 || K[nl] != KEY_END) return -1;
+    Linker lk;
+    lk.K = K;
+    lk.nl = nl;
+    lk.build(0, 0);
+    if (lk.bad || lk.cursor != nl) return -1;
+    const std::vector<BuildNode>& nd = lk.nodes;
+    const uint32_t n = (uint32_t)nd.size();
+    // breadth-first numbering: queue order = level by level, key order inside a level
+    std::vector<int64_t> order;  order.reserve(n);
+    std::vector<uint32_t> number(n);
+    order.push_back(0);
+    for (size_t h = 0; h < order.size(); ++h) {
+        const BuildNode& b = nd[order[h]];
+        if (b.leaf < 0) for (int c = 0; c < 8; ++c) order.push_back(b.child[c]);
+    }
+    for (uint32_t i = 0; i < n; ++i) number[order[i]] = i;
+    for (int l = 0; l <= L + 1; ++l) levelRange[l] = n;
+    parents[0] = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const BuildNode& b = nd[order[i]];
+        prefixes[i] = (1ull << (3 * b.level)) | (b.level == 0 ? 0 : (b.start >> (3 * (L - b.level))));
+        levels[i] = (uint32_t)b.level;
+        if (i < levelRange[b.level]) levelRange[b.level] = i;
+        if (b.leaf >= 0) {
+            childOffsets[i] = 0;
+            nodeToLeaf[i] = (uint32_t)b.leaf;
+            leafToNode[b.leaf] = i;
+        } else {
+            childOffsets[i] = number[b.child[0]];
+            nodeToLeaf[i] = 0xFFFFFFFFu;
+            for (int c = 0; c < 8; ++c) parents[number[b.child[c]]] = i;
+        }
+    }
+    // levels deeper than the deepest one start at n (A19); already initialised to n.
+    // a level that is empty but followed by no deeper level keeps n as well.
+    return n;
+}
+
+// -------------------------------------------------------------------------------------
+// O7  per-node particle ranges and counts ("additional octree node
+// properties, such as particle counts"; PAPER.md:258 upward pass: leaves from the
+// particles, internal nodes from their children; reading A21).
+// leafCounts = N of the cornerstone array (from f).  nodeFirst = index into the sorted
+// particle array of the node's first particle, nodeCount = its particle count.
+// Recursive over the links starting at the root.
+// -------------------------------------------------------------------------------------
+namespace {
+struct Upsweep {
+    const uint32_t* childOffsets; const uint32_t* nodeToLeaf; const std::vector<uint64_t>* leafFirst;
+    const uint32_t* leafCounts; uint32_t* nodeFirst; uint32_t* nodeCount;
+    void visit(uint32_t i)
+    {
+        if (childOffsets[i] == 0) {
+            uint32_t lf = nodeToLeaf[i];
+            nodeFirst[i] = (uint32_t)(*leafFirst)[lf];
+            nodeCount[i] = leafCounts[lf];
+            return;
+        }
+        uint64_t sum = 0;
+        for (uint32_t c = 0; c < 8; ++c) {
+            visit(childOffsets[i] + c);
+            sum += nodeCount[childOffsets[i] + c];
+        }
+        nodeFirst[i] = nodeFirst[childOffsets[i]];
+        nodeCount[i] = (uint32_t)sum;
+    }
+};
+}  // namespace
+
+void orc_node_counts(const uint32_t* leafCounts, uint32_t nl, const uint32_t* childOffsets,
+                     const uint32_t* nodeToLeaf, uint32_t numNodes, uint32_t* nodeFirst, uint32_t* nodeCount)
+{
+    (void)numNodes;
+    std::vector<uint64_t> leafFirst(nl + 1, 0);
+    for (uint32_t i = 0; i < nl; ++i) leafFirst[i + 1] = leafFirst[i] + leafCounts[i];
+    Upsweep up{childOffsets, nodeToLeaf, &leafFirst, leafCounts, nodeFirst, nodeCount};
+    up.visit(0);
+}
+
+}  // extern "C"
