@@ -1,0 +1,222 @@
+/* =====================================================================================
+ * cornerstone.h -- C ABI of the B200-native Cornerstone octree builder.
+ *
+ * One data-parallel hot path of arXiv 2307.06345: single-GPU construction of
+ * the cornerstone octree from particle coordinates,
+ *
+ *   coordinates -> bounding box -> 64-bit Morton keys -> stable radix sort (+ permutation)
+ *               -> cornerstone leaf array K by iterating f, g -> linked octree -> node counts
+ *
+ * Every entry point is extern "C", takes plain pointers and sizes, and never throws or
+ * aborts: the return code is the only error channel (cs_lastError gives the text).
+ *
+ * Conventions
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. a torch tensor's
+ *     data_ptr()); the library never frees them and keeps no reference after the call.
+ *     "host" pointers are ordinary host memory.  Scratch memory lives in the context.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Calls enqueue work on `stream`.  A call with a *host out* argument synchronises
+ *     `stream` before returning; calls without one return as soon as the work is enqueued.
+ *   - L = 21: keys are 63-bit Morton codes in a uint64_t, 8^21 = 2^63 is the
+ *     terminal element of a cornerstone array (Eq. 2).
+ *   - Arrays are structure-of-arrays, densely packed, naturally aligned; x, y, z, keys and
+ *     leaves must be 16-byte aligned (any cudaMalloc / torch allocation is).
+ *   - n < 2^32 particles (indices are uint32_t).
+ * ===================================================================================== */
+#ifndef CORNERSTONE_B200_H
+#define CORNERSTONE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CS_MAX_LEVEL 21u               /* L */
+#define CS_KEY_END (1ull << 63)        /* 8^L */
+#define CS_NUM_LEVEL_OFFSETS 23u       /* L + 2 entries of the level-offset array LO */
+#define CS_NO_LEAF 0xFFFFFFFFu         /* nodeToLeaf[] of an internal node */
+
+typedef struct cs_context cs_context;  /* opaque; owns the workspace; bound to one device */
+
+typedef enum cs_status {
+    CS_OK = 0,
+    CS_ERR_INVALID_ARG = 1,      /* null pointer, n == 0 where a box is needed, n >= 2^32, bucketSize == 0 */
+    CS_ERR_CAPACITY = 2,         /* result exceeds leafCapacity / the context's maxLeaves / maxParticles */
+    CS_ERR_NOT_CORNERSTONE = 3,  /* prevLeaves / leaves violates Eq. 2 */
+    CS_ERR_NOT_CONVERGED = 4,    /* maxRounds reached before a round with O_i = 1 for all i */
+    CS_ERR_CUDA = 5              /* a CUDA runtime call failed; see cs_lastError */
+} cs_status;
+
+/* Stage identifiers for cs_stageTimes (milliseconds of device time, CUDA events). */
+enum {
+    CS_STAGE_BOX = 0, CS_STAGE_KEYS = 1, CS_STAGE_SORT = 2, CS_STAGE_LEAVES = 3, CS_STAGE_LINK = 4,
+    CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6, CS_STAGE_SORT_PASSES = 7, CS_NUM_STAGES = 8
+};
+
+/* ---- context ------------------------------------------------------------------------ */
+
+/* Bytes of device workspace cs_create will allocate for these capacities. */
+size_t cs_workspaceBytes(uint64_t maxParticles, uint32_t maxLeaves);
+
+/* Create a context on CUDA device `device` able to process up to maxParticles particles and
+ * trees of up to maxLeaves leaves.  Allocates the workspace (cudaMalloc) once. */
+cs_status cs_create(cs_context** ctx, int device, uint64_t maxParticles, uint32_t maxLeaves);
+void cs_destroy(cs_context* ctx);
+
+/* Text of the last error on this context ("" if none).  ctx may be NULL (global text). */
+const char* cs_lastError(const cs_context* ctx);
+const char* cs_version(void);
+
+/* Enable (1) / disable (0) per-stage CUDA-event timing; read it back after the stream is
+ * idle.  ms[CS_NUM_STAGES], host.  Stages not run since the last reset read 0.
+ * launches (host, nullable) receives the number of kernels the library has launched on
+ * this context since cs_create. */
+cs_status cs_setProfiling(cs_context* ctx, int enabled);
+cs_status cs_stageTimes(cs_context* ctx, float* ms, uint64_t* launches);
+
+/* ---- stages of the path ----------------------------------------------------------------
+ *
+ * cs_computeBox -- per-dimension closed bounding box [min, max] of the particles.
+ *   The paper starts from grid coordinates and is silent on the box; the key
+ *   definition of BASELINE.json:north_star needs (xmin, xmax) per dimension (A1).
+ *   x, y, z: dev, n doubles each, finite.  box6: dev, 6 doubles out
+ *   {xmin, xmax, ymin, ymax, zmin, zmax}; a zero extreme is returned as +0.0.
+ *   Errors: INVALID_ARG (null, n == 0, n >= 2^32), CAPACITY (n > maxParticles), CUDA.
+ */
+cs_status cs_computeBox(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                        double* box6, void* stream);
+
+/* cs_computeKeys -- 64-bit Morton keys, 21 bits per dimension (Eq. 1).
+ *   g_d = clamp(floor(((c_d - lo_d) / (hi_d - lo_d)) * 2^21), 0, 2^21 - 1) in IEEE binary64,
+ *   one rounding per operation in that order, no FMA contraction (A2);
+ *   octal digit = 4*xbit + 2*ybit + zbit, key bit 62 = x bit 20, bit 63 = 0 (A3).
+ *   A flat dimension (hi == lo) maps to grid coordinate 0 (A1).
+ *   box6: dev (as written by cs_computeBox, or any user box).  keys: dev, n uint64 out.
+ */
+cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                         const double* box6, uint64_t* keys, void* stream);
+
+/* cs_sortKeys -- stable ascending radix sort of the keys, carrying the particle index
+ *   ("keys ... and the identity permutation as values"; A5).
+ *   keys: dev, in: n keys < 2^63 in any order, out: sorted.  perm: dev, n uint32 out,
+ *   perm[j] = original index of the particle now at sorted slot j (equal keys keep their
+ *   original relative order).  n == 0 is a no-op.
+ */
+cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream);
+
+/* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1
+ *   (Eqs. 4-9), until a round reports O_i = 1 for all i.
+ *   sortedKeys: dev, n ascending keys < 2^63 (the array P).  bucketSize = N_crit >= 1.
+ *   prevLeaves: dev, nullable.  NULL: start from the root {0, 8^21}.  Otherwise a valid
+ *   cornerstone array with prevNumLeaves leaves (prevNumLeaves+1 keys), e.g. the previous
+ *   time step's; it is validated against Eq. 2.
+ *   maxRounds: 0 = iterate until converged (at most L+1 = 22 rounds are ever needed);
+ *   k > 0 = at most k rounds; maxRounds = 1 is the paper's "single histogram count and
+ *   rebalance update".  If the last round performed was not all-ones the
+ *   outputs hold that round's result and the status is CS_ERR_NOT_CONVERGED.
+ *   Readings: split only below depth L (A7); merge iff the 8 siblings hold <= bucketSize
+ *   particles together (A8); the root never merges (A9); K'[O'_i + j] = K_i + j*delta_i/8 (A10).
+ *   leaves: dev out, numLeaves+1 keys (capacity leafCapacity+1).  counts: dev out, N_i for
+ *   the returned leaves (capacity leafCapacity).  numLeaves, rounds: host out (rounds counts
+ *   f evaluations including the confirming one).  Synchronises `stream`.
+ *   Errors: CAPACITY if a round would exceed leafCapacity or the context's maxLeaves
+ *   (leaves / counts are then left untouched), NOT_CORNERSTONE, INVALID_ARG, CUDA.
+ */
+cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, uint32_t bucketSize,
+                         const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds,
+                         uint64_t* leaves, uint32_t* counts, uint32_t leafCapacity,
+                         uint32_t* numLeaves, uint32_t* rounds, void* stream);
+
+/* cs_linkOctree -- the fully linked octree of Sec. 5, all levels in
+ *   parallel, in the paper's format: node keys NK in Warren-Salmon placeholder-bit form
+ *   (a 1 bit followed by `level` octal digits), connectivity CO (index of
+ *   the first of 8 children, 0 = leaf), level offsets LO[L+2].
+ *   Node order = ascending placeholder key = breadth-first, SFC order within a level
+ *   (A16).  numNodes = numLeaves + (numLeaves-1)/7.
+ *   leaves: dev, numLeaves+1 keys forming a closed octree.  All outputs dev, sized numNodes
+ *   unless noted: prefixes (NK), levels, childOffsets (CO), parents (parent[0] = 0; A20),
+ *   levelRange[23] (LO; entries past the deepest level = numNodes; A19),
+ *   leafToNode[numLeaves], nodeToLeaf[numNodes] (CS_NO_LEAF for internal nodes; A23).
+ *   levels, parents, leafToNode, nodeToLeaf may be NULL (not produced).
+ *   numNodes: host out.  nodeCapacity: capacity of the per-node arrays.  Synchronises.
+ *   Errors: NOT_CORNERSTONE ((numLeaves-1) mod 7 != 0 or the leaves do not close into an
+ *   octree), CAPACITY, INVALID_ARG, CUDA.
+ */
+cs_status cs_linkOctree(cs_context* ctx, const uint64_t* leaves, uint32_t numLeaves,
+                        uint64_t* prefixes, uint32_t* levels, uint32_t* childOffsets, uint32_t* parents,
+                        uint32_t* levelRange, uint32_t* leafToNode, uint32_t* nodeToLeaf,
+                        uint32_t nodeCapacity, uint32_t* numNodes, void* stream);
+
+/* cs_nodeCounts -- per-node particle range in the sorted particle array (PAPER.md:80, 192,
+ *   258; A21): nodeFirst[i] = lower_bound(P, start_i), nodeCount[i] = lower_bound(P, end_i)
+ *   - nodeFirst[i], where [start_i, end_i) is the key range encoded by prefixes[i].
+ *   sortedKeys: dev, n.  prefixes: dev, numNodes placeholder-bit keys (from cs_linkOctree).
+ *   Optional accelerator (both or neither): leafCounts[numLeaves] as returned by
+ *   cs_buildLeaves for the same leaves, and nodeToLeaf[numNodes] from cs_linkOctree; leaf
+ *   nodes then take their range from the prefix sum of leafCounts instead of searching P
+ *   (the two definitions coincide).  Does not synchronise.
+ */
+cs_status cs_nodeCounts(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n,
+                        const uint64_t* prefixes, uint32_t numNodes,
+                        const uint32_t* leafCounts, const uint32_t* nodeToLeaf, uint32_t numLeaves,
+                        uint32_t* nodeFirst, uint32_t* nodeCount, void* stream);
+
+/* ---- the whole path in one call ---------------------------------------------------------
+ *
+ * Output buffers of a full build.  All dev, caller-owned.  Per-leaf arrays hold leafCapacity
+ * (+1 for leaves) entries, per-node arrays nodeCapacity entries. */
+typedef struct cs_octree_buffers {
+    double*   box6;          /* [6]   out */
+    uint64_t* keys;          /* [n]   out: sorted keys P */
+    uint32_t* perm;          /* [n]   out: permutation */
+    uint64_t* leaves;        /* [leafCapacity + 1] out: K */
+    uint32_t* counts;        /* [leafCapacity]     out: N */
+    uint64_t* prefixes;      /* [nodeCapacity] out: NK */
+    uint32_t* levels;        /* [nodeCapacity] out (nullable) */
+    uint32_t* childOffsets;  /* [nodeCapacity] out: CO */
+    uint32_t* parents;       /* [nodeCapacity] out (nullable) */
+    uint32_t* levelRange;    /* [23] out: LO */
+    uint32_t* leafToNode;    /* [leafCapacity] out (nullable) */
+    uint32_t* nodeToLeaf;    /* [nodeCapacity] out */
+    uint32_t* nodeFirst;     /* [nodeCapacity] out */
+    uint32_t* nodeCount;     /* [nodeCapacity] out */
+    uint32_t  leafCapacity;
+    uint32_t  nodeCapacity;
+} cs_octree_buffers;
+
+typedef struct cs_octree_sizes {
+    uint32_t numLeaves;
+    uint32_t numNodes;
+    uint32_t rounds;
+    uint32_t converged;
+} cs_octree_sizes;
+
+/* cs_buildOctree -- box, keys, sort, leaves, link and node counts back to back on `stream`
+ *   with every intermediate size kept on the device: no host round trip until the single
+ *   synchronisation at the end that fills *sizes (host out).  Semantics of each stage are
+ *   exactly those of the stage calls above (prevLeaves / prevNumLeaves / maxRounds as in
+ *   cs_buildLeaves; prevLeaves may alias buffers->leaves).
+ *   x, y, z: dev.  Errors: as the stages; on error the buffers hold unspecified data.
+ */
+cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                         uint32_t bucketSize, const uint64_t* prevLeaves, uint32_t prevNumLeaves,
+                         uint32_t maxRounds, const cs_octree_buffers* buffers, cs_octree_sizes* sizes,
+                         void* stream);
+
+/* cs_buildOctreeHost -- the same path for HOST coordinate buffers (end-to-end form):
+ *   copies x, y, z host -> device, runs cs_buildOctree into context-owned device buffers
+ *   (the context must have been created with capacities covering n and the tree), and
+ *   copies the tree back into the caller's HOST arrays.  `host` has the layout of
+ *   cs_octree_buffers but every pointer is host memory; NULL members are not copied back.
+ *   Pinned (page-locked) host memory gives the full PCIe rate; pageable memory works.
+ */
+cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                             uint32_t bucketSize, const cs_octree_buffers* host, cs_octree_sizes* sizes,
+                             void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CORNERSTONE_B200_H */

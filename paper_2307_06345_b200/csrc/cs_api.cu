@@ -1,0 +1,262 @@
+// extern "C" entry points of libcornerstone_b200.so (see include/cornerstone.h).
+#include <new>
+
+#include "cs_internal.cuh"
+
+using namespace cs;
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+cs_status statusFromCtrl(cs_context* ctx, const char* where)
+{
+    const u32 st = ctx->hostCtrl->c.status;
+    switch (st) {
+        case CS_OK: return CS_OK;
+        case CS_ERR_CAPACITY: return fail(ctx, CS_ERR_CAPACITY, "%s: result exceeds the given capacity", where);
+        case CS_ERR_NOT_CORNERSTONE:
+            return fail(ctx, CS_ERR_NOT_CORNERSTONE, "%s: leaf array violates Eq. 2 (not a cornerstone array)", where);
+        case CS_ERR_NOT_CONVERGED:
+            return fail(ctx, CS_ERR_NOT_CONVERGED, "%s: maxRounds reached before convergence", where);
+        default: return fail(ctx, CS_ERR_CUDA, "%s: unexpected device status %u", where, st);
+    }
+}
+
+cs_status checkParticles(cs_context* ctx, const char* fn, uint64_t n)
+{
+    if (n >= (1ull << 32)) return fail(ctx, CS_ERR_INVALID_ARG, "%s: n >= 2^32", fn);
+    if (n > ctx->maxParticles)
+        return fail(ctx, CS_ERR_CAPACITY, "%s: n = %llu exceeds the context's maxParticles = %llu", fn,
+                    (unsigned long long)n, (unsigned long long)ctx->maxParticles);
+    return CS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+cs_status cs_computeBox(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                        double* box6, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_computeBox: ctx is null");
+    if (!x || !y || !z || !box6) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeBox: null pointer");
+    if (n == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeBox: n == 0 (an empty set has no box)");
+    CS_TRY(checkParticles(ctx, "cs_computeBox", n));
+    DeviceGuard g(ctx->device);
+    return enqueueBox(ctx, x, y, z, n, box6, (cudaStream_t)stream);
+}
+
+cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                         const double* box6, uint64_t* keys, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_computeKeys: ctx is null");
+    if (n == 0) return CS_OK;
+    if (!x || !y || !z || !box6 || !keys) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeKeys: null pointer");
+    CS_TRY(checkParticles(ctx, "cs_computeKeys", n));
+    DeviceGuard g(ctx->device);
+    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, (cudaStream_t)stream);
+}
+
+cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_sortKeys: ctx is null");
+    if (n == 0) return CS_OK;
+    if (!keys || !perm) return fail(ctx, CS_ERR_INVALID_ARG, "cs_sortKeys: null pointer");
+    CS_TRY(checkParticles(ctx, "cs_sortKeys", n));
+    DeviceGuard g(ctx->device);
+    return enqueueSort(ctx, (u64*)keys, perm, n, false, (cudaStream_t)stream);
+}
+
+cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, uint32_t bucketSize,
+                         const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, uint64_t* leaves,
+                         uint32_t* counts, uint32_t leafCapacity, uint32_t* numLeaves, uint32_t* rounds, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_buildLeaves: ctx is null");
+    if ((!sortedKeys && n) || !leaves || !counts || !numLeaves || !rounds)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: null pointer");
+    if (bucketSize == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: bucketSize == 0");
+    if (leafCapacity == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: leafCapacity == 0");
+    if (prevLeaves && prevNumLeaves == 0)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: prevLeaves given with prevNumLeaves == 0");
+    CS_TRY(checkParticles(ctx, "cs_buildLeaves", n));
+    if (prevLeaves && (prevNumLeaves > ctx->maxLeaves || prevNumLeaves > leafCapacity))
+        return fail(ctx, CS_ERR_CAPACITY, "cs_buildLeaves: prevNumLeaves exceeds the leaf capacity");
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    CS_TRY(enqueueLeaves(ctx, (const u64*)sortedKeys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
+                         (u64*)leaves, counts, leafCapacity, s));
+    CS_TRY(readCtrl(ctx, s));
+    const DeviceCtrl& c = ctx->hostCtrl->c;
+    *rounds = c.rounds;
+    *numLeaves = (c.status == CS_OK || c.status == CS_ERR_NOT_CONVERGED) ? c.nl[c.rounds] : 0;
+    return statusFromCtrl(ctx, "cs_buildLeaves");
+}
+
+cs_status cs_linkOctree(cs_context* ctx, const uint64_t* leaves, uint32_t numLeaves, uint64_t* prefixes,
+                        uint32_t* levels, uint32_t* childOffsets, uint32_t* parents, uint32_t* levelRange,
+                        uint32_t* leafToNode, uint32_t* nodeToLeaf, uint32_t nodeCapacity, uint32_t* numNodes,
+                        void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_linkOctree: ctx is null");
+    if (!leaves || !prefixes || !childOffsets || !levelRange || !numNodes)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_linkOctree: null pointer");
+    if (numLeaves == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_linkOctree: numLeaves == 0");
+    if ((numLeaves - 1) % 7 != 0)
+        return fail(ctx, CS_ERR_NOT_CORNERSTONE, "cs_linkOctree: (numLeaves - 1) mod 7 != 0 (PAPER.md:146)");
+    if (numLeaves > ctx->maxLeaves) return fail(ctx, CS_ERR_CAPACITY, "cs_linkOctree: numLeaves exceeds maxLeaves");
+    if (numLeaves + (numLeaves - 1) / 7 > nodeCapacity)
+        return fail(ctx, CS_ERR_CAPACITY, "cs_linkOctree: nodeCapacity too small");
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    CS_CUDA(ctx, cudaMemsetAsync(&ctx->ctrl->status, 0, sizeof(u32), s));
+    CS_TRY(enqueueLink(ctx, (const u64*)leaves, nullptr, numLeaves, numLeaves, (u64*)prefixes, levels, childOffsets,
+                       parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity, s));
+    CS_TRY(readCtrl(ctx, s));
+    *numNodes = ctx->hostCtrl->c.status == CS_OK ? ctx->hostCtrl->c.numNodes : 0;
+    return statusFromCtrl(ctx, "cs_linkOctree");
+}
+
+cs_status cs_nodeCounts(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, const uint64_t* prefixes,
+                        uint32_t numNodes, const uint32_t* leafCounts, const uint32_t* nodeToLeaf, uint32_t numLeaves,
+                        uint32_t* nodeFirst, uint32_t* nodeCount, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_nodeCounts: ctx is null");
+    if (numNodes == 0) return CS_OK;
+    if ((!sortedKeys && n) || !prefixes || !nodeFirst || !nodeCount)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeCounts: null pointer");
+    if ((leafCounts == nullptr) != (nodeToLeaf == nullptr))
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeCounts: leafCounts and nodeToLeaf must be given together");
+    CS_TRY(checkParticles(ctx, "cs_nodeCounts", n));
+    if (leafCounts && numLeaves > ctx->maxLeaves)
+        return fail(ctx, CS_ERR_CAPACITY, "cs_nodeCounts: numLeaves exceeds maxLeaves");
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const u32* leafOffsets = nullptr;
+    if (leafCounts) {
+        CS_TRY(enqueueExclusiveScan(ctx, leafCounts, ctx->leafOffFinal, numLeaves, s));
+        leafOffsets = ctx->leafOffFinal;
+    }
+    return enqueueNodeCounts(ctx, (const u64*)sortedKeys, n, (const u64*)prefixes, nullptr, numNodes, numNodes,
+                             leafOffsets, nodeToLeaf, nodeFirst, nodeCount, s);
+}
+
+cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                         uint32_t bucketSize, const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds,
+                         const cs_octree_buffers* b, cs_octree_sizes* sizes, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_buildOctree: ctx is null");
+    if (!x || !y || !z || !b || !sizes) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: null pointer");
+    if (!b->box6 || !b->keys || !b->perm || !b->leaves || !b->counts || !b->prefixes || !b->childOffsets ||
+        !b->levelRange || !b->nodeToLeaf || !b->nodeFirst || !b->nodeCount)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: a required output buffer is null");
+    if (n == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: n == 0");
+    if (bucketSize == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: bucketSize == 0");
+    if (b->leafCapacity == 0 || b->nodeCapacity == 0)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: zero capacity");
+    if (prevLeaves && prevNumLeaves == 0)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: prevLeaves given with prevNumLeaves == 0");
+    CS_TRY(checkParticles(ctx, "cs_buildOctree", n));
+    if (prevLeaves && (prevNumLeaves > ctx->maxLeaves || prevNumLeaves > b->leafCapacity))
+        return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctree: prevNumLeaves exceeds the leaf capacity");
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
+    const u32 nodeBound = b->nodeCapacity;
+
+    CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
+    CS_TRY(enqueueSortReset(ctx, s));
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, (u64*)b->keys, /*withHist=*/true, s));
+    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*histReady=*/true, s));
+    CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
+                         (u64*)b->leaves, b->counts, leafCap, s));
+    CS_TRY(enqueueLink(ctx, (const u64*)b->leaves, &ctx->ctrl->numLeaves, 0, leafCap, (u64*)b->prefixes, b->levels,
+                       b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity, s));
+    CS_TRY(enqueueNodeCounts(ctx, (const u64*)b->keys, n, (const u64*)b->prefixes, &ctx->ctrl->numNodes, 0, nodeBound,
+                             ctx->leafOffFinal, b->nodeToLeaf, b->nodeFirst, b->nodeCount, s));
+    CS_TRY(readCtrl(ctx, s));
+    const DeviceCtrl& c = ctx->hostCtrl->c;
+    sizes->rounds = c.rounds;
+    sizes->converged = c.converged;
+    const bool ok = (c.status == CS_OK || c.status == CS_ERR_NOT_CONVERGED);
+    sizes->numLeaves = ok ? c.numLeaves : 0;
+    sizes->numNodes = ok ? c.numNodes : 0;
+    return statusFromCtrl(ctx, "cs_buildOctree");
+}
+
+cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                             uint32_t bucketSize, const cs_octree_buffers* h, cs_octree_sizes* sizes, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_buildOctreeHost: ctx is null");
+    if (!x || !y || !z || !h || !sizes) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctreeHost: null pointer");
+    if (n == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctreeHost: n == 0");
+    CS_TRY(checkParticles(ctx, "cs_buildOctreeHost", n));
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    // context-owned device staging: sized once for the context's capacities
+    const size_t np = ctx->maxParticles, nlc = ctx->maxLeaves, nnc = ctx->maxNodes;
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = up(o + bytes); return at; };
+    const size_t oX = take(np * 8), oY = take(np * 8), oZ = take(np * 8), oBox = take(64), oKeys = take(np * 8),
+                 oPerm = take(np * 4), oLeaves = take((nlc + 1) * 8), oCounts = take(nlc * 4), oPre = take(nnc * 8),
+                 oLev = take(nnc * 4), oCO = take(nnc * 4), oPar = take(nnc * 4), oLR = take(256),
+                 oL2N = take(nlc * 4), oN2L = take(nnc * 4), oNF = take(nnc * 4), oNC = take(nnc * 4);
+    if (!ctx->hostPathSlab) {
+        CS_CUDA(ctx, cudaMalloc((void**)&ctx->hostPathSlab, o));
+        ctx->hostPathBytes = o;
+    }
+    char* d = ctx->hostPathSlab;
+    double* dx = (double*)(d + oX); double* dy = (double*)(d + oY); double* dz = (double*)(d + oZ);
+    CS_CUDA(ctx, cudaMemcpyAsync(dx, x, n * 8, cudaMemcpyHostToDevice, s));
+    CS_CUDA(ctx, cudaMemcpyAsync(dy, y, n * 8, cudaMemcpyHostToDevice, s));
+    CS_CUDA(ctx, cudaMemcpyAsync(dz, z, n * 8, cudaMemcpyHostToDevice, s));
+    cs_octree_buffers b{};
+    b.box6 = (double*)(d + oBox); b.keys = (uint64_t*)(d + oKeys); b.perm = (uint32_t*)(d + oPerm);
+    b.leaves = (uint64_t*)(d + oLeaves); b.counts = (uint32_t*)(d + oCounts); b.prefixes = (uint64_t*)(d + oPre);
+    b.levels = (uint32_t*)(d + oLev); b.childOffsets = (uint32_t*)(d + oCO); b.parents = (uint32_t*)(d + oPar);
+    b.levelRange = (uint32_t*)(d + oLR); b.leafToNode = (uint32_t*)(d + oL2N); b.nodeToLeaf = (uint32_t*)(d + oN2L);
+    b.nodeFirst = (uint32_t*)(d + oNF); b.nodeCount = (uint32_t*)(d + oNC);
+    b.leafCapacity = ctx->maxLeaves; b.nodeCapacity = ctx->maxNodes;
+    cs_status st = cs_buildOctree(ctx, dx, dy, dz, n, bucketSize, nullptr, 0, 0, &b, sizes, stream);
+    if (st != CS_OK) return st;
+    const size_t nl = sizes->numLeaves, nn = sizes->numNodes;
+    if ((h->leaves || h->counts || h->leafToNode) && nl > h->leafCapacity)
+        return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctreeHost: host leafCapacity too small");
+    if ((h->prefixes || h->childOffsets) && nn > h->nodeCapacity)
+        return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctreeHost: host nodeCapacity too small");
+    auto back = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
+        if (!dst || bytes == 0) return cudaSuccess;
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s);
+    };
+    CS_CUDA(ctx, back(h->box6, b.box6, 48));
+    CS_CUDA(ctx, back(h->keys, b.keys, n * 8));
+    CS_CUDA(ctx, back(h->perm, b.perm, n * 4));
+    CS_CUDA(ctx, back(h->leaves, b.leaves, (nl + 1) * 8));
+    CS_CUDA(ctx, back(h->counts, b.counts, nl * 4));
+    CS_CUDA(ctx, back(h->prefixes, b.prefixes, nn * 8));
+    CS_CUDA(ctx, back(h->levels, b.levels, nn * 4));
+    CS_CUDA(ctx, back(h->childOffsets, b.childOffsets, nn * 4));
+    CS_CUDA(ctx, back(h->parents, b.parents, nn * 4));
+    CS_CUDA(ctx, back(h->levelRange, b.levelRange, CS_NUM_LEVEL_OFFSETS * 4));
+    CS_CUDA(ctx, back(h->leafToNode, b.leafToNode, nl * 4));
+    CS_CUDA(ctx, back(h->nodeToLeaf, b.nodeToLeaf, nn * 4));
+    CS_CUDA(ctx, back(h->nodeFirst, b.nodeFirst, nn * 4));
+    CS_CUDA(ctx, back(h->nodeCount, b.nodeCount, nn * 4));
+    CS_CUDA(ctx, cudaStreamSynchronize(s));
+    return CS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,173 @@
+// Internal declarations shared by the translation units of libcornerstone_b200.so.
+// sm_100a only.  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/cornerstone.h"
+
+namespace cs {
+
+typedef unsigned long long u64;
+typedef unsigned int u32;
+
+constexpr int kL = 21;
+constexpr u64 kKeyEnd = 1ull << 63;          // 8^L
+constexpr int kMaxRounds = kL + 1;           // DESIGN.md A12
+constexpr int kRoundSlots = kMaxRounds + 2;
+
+// ---- radix sort geometry -------------------------------------------------------------
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kSortPasses = 8;               // 63 key bits, 8 bits per pass
+constexpr int kSortBlock = 512;
+constexpr int kSortItems = 15;
+constexpr int kSortTile = kSortBlock * kSortItems;   // 7680 keys per tile
+
+// ---- leaf refinement / link geometry -------------------------------------------------
+constexpr int kLeafBlock = 256;
+constexpr int kLeafItems = 4;
+constexpr int kLeafTile = kLeafBlock * kLeafItems;   // 1024 leaves per tile
+
+constexpr int kLinkBlock = 256;
+constexpr int kLinkItems = 4;
+constexpr int kLinkTile = kLinkBlock * kLinkItems;   // 1024 leaf boundaries per tile
+constexpr int kLinkBins = 2 * (kL + 1);              // per level: all nodes, internal nodes
+
+constexpr int kScanBlock = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanTile = kScanBlock * kScanItems;
+
+// Device-resident control block: every size the path produces stays here, so the whole
+// build can be enqueued without a host round trip.
+struct DeviceCtrl {
+    u32 nl[kRoundSlots];         // leaf count entering round r (nl[r+1] = after round r)
+    u32 ticket[kRoundSlots];     // tile tickets of round r
+    u32 tilesDone[kRoundSlots];
+    u32 changed[kRoundSlots];    // some O_i != 1 in round r
+    u32 done;                    // refinement finished (converged / maxRounds / error)
+    u32 rounds;                  // rounds performed
+    u32 converged;
+    u32 status;                  // cs_status of the device-side checks
+    u32 numLeaves;               // final leaf count
+    u32 numNodes;
+    u32 linkTicket;
+    u32 scanTicket;
+    u32 levelTotals[kLinkBins];  // link: nodes per level (all / internal)
+    u32 levelRange[kL + 2];
+    u32 pad[7];
+};
+
+struct HostCtrl {                // pinned mirror read back once per call
+    DeviceCtrl c;
+};
+
+}  // namespace cs
+
+struct cs_context {
+    int device = 0;
+    uint64_t maxParticles = 0;
+    uint32_t maxLeaves = 0;
+    uint32_t maxNodes = 0;
+    int numSMs = 148;
+
+    char* slab = nullptr;
+    size_t slabBytes = 0;
+
+    // sort
+    cs::u64* keysAlt = nullptr;
+    cs::u32* permAlt = nullptr;
+    cs::u32* sortHist = nullptr;       // [kSortPasses][kRadix] + kSortPasses tickets
+    cs::u32* sortTickets = nullptr;
+    cs::u64* sortLookback = nullptr;   // [tiles][kRadix]
+    cs::u32 epoch = 0;                 // look-back epoch, bumped per launch that uses a look-back array
+
+    // box
+    double* boxPartials = nullptr;     // [grid][6]
+    cs::u32* boxCounter = nullptr;
+
+    // leaves
+    cs::u64* leafK[2] = {nullptr, nullptr};
+    cs::u32* leafOff[2] = {nullptr, nullptr};
+    cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
+    cs::u64* tileLookback = nullptr;   // [tiles][kLinkBins] (also used by the scan and the leaf rounds)
+    cs::DeviceCtrl* ctrl = nullptr;
+    cs::HostCtrl* hostCtrl = nullptr;  // pinned
+
+    // buffers for cs_buildOctreeHost (allocated lazily)
+    char* hostPathSlab = nullptr;
+    size_t hostPathBytes = 0;
+
+    // profiling
+    bool profiling = false;
+    cudaEvent_t evBegin[CS_NUM_STAGES] = {};
+    cudaEvent_t evEnd[CS_NUM_STAGES] = {};
+    bool evUsed[CS_NUM_STAGES] = {};
+    uint64_t launches = 0;
+
+    std::string lastError;
+};
+
+namespace cs {
+
+// ---- error plumbing --------------------------------------------------------------------
+cs_status fail(cs_context* ctx, cs_status st, const char* fmt, ...);
+cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what);
+#define CS_CUDA(ctx, call)                                                     \
+    do {                                                                       \
+        cudaError_t e__ = (call);                                              \
+        if (e__ != cudaSuccess) return ::cs::cudaFail((ctx), e__, #call);      \
+    } while (0)
+#define CS_TRY(expr)                                   \
+    do {                                               \
+        cs_status s__ = (expr);                        \
+        if (s__ != CS_OK) return s__;                  \
+    } while (0)
+#define CS_LAUNCH_CHECK(ctx, name)                                             \
+    do {                                                                       \
+        (ctx)->launches++;                                                     \
+        cudaError_t e__ = cudaGetLastError();                                  \
+        if (e__ != cudaSuccess) return ::cs::cudaFail((ctx), e__, name);       \
+    } while (0)
+
+struct StageTimer {               // records CUDA events around a stage when profiling is on
+    cs_context* ctx; int stage; cudaStream_t s;
+    StageTimer(cs_context* c, int st, cudaStream_t stream) : ctx(c), stage(st), s(stream)
+    {
+        if (ctx->profiling) { cudaEventRecord(ctx->evBegin[stage], s); }
+    }
+    ~StageTimer()
+    {
+        if (ctx->profiling) { cudaEventRecord(ctx->evEnd[stage], s); ctx->evUsed[stage] = true; }
+    }
+};
+
+inline u32 divUp(u64 a, u64 b) { return (u32)((a + b - 1) / b); }
+u32 nextEpoch(cs_context* ctx, cudaStream_t s);
+
+// ---- stage enqueue functions (no synchronisation; sizes device-resident) ---------------
+cs_status enqueueBox(cs_context*, const double* x, const double* y, const double* z, u64 n, double* box6,
+                     cudaStream_t);
+// withHist: also accumulate the 8 digit histograms of the radix sort into ctx->sortHist
+cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
+                      u64* keys, bool withHist, cudaStream_t);
+cs_status enqueueSortReset(cs_context*, cudaStream_t);
+cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool histReady, cudaStream_t);
+cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
+                        u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity,
+                        cudaStream_t);
+// leaves/numLeaves: if dNumLeaves is null the host value is used
+cs_status enqueueLink(cs_context*, const u64* leaves, const u32* dNumLeaves, u32 hNumLeaves, u32 leafBound,
+                      u64* prefixes, u32* levels, u32* childOffsets, u32* parents, u32* levelRange,
+                      u32* leafToNode, u32* nodeToLeaf, u32 nodeCapacity, cudaStream_t);
+cs_status enqueueNodeCounts(cs_context*, const u64* sortedKeys, u64 n, const u64* prefixes, const u32* dNumNodes,
+                            u32 hNumNodes, u32 nodeBound, const u32* leafOffsets, const u32* nodeToLeaf,
+                            u32* nodeFirst, u32* nodeCount, cudaStream_t);
+// device-wide exclusive scan of u32 (decoupled look-back): out[i] = sum_{j<i} in[j], out[n] = total
+cs_status enqueueExclusiveScan(cs_context*, const u32* in, u32* out, u32 n, cudaStream_t);
+cs_status readCtrl(cs_context*, cudaStream_t);   // D2H of the control block + stream sync
+
+}  // namespace cs

@@ -1,0 +1,254 @@
+// H4-H8: cornerstone leaf array by iterating f and g = g3 o g2 o g1 (Eqs. 2-9).
+//
+// One kernel launch per round does all of f, g1, g2, g3:
+//   f   (Eq. 3)  the lower-bound position off_i of every K_i in P is carried with K from round to
+//                round; N_i = off_{i+1} - off_i.  Only the 7 new boundaries of a split leaf are
+//                searched, inside the parent's particle range [off_i, off_{i+1}).
+//   g1  (Eq. 5)  O_i in {8, 0, 1} per leaf (readings A7, A8, A9).
+//   g2  (Eq. 6)  exclusive prefix sum of O: in-tile scan + decoupled look-back across tiles.
+//   g3  (Eqs. 7-9, A10, A11) scatter of kept keys / 8 child keys to K'.
+// All sizes stay in the device control block; round r reads nl[r] and writes nl[r+1], so the
+// host can enqueue the maximum number of rounds without reading anything back: rounds after
+// convergence return at once (ctrl->done).
+#include "cs_device.cuh"
+
+namespace cs {
+
+__device__ __forceinline__ u32 ldVolatile(const u32* p) { return *(const volatile u32*)p; }
+
+// ---- start arrays -----------------------------------------------------------------------------
+__global__ void leavesInitRootKernel(DeviceCtrl* ctrl, u64* K0, u32* off0, u32 n)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        K0[0] = 0;
+        K0[1] = kKeyEnd;
+        off0[0] = 0;
+        off0[1] = n;
+        ctrl->nl[0] = 1;
+    }
+}
+
+// Copy the caller's previous cornerstone array into the workspace, check Eq. 2
+// and locate every K_i in P (the full f of the first incremental round).
+__global__ void __launch_bounds__(256) leavesInitPrevKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n,
+                                                            const u64* __restrict__ prev, u32 nlPrev, u64* K0,
+                                                            u32* off0)
+{
+    const u32 stride = gridDim.x * blockDim.x;
+    bool bad = false;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i <= nlPrev; i += stride) {
+        const u64 k = prev[i];
+        if (i == 0 && k != 0) bad = true;
+        if (i == nlPrev) {
+            if (k != kKeyEnd) bad = true;
+            off0[i] = n;
+        } else {
+            const u64 kn = prev[i + 1];
+            const u64 delta = kn - k;
+            if (kn <= k || !isPowerOf8(delta) || (k & (delta - 1))) bad = true;
+            off0[i] = lowerBound(P, 0, n, k);
+        }
+        K0[i] = k;
+    }
+    if (bad) {
+        ctrl->status = CS_ERR_NOT_CORNERSTONE;
+        ctrl->done = 1;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->nl[0] = nlPrev;
+}
+
+// ---- one round ----------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kLeafBlock)
+    leafRoundKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const u64* __restrict__ Kin,
+                    const u32* __restrict__ offIn, u64* __restrict__ Kout, u32* __restrict__ offOut, u64* lookback,
+                    u32 epoch, u32 r, u32 bucket, u32 cap, u32 lastRound)
+{
+    __shared__ u32 sTile, sPrefix, sDone;
+    __shared__ u32 warpSums[kLeafBlock / 32 + 1];
+    if (threadIdx.x == 0) sDone = ldVolatile(&ctrl->done);   // one read per CTA: the decision must be uniform
+    __syncthreads();
+    if (sDone) return;
+    const u32 nl = ctrl->nl[r];
+    const u32 tiles = (nl + kLeafTile - 1) / kLeafTile;
+    const u32 tid = threadIdx.x;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) sTile = atomicAdd(&ctrl->ticket[r], 1u);
+        __syncthreads();
+        const u32 tile = sTile;
+        if (tile >= tiles) break;
+        const u32 first = tile * kLeafTile + tid * kLeafItems;
+
+        u64 K[kLeafItems + 1];
+        u32 off[kLeafItems + 1];
+#pragma unroll
+        for (int k = 0; k <= kLeafItems; ++k) {
+            u32 i = first + k;
+            K[k] = i <= nl ? Kin[i] : kKeyEnd;
+            off[k] = i <= nl ? offIn[i] : n;
+        }
+        // g1: rebalance decision (Eq. 5)
+        u32 O[kLeafItems];
+        u32 sum = 0;
+        bool anyChange = false;
+#pragma unroll
+        for (int k = 0; k < kLeafItems; ++k) {
+            const u32 i = first + k;
+            u32 o = 0;
+            if (i < nl) {
+                const u64 delta = K[k + 1] - K[k];
+                const u32 cnt = off[k + 1] - off[k];                      // f: N_i
+                o = 1;
+                if (cnt > bucket && delta > 1) o = 8;                    // split (A7: not at depth L)
+                else if (delta != kKeyEnd) {                             // the root never merges (A9)
+                    const u32 j = (u32)(K[k] / delta) & 7u;              // octant index among siblings
+                    if (j != 0 && i >= j && i - j + 8 <= nl) {
+                        const u32 a = i - j;
+                        if (Kin[a + 8] - Kin[a] == (delta << 3)) {       // all 8 siblings are leaves
+                            const u32 combined = offIn[a + 8] - offIn[a];
+                            if (combined <= bucket) o = 0;               // merged away (A8)
+                        }
+                    }
+                }
+                anyChange |= (o != 1);
+            }
+            O[k] = o;
+            sum += o;
+        }
+        // g2: exclusive prefix sum (Eq. 6): tile scan + look-back
+        u32 total;
+        const u32 excl = blockExclusiveScan<kLeafBlock>(sum, warpSums, &total);
+        if (tid == 0) {
+            u64* st = lookback + tile;
+            u32 p = 0;
+            if (tile == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
+            else {
+                lbStore(st, lbPack(epoch, kLbAggregate, total));
+                p = lbLookBack(lookback, 1, 0, tile, epoch);
+                lbStore(st, lbPack(epoch, kLbPrefix, p + total));
+            }
+            sPrefix = p;
+        }
+        const int tileChanged = __syncthreads_or(anyChange ? 1 : 0);
+        // g3: node rebalancing (Eqs. 8, 9); children's off by binary search in the parent's range
+        u32 p = sPrefix + excl;
+#pragma unroll
+        for (int k = 0; k < kLeafItems; ++k) {
+            if (O[k] == 1) {
+                if (p < cap) {
+                    Kout[p] = K[k];
+                    offOut[p] = off[k];
+                }
+                p += 1;
+            } else if (O[k] == 8) {
+                const u64 step = (K[k + 1] - K[k]) >> 3;
+                u32 lo = off[k];
+                const u32 hi = off[k + 1];
+#pragma unroll 1
+                for (u32 c = 0; c < 8; ++c) {
+                    const u64 key = K[k] + c * step;
+                    if (c) lo = lowerBound(P, lo, hi, key);
+                    if (p + c < cap) {
+                        Kout[p + c] = key;
+                        offOut[p + c] = lo;
+                    }
+                }
+                p += 8;
+            }
+        }
+        if (tid == 0) {
+            const u32 newTotal = sPrefix + total;
+            if (tile == tiles - 1) {                         // A11: terminal element of K'
+                if (newTotal <= cap) {
+                    Kout[newTotal] = kKeyEnd;
+                    offOut[newTotal] = n;
+                }
+                ctrl->nl[r + 1] = newTotal;
+            }
+            if (tileChanged) atomicOr(&ctrl->changed[r], 1u);
+            __threadfence();
+            const u32 finished = atomicAdd(&ctrl->tilesDone[r], 1u) + 1u;
+            if (finished == tiles) {                         // last tile to finish closes the round
+                __threadfence();
+                const u32 nlNew = ldVolatile(&ctrl->nl[r + 1]);
+                const u32 ch = ldVolatile(&ctrl->changed[r]);
+                ctrl->rounds = r + 1;
+                if (nlNew > cap) {
+                    ctrl->status = CS_ERR_CAPACITY;
+                    ctrl->done = 1;
+                } else {
+                    ctrl->numLeaves = nlNew;
+                    ctrl->converged = ch ? 0u : 1u;
+                    if (!ch) ctrl->done = 1;                 // O_i = 1 for all i
+                    else if (r == lastRound) {
+                        ctrl->status = CS_ERR_NOT_CONVERGED;
+                        ctrl->done = 1;
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ---- hand the result to the caller: leaves, counts (f of the returned K), and off[] ---------------
+__global__ void __launch_bounds__(256) leavesEmitKernel(const DeviceCtrl* ctrl, const u64* K0, const u64* K1,
+                                                        const u32* off0, const u32* off1, u64* leaves, u32* counts,
+                                                        u32* offFinal)
+{
+    const u32 st = ctrl->status;
+    if (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) return;   // outputs untouched
+    const u32 rounds = ctrl->rounds;
+    const u32 nl = ctrl->nl[rounds];
+    const u64* K = (rounds & 1) ? K1 : K0;
+    const u32* off = (rounds & 1) ? off1 : off0;
+    const u32 stride = gridDim.x * blockDim.x;
+    for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i <= nl; i += stride) {
+        const u32 o = off[i];
+        leaves[i] = K[i];
+        offFinal[i] = o;
+        if (i < nl && counts) counts[i] = off[i + 1] - o;
+    }
+}
+
+cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const u64* prevLeaves, u32 prevNumLeaves,
+                        u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, cudaStream_t s)
+{
+    StageTimer t(ctx, CS_STAGE_LEAVES, s);
+    const u32 cap = leafCapacity < ctx->maxLeaves ? leafCapacity : ctx->maxLeaves;
+    DeviceCtrl* ctrl = ctx->ctrl;
+    CS_CUDA(ctx, cudaMemsetAsync(ctrl, 0, sizeof(DeviceCtrl), s));
+    const u32 persistentGrid = (u32)ctx->numSMs * 8;
+    if (prevLeaves) {
+        u32 grid = divUp((u64)prevNumLeaves + 1, 256);
+        if (grid > persistentGrid) grid = persistentGrid;
+        leavesInitPrevKernel<<<grid, 256, 0, s>>>(ctrl, P, (u32)n, prevLeaves, prevNumLeaves, ctx->leafK[0],
+                                                  ctx->leafOff[0]);
+        CS_LAUNCH_CHECK(ctx, "leavesInitPrevKernel");
+    } else {
+        leavesInitRootKernel<<<1, 32, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafOff[0], (u32)n);
+        CS_LAUNCH_CHECK(ctx, "leavesInitRootKernel");
+    }
+    const u32 roundsToLaunch = (maxRounds == 0 || maxRounds > (u32)kMaxRounds) ? (u32)kMaxRounds : maxRounds;
+    // grid: enough CTAs for the largest array this context can hold, capped at a persistent size
+    u32 grid = divUp((u64)cap + 1, kLeafTile);
+    if (grid > persistentGrid) grid = persistentGrid;
+    for (u32 r = 0; r < roundsToLaunch; ++r) {
+        const u32 epoch = nextEpoch(ctx, s);
+        // early rounds from the root touch at most 8^r leaves: do not launch more CTAs than that
+        u32 g = grid;
+        if (!prevLeaves && r < 8) {
+            u32 bound = divUp(1ull << (3 * r), kLeafTile);
+            if (bound < g) g = bound;
+        }
+        leafRoundKernel<<<g, kLeafBlock, 0, s>>>(ctrl, P, (u32)n, ctx->leafK[r & 1], ctx->leafOff[r & 1],
+                                                 ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
+                                                 ctx->tileLookback, epoch, r, bucket, cap, roundsToLaunch - 1);
+        CS_LAUNCH_CHECK(ctx, "leafRoundKernel");
+    }
+    leavesEmitKernel<<<grid, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafK[1], ctx->leafOff[0], ctx->leafOff[1],
+                                          leaves, counts, ctx->leafOffFinal);
+    CS_LAUNCH_CHECK(ctx, "leavesEmitKernel");
+    return CS_OK;
+}
+
+}  // namespace cs

@@ -1,0 +1,280 @@
+// H1 bounding box and H2 Morton keys (readings A1-A3).
+// Both are single streaming passes over the SoA coordinates: HBM-bound, 128-bit loads,
+// persistent grid sized in multiples of the SM count.
+#include "cs_device.cuh"
+
+namespace cs {
+
+constexpr int kBoxBlock = 512;
+constexpr int kBoxBlocksPerSM = 4;
+constexpr int kKeysBlock = 256;
+constexpr int kKeysBlocksPerSM = 8;
+
+// ---------------------------------------------------------------------------------------------
+// H1: per-dimension min / max.  Each CTA reduces a grid-strided slice, writes 6 partials, and
+// the last CTA to finish (atomic counter) folds the partials into box6.  min/max of finite
+// doubles is exact and order independent, so any reduction tree gives the oracle's bits
+// (a zero extreme is canonicalised to +0.0 on both sides, A1).
+// ---------------------------------------------------------------------------------------------
+struct MinMax3 {
+    double lo[3], hi[3];
+};
+
+__device__ __forceinline__ void mmInit(MinMax3& m)
+{
+    const double inf = __longlong_as_double(0x7FF0000000000000ll);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { m.lo[d] = inf; m.hi[d] = -inf; }
+}
+__device__ __forceinline__ void mmAdd(MinMax3& m, int d, double v)
+{
+    m.lo[d] = fmin(m.lo[d], v);
+    m.hi[d] = fmax(m.hi[d], v);
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(kBoxBlock) boxKernel(const double* __restrict__ x, const double* __restrict__ y,
+                                                       const double* __restrict__ z, u64 n, double* partials,
+                                                       u32* counter, double* box6)
+{
+    MinMax3 m;
+    mmInit(m);
+    const double* c[3] = {x, y, z};
+    const u64 tid = (u64)blockIdx.x * kBoxBlock + threadIdx.x;
+    const u64 nthreads = (u64)gridDim.x * kBoxBlock;
+    if (VEC) {
+        const u64 pairs = n >> 1;
+        u64 i = tid;
+        // 2 iterations x 3 dims x 16 B = 96 B in flight per thread
+        for (; i + nthreads < pairs; i += 2 * nthreads) {
+            double2 a[3], b[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                a[d] = ldStreamD2(c[d] + 2 * i);
+                b[d] = ldStreamD2(c[d] + 2 * (i + nthreads));
+            }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                mmAdd(m, d, a[d].x); mmAdd(m, d, a[d].y);
+                mmAdd(m, d, b[d].x); mmAdd(m, d, b[d].y);
+            }
+        }
+        for (; i < pairs; i += nthreads) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double2 a = ldStreamD2(c[d] + 2 * i);
+                mmAdd(m, d, a.x); mmAdd(m, d, a.y);
+            }
+        }
+        if ((n & 1) && tid == 0) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) mmAdd(m, d, c[d][n - 1]);
+        }
+    } else {
+        for (u64 i = tid; i < n; i += nthreads) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) mmAdd(m, d, ldStreamD(c[d] + i));
+        }
+    }
+    // warp reduce
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            m.lo[d] = fmin(m.lo[d], __shfl_xor_sync(kFull, m.lo[d], o));
+            m.hi[d] = fmax(m.hi[d], __shfl_xor_sync(kFull, m.hi[d], o));
+        }
+    }
+    __shared__ double sRed[kBoxBlock / 32][6];
+    __shared__ bool sLast;
+    const u32 warp = threadIdx.x >> 5, lane = laneId();
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { sRed[warp][2 * d] = m.lo[d]; sRed[warp][2 * d + 1] = m.hi[d]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = sRed[0][threadIdx.x];
+        for (int w = 1; w < kBoxBlock / 32; ++w)
+            v = (threadIdx.x & 1) ? fmax(v, sRed[w][threadIdx.x]) : fmin(v, sRed[w][threadIdx.x]);
+        partials[(size_t)blockIdx.x * 6 + threadIdx.x] = v;
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sLast = (atomicAdd(counter, 1u) + 1u == gridDim.x);
+    __syncthreads();
+    if (!sLast) return;
+    __threadfence();
+    // last CTA: fold gridDim.x partials
+    const double inf = __longlong_as_double(0x7FF0000000000000ll);
+    double acc[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) acc[q] = (q & 1) ? -inf : inf;
+    for (u32 b = threadIdx.x; b < gridDim.x; b += kBoxBlock) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            double v = ((volatile double*)partials)[(size_t)b * 6 + q];
+            acc[q] = (q & 1) ? fmax(acc[q], v) : fmin(acc[q], v);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            double t = __shfl_xor_sync(kFull, acc[q], o);
+            acc[q] = (q & 1) ? fmax(acc[q], t) : fmin(acc[q], t);
+        }
+    }
+    __syncthreads();
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) sRed[warp][q] = acc[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = sRed[0][threadIdx.x];
+        for (int w = 1; w < kBoxBlock / 32; ++w)
+            v = (threadIdx.x & 1) ? fmax(v, sRed[w][threadIdx.x]) : fmin(v, sRed[w][threadIdx.x]);
+        box6[threadIdx.x] = __dadd_rn(v, 0.0);   // -0.0 -> +0.0 (A1)
+    }
+    if (threadIdx.x == 0) *counter = 0;          // ready for the next call
+}
+
+cs_status enqueueBox(cs_context* ctx, const double* x, const double* y, const double* z, u64 n, double* box6,
+                     cudaStream_t s)
+{
+    StageTimer t(ctx, CS_STAGE_BOX, s);
+    const bool vec = ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z)) & 15u) == 0;
+    u64 work = vec ? (n + 1) / 2 : n;
+    u32 grid = (u32)ctx->numSMs * kBoxBlocksPerSM;
+    u32 need = divUp(work, kBoxBlock);
+    if (need < grid) grid = need ? need : 1;
+    if (vec) boxKernel<true><<<grid, kBoxBlock, 0, s>>>(x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
+    else boxKernel<false><<<grid, kBoxBlock, 0, s>>>(x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
+    CS_LAUNCH_CHECK(ctx, "boxKernel");
+    return CS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// H2: Morton keys.  g = clamp(floor(((c - lo) / e) * 2^21), 0, 2^21 - 1) with explicitly
+// rounded intrinsics (__dsub_rn, __ddiv_rn, __dmul_rn are never contracted into FMAs), then
+// the 21 bits of each coordinate are spread to every third bit with 5 shift-or-mask steps.
+// cvt.rmi.s64.f64 saturates and maps NaN (0/0 of a flat box) to 0, which is reading A1.
+// Optionally (HIST) the 8 radix-digit histograms of the sort are accumulated on the fly,
+// saving the sort a pass over the keys.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ u64 spread21(u64 v)
+{
+    v &= 0x1fffffull;
+    v = (v | (v << 32)) & 0x001f00000000ffffull;
+    v = (v | (v << 16)) & 0x001f0000ff0000ffull;
+    v = (v | (v << 8)) & 0x100f00f00f00f00full;
+    v = (v | (v << 4)) & 0x10c30c30c30c30c3ull;
+    v = (v | (v << 2)) & 0x1249249249249249ull;
+    return v;
+}
+
+__device__ __forceinline__ u64 gridCoordinate(double c, double lo, double e)
+{
+    double t = __dmul_rn(__ddiv_rn(__dsub_rn(c, lo), e), 2097152.0);
+    long long g = __double2ll_rd(t);
+    g = g < 0 ? 0 : g;
+    g = g > 2097151 ? 2097151 : g;
+    return (u64)g;
+}
+
+struct BoxParams {
+    double lo[3], e[3];
+};
+
+__device__ __forceinline__ u64 mortonKey(double x, double y, double z, const BoxParams& b)
+{
+    u64 gx = gridCoordinate(x, b.lo[0], b.e[0]);
+    u64 gy = gridCoordinate(y, b.lo[1], b.e[1]);
+    u64 gz = gridCoordinate(z, b.lo[2], b.e[2]);
+    return (spread21(gx) << 2) | (spread21(gy) << 1) | spread21(gz);   // digit = 4x + 2y + z (A3)
+}
+
+template <bool HIST>
+__device__ __forceinline__ void histAdd(u32* sh, u64 key)
+{
+    if (HIST) {
+#pragma unroll
+        for (int p = 0; p < kSortPasses; ++p)
+            atomicAdd(&sh[p * kRadix + (u32)((key >> (p * kRadixBits)) & (kRadix - 1))], 1u);
+    }
+}
+
+template <bool VEC, bool HIST>
+__global__ void __launch_bounds__(kKeysBlock) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
+                                                         const double* __restrict__ z, u64 n,
+                                                         const double* __restrict__ box6, u64* __restrict__ keys,
+                                                         u32* gHist)
+{
+    __shared__ u32 sh[HIST ? kSortPasses * kRadix : 1];
+    if (HIST) {
+        for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) sh[i] = 0;
+        __syncthreads();
+    }
+    BoxParams b;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        b.lo[d] = box6[2 * d];
+        b.e[d] = __dsub_rn(box6[2 * d + 1], box6[2 * d]);
+    }
+    const u64 tid = (u64)blockIdx.x * kKeysBlock + threadIdx.x;
+    const u64 nthreads = (u64)gridDim.x * kKeysBlock;
+    if (VEC) {
+        const u64 pairs = n >> 1;
+        for (u64 i = tid; i < pairs; i += nthreads) {
+            double2 vx = ldStreamD2(x + 2 * i);
+            double2 vy = ldStreamD2(y + 2 * i);
+            double2 vz = ldStreamD2(z + 2 * i);
+            u64 k0 = mortonKey(vx.x, vy.x, vz.x, b);
+            u64 k1 = mortonKey(vx.y, vy.y, vz.y, b);
+            stStreamU2(keys + 2 * i, k0, k1);
+            histAdd<HIST>(sh, k0);
+            histAdd<HIST>(sh, k1);
+        }
+        if ((n & 1) && tid == 0) {
+            u64 k = mortonKey(x[n - 1], y[n - 1], z[n - 1], b);
+            keys[n - 1] = k;
+            histAdd<HIST>(sh, k);
+        }
+    } else {
+        for (u64 i = tid; i < n; i += nthreads) {
+            u64 k = mortonKey(ldStreamD(x + i), ldStreamD(y + i), ldStreamD(z + i), b);
+            keys[i] = k;
+            histAdd<HIST>(sh, k);
+        }
+    }
+    if (HIST) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) {
+            u32 v = sh[i];
+            if (v) atomicAdd(&gHist[i], v);
+        }
+    }
+}
+
+cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const double* z, u64 n, const double* box6,
+                      u64* keys, bool withHist, cudaStream_t s)
+{
+    StageTimer t(ctx, CS_STAGE_KEYS, s);
+    if (n == 0) return CS_OK;
+    const bool vec =
+        ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z) | ((uintptr_t)keys)) & 15u) == 0;
+    u64 work = vec ? (n + 1) / 2 : n;
+    u32 grid = (u32)ctx->numSMs * kKeysBlocksPerSM;
+    u32 need = divUp(work, kKeysBlock);
+    if (need < grid) grid = need ? need : 1;
+    u32* h = ctx->sortHist;
+    if (vec && withHist) keysKernel<true, true><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
+    else if (vec) keysKernel<true, false><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
+    else if (withHist) keysKernel<false, true><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
+    else keysKernel<false, false><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
+    CS_LAUNCH_CHECK(ctx, "keysKernel");
+    return CS_OK;
+}
+
+}  // namespace cs
