@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py -- full cornerstone octree build throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4]
+
+A "step" is one pass of the whole hot path (bounding box -> Morton keys -> stable radix sort
+-> leaf refinement from {0, 8^21} -> linked octree -> node counts) over one batch of synthetic
+particles, through cs_buildOctree (one C-ABI call, one synchronisation).  The N=1 workload is
+BASELINE.json's headline configuration (configs[3]: N = 2^26, Gaussian blobs + background,
+bucketSize 64).  Prints ONE JSON line (rank 0).
+
+--impl reference times the CPU oracle (oracle/, single core, as it stands) on a bounded sample
+of the same workload: a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "Mparticles/s full octree build"
+UNIT = "Mparticles/s"
+# algorithmic bytes per particle: box 24 + keys 32 + sort 196
+MODEL_BYTES_PER_PARTICLE = 252
+# dominant kernel: one radix pass reads 12 B and writes 12 B per particle (pass 0 reads 8): mean over 8 passes
+SORT_PASS_BYTES_PER_PARTICLE = (20 + 7 * 24) / 8.0
+NOMINAL_HBM_GBS = 8000.0
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _traffic():
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full summary."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self._stop = threading.Event()
+        self._t = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            if len(r) < 6:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _workload(name: str):
+    from paper_2307_06345_b200 import workloads as W
+    table = {"c1": W.CONFIGS[0], "c2": W.CONFIGS[1], "c3": W.CONFIGS[2], "c4": W.CONFIGS[3], "c5": W.CONFIGS[4]}
+    return table[name]
+
+
+def _oracle_sample(cfg, sample_n: int, bucket: int, seed_shift: int = 0):
+    """Time the oracle, as it stands, on a bounded sample of the workload (single core)."""
+    import oracle
+    x, y, z = cfg.generate(sample_n)
+    t0 = time.perf_counter()
+    ref = oracle.full_build(x, y, z, bucket)
+    dt = time.perf_counter() - t0
+    return dt, ref["leaves"].size - 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = _workload(args.workload)
+    bucket = cfg.bucket_sizes[-1]
+    sample_n = min(cfg.n, args.ref_sample)
+    for _ in range(args.warmup):
+        _oracle_sample(cfg, min(sample_n, 1 << 18), bucket)
+    t = []
+    for _ in range(args.steps):
+        dt, _ = _oracle_sample(cfg, sample_n, bucket)
+        t.append(dt)
+    total = sum(t)
+    value = sample_n * args.steps / total / 1e6
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_particles": cfg.n, "bucketSize": bucket,
+                   "sample": f"first {sample_n} particles of the same recipe per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"{sample_n} particles of {cfg.name}, full path, per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2307_06345_b200 import binding as cs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = _workload(args.workload)
+    n = cfg.n if args.n is None else args.n
+    bucket = cfg.bucket_sizes[-1]
+    # replicas only: every rank builds its own tree on its own particle set
+    cfg_rank = cfg
+    if rank:
+        import dataclasses
+        cfg_rank = dataclasses.replace(cfg, seed=cfg.seed + 7919 * rank)
+    x, y, z = cfg_rank.generate(n)
+    in_sum = None
+    if rank == 0:
+        from paper_2307_06345_b200.workloads import checksum
+        in_sum = checksum(x[: 1 << 20], y[: 1 << 20], z[: 1 << 20])
+    hx, hy, hz = (torch.from_numpy(a).pin_memory() for a in (x, y, z))
+    dx, dy, dz = (t.cuda(non_blocking=True) for t in (hx, hy, hz))
+    max_leaves = max(1 << 12, n // 4)
+    ctx = cs.Context(max_particles=n, max_leaves=max_leaves, device=local_rank)
+    bufs = cs.TreeBuffers(ctx, n)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up ---------------------------------------------------------------------------
+    ctx.setProfiling(True)
+    for _ in range(max(args.warmup, 1)):
+        tree = cs.buildOctree(ctx, dx, dy, dz, bucket, buffers=bufs)
+    barrier()
+
+    # ---- timed region: K full builds, inputs resident in HBM ---------------------------------
+    stages = {k: 0.0 for k in cs.STAGE_NAMES}
+    launches0 = ctx.stageTimes()["launches"]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev0.record()
+        for _ in range(args.steps):
+            tree = cs.buildOctree(ctx, dx, dy, dz, bucket, buffers=bufs)
+            st = ctx.stageTimes()                 # events already complete: the call synchronised
+            for k in cs.STAGE_NAMES:
+                stages[k] += st[k]
+        ev1.record()
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = ctx.stageTimes()["launches"] - launches0
+    if world > 1:
+        tmax = torch.tensor([ms], device="cuda")
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
+    ms_per_step = ms / args.steps
+    value = n * world / (ms_per_step * 1e-3) / 1e6
+    stages = {k: v / args.steps for k, v in stages.items()}
+
+    # ---- end to end: HOST buffers through cs_buildOctreeHost, copies inside the timed region ---
+    e2e = None
+    if not args.no_e2e:
+        hb = cs.HostBuffers(n, max_leaves)
+        e2e_steps = max(1, min(args.steps, 3))
+        cs.buildOctreeHost(ctx, hx, hy, hz, bucket, hb)      # warm-up (allocates the staging slab)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            sz = cs.buildOctreeHost(ctx, hx, hy, hz, bucket, hb)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / e2e_steps
+        if world > 1:
+            tmax = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+            dt = float(tmax.item())
+        e2e = {"value": n * world / dt / 1e6, "unit": UNIT, "h2d_bytes_per_step": 24 * n,
+               "d2h_bytes_per_step": hb.bytes_back(n, sz["numLeaves"], sz["numNodes"]),
+               "ms_per_step": dt * 1e3, "steps": e2e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (radix pass), timed live with CUDA events -------------
+    peak, peak_src = _peaks()
+    pass_ms = stages["sort_passes"] / 8.0
+    pass_bytes = SORT_PASS_BYTES_PER_PARTICLE * n
+    achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+    tr = _traffic()
+    roofline = {"bound": "hbm", "kernel": "onesweepKernel (one 8-bit radix pass over u64 key + u32 index)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": (tr or {}).get("onesweep_dram_bytes_per_launch"), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": pass_bytes, "avg_launch_ms": pass_ms, "launches_per_step": 8}
+    model_bytes = MODEL_BYTES_PER_PARTICLE * n
+    full_build = {"model_bytes": model_bytes, "model_gbs": model_bytes / (ms_per_step * 1e-3) / 1e9,
+                  "frac_of_nominal_8TBs": model_bytes / (ms_per_step * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+                  "frac_of_measured_peak": model_bytes / (ms_per_step * 1e-3) / 1e9 / peak}
+
+    # ---- CPU baseline: the oracle as it stands, one core, bounded sample ---------------------
+    cpu = None
+    if not args.no_cpu:
+        sample_n = min(n, args.cpu_sample)
+        dt, _ = _oracle_sample(cfg, sample_n, bucket)
+        cpu = {"value": sample_n / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"first {sample_n} particles of {cfg.name} (same recipe), full path once, {dt:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_particles": n, "bucketSize": bucket, "leaves": tree["numLeaves"],
+                   "nodes": tree["numNodes"], "rounds": tree["rounds"], "parallelism": "replicas only",
+                   "l2": "inputs larger than L2 (1.5 GiB of coordinates per step at N=2^26)",
+                   "input_checksum_first_1Mi": in_sum},
+        "roofline": roofline, "full_build": full_build, "cpu_baseline": cpu, "e2e": e2e,
+        "gpu_launches": int(launches), "stages_ms": stages, "clocks": clocks.summary(),
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--n", type=int, default=None, help="override the particle count (same recipe)")
+    ap.add_argument("--cpu-sample", type=int, default=1 << 24)
+    ap.add_argument("--ref-sample", type=int, default=1 << 22)
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
