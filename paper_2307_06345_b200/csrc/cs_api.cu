@@ -123,7 +123,7 @@ cs_status cs_linkOctree(cs_context* ctx, const uint64_t* leaves, uint32_t numLea
     cudaStream_t s = (cudaStream_t)stream;
     CS_CUDA(ctx, cudaMemsetAsync(&ctx->ctrl->status, 0, sizeof(u32), s));
     CS_TRY(enqueueLink(ctx, (const u64*)leaves, nullptr, numLeaves, numLeaves, (u64*)prefixes, levels, childOffsets,
-                       parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity, s));
+                       parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity, nullptr, nullptr, nullptr, s));
     CS_TRY(readCtrl(ctx, s));
     *numNodes = ctx->hostCtrl->c.status == CS_OK ? ctx->hostCtrl->c.numNodes : 0;
     return statusFromCtrl(ctx, "cs_linkOctree");
@@ -174,7 +174,6 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     DeviceGuard g(ctx->device);
     cudaStream_t s = (cudaStream_t)stream;
     const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
-    const u32 nodeBound = b->nodeCapacity;
 
     CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
@@ -182,10 +181,10 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*histReady=*/true, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
                          (u64*)b->leaves, b->counts, leafCap, s));
+    // link and node counts in one pass: the leaves' particle offsets are still in the workspace
     CS_TRY(enqueueLink(ctx, (const u64*)b->leaves, &ctx->ctrl->numLeaves, 0, leafCap, (u64*)b->prefixes, b->levels,
-                       b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity, s));
-    CS_TRY(enqueueNodeCounts(ctx, (const u64*)b->keys, n, (const u64*)b->prefixes, &ctx->ctrl->numNodes, 0, nodeBound,
-                             ctx->leafOffFinal, b->nodeToLeaf, b->nodeFirst, b->nodeCount, s));
+                       b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,
+                       ctx->leafOffFinal, b->nodeFirst, b->nodeCount, s));
     CS_TRY(readCtrl(ctx, s));
     const DeviceCtrl& c = ctx->hostCtrl->c;
     sizes->rounds = c.rounds;

@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, tileLookback, ctrl, total;
+        leafOffFinal, leafTasks, tileLookback, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -53,6 +53,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafOff0 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOff1 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOffFinal = take(((size_t)maxLeaves + 2) * sizeof(u32));
+    L.leafTasks = take(((size_t)maxLeaves / 8 + 8) * sizeof(uint2));
     L.tileLookback = take(leafTiles * kLinkBins * sizeof(u64));
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
@@ -199,6 +200,8 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->leafOff[0] = (u32*)(ctx->slab + L.leafOff0);
     ctx->leafOff[1] = (u32*)(ctx->slab + L.leafOff1);
     ctx->leafOffFinal = (u32*)(ctx->slab + L.leafOffFinal);
+    ctx->leafTasks = (uint2*)(ctx->slab + L.leafTasks);
+    ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
     *out = ctx;

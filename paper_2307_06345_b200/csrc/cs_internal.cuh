@@ -48,6 +48,7 @@ struct DeviceCtrl {
     u32 ticket[kRoundSlots];     // tile tickets of round r
     u32 tilesDone[kRoundSlots];
     u32 changed[kRoundSlots];    // some O_i != 1 in round r
+    u32 taskCount[kRoundSlots];  // split leaves of round r (search tasks)
     u32 done;                    // refinement finished (converged / maxRounds / error)
     u32 rounds;                  // rounds performed
     u32 converged;
@@ -92,6 +93,8 @@ struct cs_context {
     // leaves
     cs::u64* leafK[2] = {nullptr, nullptr};
     cs::u32* leafOff[2] = {nullptr, nullptr};
+    uint2* leafTasks = nullptr;        // (first child slot, end of the parent's particle range) per split leaf
+    cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
     cs::u64* tileLookback = nullptr;   // [tiles][kLinkBins] (also used by the scan and the leaf rounds)
     cs::DeviceCtrl* ctrl = nullptr;
@@ -162,7 +165,8 @@ cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSiz
 // leaves/numLeaves: if dNumLeaves is null the host value is used
 cs_status enqueueLink(cs_context*, const u64* leaves, const u32* dNumLeaves, u32 hNumLeaves, u32 leafBound,
                       u64* prefixes, u32* levels, u32* childOffsets, u32* parents, u32* levelRange,
-                      u32* leafToNode, u32* nodeToLeaf, u32 nodeCapacity, cudaStream_t);
+                      u32* leafToNode, u32* nodeToLeaf, u32 nodeCapacity, const u32* leafOffsets /*nullable*/,
+                      u32* nodeFirst, u32* nodeCount, cudaStream_t);
 cs_status enqueueNodeCounts(cs_context*, const u64* sortedKeys, u64 n, const u64* prefixes, const u32* dNumNodes,
                             u32 hNumNodes, u32 nodeBound, const u32* leafOffsets, const u32* nodeToLeaf,
                             u32* nodeFirst, u32* nodeCount, cudaStream_t);

@@ -1,9 +1,9 @@
 // H4-H8: cornerstone leaf array by iterating f and g = g3 o g2 o g1 (Eqs. 2-9).
 //
-// One kernel launch per round does all of f, g1, g2, g3:
+// Two kernel launches per round do f, g1, g2, g3:
 //   f   (Eq. 3)  the lower-bound position off_i of every K_i in P is carried with K from round to
 //                round; N_i = off_{i+1} - off_i.  Only the 7 new boundaries of a split leaf are
-//                searched, inside the parent's particle range [off_i, off_{i+1}).
+//                searched, inside the parent's particle range [off_i, off_{i+1}) (second kernel).
 //   g1  (Eq. 5)  O_i in {8, 0, 1} per leaf (readings A7, A8, A9).
 //   g2  (Eq. 6)  exclusive prefix sum of O: in-tile scan + decoupled look-back across tiles.
 //   g3  (Eqs. 7-9, A10, A11) scatter of kept keys / 8 child keys to K'.
@@ -57,14 +57,18 @@ __global__ void __launch_bounds__(256) leavesInitPrevKernel(DeviceCtrl* ctrl, co
     if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->nl[0] = nlPrev;
 }
 
-// ---- one round ----------------------------------------------------------------------------------
+// ---- one round, kernel 1: g1, g2, g3 and the task list for f ----------------------------------------
+// Each split leaf becomes a search task (slot of its first child in K', end of its particle
+// range): the 7 inner child boundaries are located in P by leafSearchKernel, spread over the
+// whole GPU, instead of serially by the thread that owns the leaf.
 __global__ void __launch_bounds__(kLeafBlock)
-    leafRoundKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const u64* __restrict__ Kin,
-                    const u32* __restrict__ offIn, u64* __restrict__ Kout, u32* __restrict__ offOut, u64* lookback,
-                    u32 epoch, u32 r, u32 bucket, u32 cap, u32 lastRound)
+    leafRoundKernel(DeviceCtrl* ctrl, u32 n, const u64* __restrict__ Kin, const u32* __restrict__ offIn,
+                    u64* __restrict__ Kout, u32* __restrict__ offOut, uint2* __restrict__ tasks, u32 maxTasks,
+                    u64* lookback, u32 epoch, u32 r, u32 bucket, u32 cap, u32 lastRound)
 {
-    __shared__ u32 sTile, sPrefix, sDone;
+    __shared__ u32 sTile, sPrefix, sDone, sTaskBase;
     __shared__ u32 warpSums[kLeafBlock / 32 + 1];
+    __shared__ u32 warpSums2[kLeafBlock / 32 + 1];
     if (threadIdx.x == 0) sDone = ldVolatile(&ctrl->done);   // one read per CTA: the decision must be uniform
     __syncthreads();
     if (sDone) return;
@@ -89,7 +93,7 @@ __global__ void __launch_bounds__(kLeafBlock)
         }
         // g1: rebalance decision (Eq. 5)
         u32 O[kLeafItems];
-        u32 sum = 0;
+        u32 sum = 0, splits = 0;
         bool anyChange = false;
 #pragma unroll
         for (int k = 0; k < kLeafItems; ++k) {
@@ -114,10 +118,12 @@ __global__ void __launch_bounds__(kLeafBlock)
             }
             O[k] = o;
             sum += o;
+            splits += (o == 8);
         }
         // g2: exclusive prefix sum (Eq. 6): tile scan + look-back
-        u32 total;
+        u32 total, totalSplits;
         const u32 excl = blockExclusiveScan<kLeafBlock>(sum, warpSums, &total);
+        u32 taskSlot = blockExclusiveScan<kLeafBlock>(splits, warpSums2, &totalSplits);
         if (tid == 0) {
             u64* st = lookback + tile;
             u32 p = 0;
@@ -128,10 +134,12 @@ __global__ void __launch_bounds__(kLeafBlock)
                 lbStore(st, lbPack(epoch, kLbPrefix, p + total));
             }
             sPrefix = p;
+            sTaskBase = totalSplits ? atomicAdd(&ctrl->taskCount[r], totalSplits) : 0u;
         }
         const int tileChanged = __syncthreads_or(anyChange ? 1 : 0);
-        // g3: node rebalancing (Eqs. 8, 9); children's off by binary search in the parent's range
+        // g3: node rebalancing (Eqs. 8, 9)
         u32 p = sPrefix + excl;
+        taskSlot += sTaskBase;
 #pragma unroll
         for (int k = 0; k < kLeafItems; ++k) {
             if (O[k] == 1) {
@@ -142,17 +150,13 @@ __global__ void __launch_bounds__(kLeafBlock)
                 p += 1;
             } else if (O[k] == 8) {
                 const u64 step = (K[k + 1] - K[k]) >> 3;
-                u32 lo = off[k];
-                const u32 hi = off[k + 1];
-#pragma unroll 1
-                for (u32 c = 0; c < 8; ++c) {
-                    const u64 key = K[k] + c * step;
-                    if (c) lo = lowerBound(P, lo, hi, key);
-                    if (p + c < cap) {
-                        Kout[p + c] = key;
-                        offOut[p + c] = lo;
-                    }
+                if (p + 8 <= cap) {
+#pragma unroll
+                    for (u32 c = 0; c < 8; ++c) Kout[p + c] = K[k] + c * step;
+                    offOut[p] = off[k];
+                    if (taskSlot < maxTasks) tasks[taskSlot] = make_uint2(p, off[k + 1]);
                 }
+                ++taskSlot;
                 p += 8;
             }
         }
@@ -186,6 +190,78 @@ __global__ void __launch_bounds__(kLeafBlock)
                     }
                 }
             }
+        }
+    }
+}
+
+// ---- one round, kernel 2: f for the new boundaries (Eq. 3) ------------------------------------------
+// A split leaf with particle range [lo, hi) needs lower_bound(P, K'[p + c]) for c = 1..7, all
+// inside [lo, hi).  Work unit = (task, c), one warp each:
+//   * short ranges (<= kLinearMax keys): the warp of c = 1 streams the range once with coalesced
+//     loads and counts, with 7 ballots per 32 keys, how many keys fall below each child boundary.
+//   * long ranges: a 32-ary search, 32 probes per step (5 bits of the range per dependent
+//     memory round trip instead of 1).
+constexpr u32 kLinearMax = 1024;
+
+__device__ __forceinline__ u32 warpLowerBound32(const u64* __restrict__ P, u32 lo, u32 hi, u64 key, u32 lane)
+{
+    // invariant: answer in [lo, hi]; P[lo-1] < key (or lo is the range start), P[hi] >= key (or hi is the end)
+    while (hi - lo > 32) {
+        const u32 w = hi - lo;
+        const u32 s = (w + 31) / 32;                               // probe stride
+        const u32 idx = lo + (lane + 1) * s - 1;                   // last probe may fall beyond hi - 1
+        const bool below = idx < hi && __ldg(P + idx) < key;
+        const u32 m = __popc(__ballot_sync(kFull, below));         // probes are monotone: m leading trues
+        const u32 newLo = lo + m * s;
+        const u32 newHi = lo + (m + 1) * s - 1;
+        lo = newLo < hi ? newLo : hi;
+        hi = newHi < hi ? newHi : hi;
+    }
+    const u32 idx = lo + lane;
+    const bool below = idx < hi && __ldg(P + idx) < key;
+    return lo + __popc(__ballot_sync(kFull, below));
+}
+
+__global__ void __launch_bounds__(256)
+    leafSearchKernel(const DeviceCtrl* ctrl, const u64* __restrict__ P, const u64* __restrict__ Kout,
+                     u32* __restrict__ offOut, const uint2* __restrict__ tasks, u32 maxTasks, u32 r)
+{
+    if (ctrl->status == CS_ERR_CAPACITY || ctrl->status == CS_ERR_NOT_CORNERSTONE) return;   // task list incomplete
+    u32 numTasks = ctrl->taskCount[r];
+    if (numTasks > maxTasks) numTasks = maxTasks;
+    const u32 lane = laneId();
+    const u32 warpsPerGrid = gridDim.x * (blockDim.x >> 5);
+    const u32 units = numTasks * 7u;
+    for (u32 u = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); u < units; u += warpsPerGrid) {
+        const u32 t = u / 7u, c = u % 7u + 1u;
+        const uint2 task = tasks[t];
+        const u32 p = task.x, hi = task.y;
+        const u32 lo = offOut[p];
+        if (hi - lo <= kLinearMax) {
+            if (c != 1u) continue;
+            const u64 base = Kout[p];
+            const int sh = __ffsll((long long)(Kout[p + 1] - base)) - 1;     // child length is a power of 8
+            u32 below = 0;                                                   // lane c: keys in children < c
+            for (u32 i0 = lo; i0 < hi; i0 += 128) {
+                u32 child[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const u32 i = i0 + q * 32 + lane;
+                    child[q] = i < hi ? (u32)((__ldg(P + i) - base) >> sh) : 8u;
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+#pragma unroll
+                    for (u32 cc = 1; cc < 8; ++cc) {
+                        const u32 b = __popc(__ballot_sync(kFull, child[q] < cc));
+                        if (lane == cc) below += b;
+                    }
+                }
+            }
+            if (lane >= 1 && lane < 8) offOut[p + lane] = lo + below;
+        } else {
+            const u32 pos = warpLowerBound32(P, lo, hi, Kout[p + c], lane);
+            if (lane == 0) offOut[p + c] = pos;
         }
     }
 }
@@ -240,10 +316,20 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
             u32 bound = divUp(1ull << (3 * r), kLeafTile);
             if (bound < g) g = bound;
         }
-        leafRoundKernel<<<g, kLeafBlock, 0, s>>>(ctrl, P, (u32)n, ctx->leafK[r & 1], ctx->leafOff[r & 1],
-                                                 ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
-                                                 ctx->tileLookback, epoch, r, bucket, cap, roundsToLaunch - 1);
+        leafRoundKernel<<<g, kLeafBlock, 0, s>>>(ctrl, (u32)n, ctx->leafK[r & 1], ctx->leafOff[r & 1],
+                                                 ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1], ctx->leafTasks,
+                                                 ctx->maxTasks, ctx->tileLookback, epoch, r, bucket, cap,
+                                                 roundsToLaunch - 1);
         CS_LAUNCH_CHECK(ctx, "leafRoundKernel");
+        // searches of this round's split leaves: at most 7 * 8^r warps of work in the early rounds
+        u32 gs = persistentGrid;
+        if (!prevLeaves && r < 4) {
+            u32 bound = divUp(7ull << (3 * r), 8);
+            if (bound < gs) gs = bound;
+        }
+        leafSearchKernel<<<gs, 256, 0, s>>>(ctrl, P, ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
+                                            ctx->leafTasks, ctx->maxTasks, r);
+        CS_LAUNCH_CHECK(ctx, "leafSearchKernel");
     }
     leavesEmitKernel<<<grid, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafK[1], ctx->leafOff[0], ctx->leafOff[1],
                                           leaves, counts, ctx->leafOffFinal);

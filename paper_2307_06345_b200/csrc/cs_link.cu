@@ -100,7 +100,31 @@ __global__ void __launch_bounds__(kLinkBlock)
 struct LinkOut {
     u64* prefixes; u32* levels; u32* childOffsets; u32* parents; u32* levelRange; u32* leafToNode; u32* nodeToLeaf;
     u32 nodeCapacity;
+    // optional, fused H10: with the leaves' particle offsets (prefix sum of N) at hand, every node's
+    // particle range is written here too: a leaf's directly, an internal node's from the leaf
+    // index where its key range ends (found by a galloping search in K, 1 probe for most nodes).
+    const u32* leafOffsets; u32* nodeFirst; u32* nodeCount;
 };
+
+// index j1 of the leaf boundary K[j1] == end, given that the node starts at boundary j (j1 >= j + 8)
+__device__ __forceinline__ u32 subtreeEnd(const u64* __restrict__ K, u32 j, u32 nl, u64 end)
+{
+    u32 cur = j + 8;
+    if (cur >= nl || K[cur] >= end) return cur < nl ? cur : nl;
+    u32 prev, w = 8;
+    do {
+        prev = cur;
+        w <<= 1;
+        cur = prev + w < nl ? prev + w : nl;
+    } while (K[cur] < end);                      // K[nl] = 8^L >= end: terminates
+    u32 lo = prev + 1, hi = cur;                 // K[prev] < end <= K[cur]
+    while (lo < hi) {
+        const u32 mid = lo + ((hi - lo) >> 1);
+        if (K[mid] < end) lo = mid + 1;
+        else hi = mid;
+    }
+    return lo;
+}
 
 __global__ void __launch_bounds__(kLinkBlock)
     linkEmitKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves, LinkOut out,
@@ -220,6 +244,13 @@ __global__ void __launch_bounds__(kLinkBlock)
                     // placeholder-bit key: a 1 followed by l octal digits
                     out.prefixes[idx] = l == 0 ? 1ull : ((1ull << (3 * l)) | (Kj[k] >> (3 * (kL - l))));
                     if (out.levels) out.levels[idx] = (u32)l;
+                    if (out.nodeFirst) {
+                        const u32 firstP = out.leafOffsets[j];
+                        u32 jEnd = j + 1;
+                        if (isInt) jEnd = l == 0 ? nl : subtreeEnd(K, j, nl, Kj[k] + (1ull << (3 * (kL - l))));
+                        out.nodeFirst[idx] = firstP;
+                        out.nodeCount[idx] = out.leafOffsets[jEnd] - firstP;
+                    }
                     if (isInt) {
                         const u32 co = childStart + 8u * (runInt + __popc(bInt & lt));
                         out.childOffsets[idx] = co;
@@ -248,7 +279,8 @@ __global__ void __launch_bounds__(kLinkBlock)
 
 cs_status enqueueLink(cs_context* ctx, const u64* leaves, const u32* dNumLeaves, u32 hNumLeaves, u32 leafBound,
                       u64* prefixes, u32* levels, u32* childOffsets, u32* parents, u32* levelRange, u32* leafToNode,
-                      u32* nodeToLeaf, u32 nodeCapacity, cudaStream_t s)
+                      u32* nodeToLeaf, u32 nodeCapacity, const u32* leafOffsets, u32* nodeFirst, u32* nodeCount,
+                      cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_LINK, s);
     DeviceCtrl* ctrl = ctx->ctrl;
@@ -265,7 +297,8 @@ cs_status enqueueLink(cs_context* ctx, const u64* leaves, const u32* dNumLeaves,
     if (gridB > persistentGrid) gridB = persistentGrid;
     if (gridB == 0) gridB = 1;
     const u32 epoch = nextEpoch(ctx, s);
-    LinkOut out{prefixes, levels, childOffsets, parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity};
+    LinkOut out{prefixes, levels, childOffsets, parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity,
+                leafOffsets, leafOffsets ? nodeFirst : nullptr, nodeCount};
     linkEmitKernel<<<gridB, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, out, ctx->tileLookback, epoch);
     CS_LAUNCH_CHECK(ctx, "linkEmitKernel");
     return CS_OK;

@@ -107,22 +107,27 @@ __global__ void __launch_bounds__(kSortBlock, 2)
         key[j] = (full || loc < valid) ? ldStreamU64(keysIn + base + loc) : ~0ull;   // pads sort last
     }
 
-    // ---- rank inside the warp: match equal digits, one counter bump per distinct digit -------
+    // ---- rank inside the warp: peers holding the same digit are found with 8 ballots (one per digit
+    // bit; the native match.any is far slower), every peer reads the warp's running count of its
+    // digit (a shared-memory broadcast) and the lowest peer bumps it once ---------------------------
     u32 rank[kSortItems];
     u32* wh = sm.warpHist[warp];
     const u32 lt = laneMaskLt();
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        u32 d = digitOf(key[j], shift);
-        u32 m = __match_any_sync(kFull, d);
-        u32 lower = __popc(m & lt);
-        u32 prev = 0;
-        if (lower == 0) {           // lowest lane holding this digit
-            prev = wh[d];
-            wh[d] = prev + __popc(m);
+        const u32 d = digitOf(key[j], shift);
+        u32 peers = kFull;
+#pragma unroll
+        for (int b = 0; b < kRadixBits; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const u32 vote = __ballot_sync(kFull, bit);
+            peers &= bit ? vote : ~vote;
         }
+        const u32 lower = __popc(peers & lt);
+        const u32 prev = wh[d];
         __syncwarp();
-        prev = __shfl_sync(kFull, prev, __ffs(m) - 1);
+        if (lower == 0) wh[d] = prev + __popc(peers);
+        __syncwarp();
         rank[j] = prev + lower;
     }
     __syncthreads();
