@@ -92,6 +92,8 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
     if (prevLeaves && prevNumLeaves == 0)
         return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: prevLeaves given with prevNumLeaves == 0");
     CS_TRY(checkParticles(ctx, "cs_buildLeaves", n));
+    if (((uintptr_t)sortedKeys) & 15u)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildLeaves: sortedKeys must be 16-byte aligned");
     if (prevLeaves && (prevNumLeaves > ctx->maxLeaves || prevNumLeaves > leafCapacity))
         return fail(ctx, CS_ERR_CAPACITY, "cs_buildLeaves: prevNumLeaves exceeds the leaf capacity");
     DeviceGuard g(ctx->device);
@@ -169,6 +171,8 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     if (prevLeaves && prevNumLeaves == 0)
         return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: prevLeaves given with prevNumLeaves == 0");
     CS_TRY(checkParticles(ctx, "cs_buildOctree", n));
+    if (((uintptr_t)b->keys) & 15u)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_buildOctree: buffers->keys must be 16-byte aligned");
     if (prevLeaves && (prevNumLeaves > ctx->maxLeaves || prevNumLeaves > b->leafCapacity))
         return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctree: prevNumLeaves exceeds the leaf capacity");
     DeviceGuard g(ctx->device);

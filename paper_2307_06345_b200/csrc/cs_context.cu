@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, tileLookback, ctrl, total;
+        leafOffFinal, leafTasks, tileLookback, linkTileHist, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -53,8 +53,9 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafOff0 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOff1 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOffFinal = take(((size_t)maxLeaves + 2) * sizeof(u32));
-    L.leafTasks = take(((size_t)maxLeaves / 8 + 8) * sizeof(uint2));
-    L.tileLookback = take(leafTiles * kLinkBins * sizeof(u64));
+    L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint2));   // linear list, search list
+    L.tileLookback = take(leafTiles * sizeof(u64));                        // one counter per tile (leaf rounds, scan)
+    L.linkTileHist = take(leafTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
     return L;
@@ -68,7 +69,7 @@ u32 nextEpoch(cs_context* ctx, cudaStream_t s)
     if (ctx->epoch >= (1u << 30)) {   // wrap: clear every look-back array once
         Layout L = makeLayout(ctx->maxParticles, ctx->maxLeaves, kBoxGridMax);
         cudaMemsetAsync(ctx->sortLookback, 0, L.boxPartials - L.sortLookback, s);
-        cudaMemsetAsync(ctx->tileLookback, 0, L.ctrl - L.tileLookback, s);
+        cudaMemsetAsync(ctx->tileLookback, 0, L.linkTileHist - L.tileLookback, s);
         ctx->epoch = 1;
     }
     return ctx->epoch;
@@ -104,17 +105,20 @@ __global__ void __launch_bounds__(kScanBlock) scanKernel(const u32* __restrict__
         }
         u32 total;
         u32 excl = blockExclusiveScan<kScanBlock>(sum, warpSums, &total);
-        if (threadIdx.x == 0) {
+        if (threadIdx.x < 32) {                       // warp 0: publish, then warp-wide look-back
             u64* st = lookback + tile;
             u32 p = 0;
-            if (tile == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
-            else {
-                lbStore(st, lbPack(epoch, kLbAggregate, total));
-                p = lbLookBack(lookback, 1, 0, tile, epoch);
-                lbStore(st, lbPack(epoch, kLbPrefix, p + total));
+            if (tile == 0) {
+                if (threadIdx.x == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
+            } else {
+                if (threadIdx.x == 0) lbStore(st, lbPack(epoch, kLbAggregate, total));
+                p = lbLookBackWarp(lookback, tile, epoch);
+                if (threadIdx.x == 0) lbStore(st, lbPack(epoch, kLbPrefix, p + total));
             }
-            sPrefix = p;
-            if (tile == tiles - 1) out[n] = p + total;
+            if (threadIdx.x == 0) {
+                sPrefix = p;
+                if (tile == tiles - 1) out[n] = p + total;
+            }
         }
         __syncthreads();
         u32 run = sPrefix + excl;
@@ -203,6 +207,7 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->leafTasks = (uint2*)(ctx->slab + L.leafTasks);
     ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
+    ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
     *out = ctx;
     return CS_OK;

@@ -101,6 +101,35 @@ __device__ __forceinline__ u32 lbLookBack(const u64* state, u32 stride, u32 c, u
     return excl;
 }
 
+// Warp-wide look-back for a single counter per tile: the 32 lanes inspect 32 predecessors per
+// step, so the frontier of finished prefixes advances 32 tiles per memory round trip.  Must be
+// called by all 32 lanes of one warp; returns the exclusive prefix of `tile` (> 0) in every lane.
+__device__ __forceinline__ u32 lbLookBackWarp(const u64* state, u32 tile, u32 epoch)
+{
+    const u32 lane = laneId();
+    u32 excl = 0;
+    int top = (int)tile - 1;                          // nearest predecessor not yet summed
+    while (true) {
+        const int p = top - (int)lane;
+        u64 w = 0;
+        bool isPrefix = false;
+        if (p >= 0) {
+            w = lbWait(state + p, epoch);
+            isPrefix = ((u32)(w >> 32) & 3u) == kLbPrefix;
+        }
+        const u32 prefMask = __ballot_sync(kFull, isPrefix);
+        // lanes up to (and including) the nearest prefix contribute; lanes with p < 0 hold 0
+        const u32 nearest = prefMask ? (u32)(__ffs(prefMask) - 1) : 31u;
+        u32 v = lane <= nearest ? (u32)w : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+        excl += v;
+        if (prefMask || top < 32) break;             // found a prefix, or reached tile 0 (always a prefix)
+        top -= 32;
+    }
+    return excl;
+}
+
 // ---- warp / block scans --------------------------------------------------------------------
 __device__ __forceinline__ u32 warpInclusiveScan(u32 v)
 {

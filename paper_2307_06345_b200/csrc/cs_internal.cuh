@@ -48,7 +48,8 @@ struct DeviceCtrl {
     u32 ticket[kRoundSlots];     // tile tickets of round r
     u32 tilesDone[kRoundSlots];
     u32 changed[kRoundSlots];    // some O_i != 1 in round r
-    u32 taskCount[kRoundSlots];  // split leaves of round r (search tasks)
+    u32 taskCount[kRoundSlots];  // split leaves of round r with a short particle range (counted linearly)
+    u32 searchCount[kRoundSlots];// split leaves of round r with a long particle range (searched)
     u32 done;                    // refinement finished (converged / maxRounds / error)
     u32 rounds;                  // rounds performed
     u32 converged;
@@ -96,7 +97,8 @@ struct cs_context {
     uint2* leafTasks = nullptr;        // (first child slot, end of the parent's particle range) per split leaf
     cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
-    cs::u64* tileLookback = nullptr;   // [tiles][kLinkBins] (also used by the scan and the leaf rounds)
+    cs::u64* tileLookback = nullptr;   // [tiles] look-back words of the leaf rounds and the scan
+    cs::u32* linkTileHist = nullptr;   // [tiles][kLinkBins] node counts per tile, level and kind
     cs::DeviceCtrl* ctrl = nullptr;
     cs::HostCtrl* hostCtrl = nullptr;  // pinned
 

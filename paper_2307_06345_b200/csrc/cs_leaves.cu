@@ -57,16 +57,19 @@ __global__ void __launch_bounds__(256) leavesInitPrevKernel(DeviceCtrl* ctrl, co
     if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->nl[0] = nlPrev;
 }
 
+constexpr u32 kLinearMax = 1024;   // split leaves with at most this many particles are counted linearly
+
 // ---- one round, kernel 1: g1, g2, g3 and the task list for f ----------------------------------------
 // Each split leaf becomes a search task (slot of its first child in K', end of its particle
 // range): the 7 inner child boundaries are located in P by leafSearchKernel, spread over the
 // whole GPU, instead of serially by the thread that owns the leaf.
 __global__ void __launch_bounds__(kLeafBlock)
     leafRoundKernel(DeviceCtrl* ctrl, u32 n, const u64* __restrict__ Kin, const u32* __restrict__ offIn,
-                    u64* __restrict__ Kout, u32* __restrict__ offOut, uint2* __restrict__ tasks, u32 maxTasks,
-                    u64* lookback, u32 epoch, u32 r, u32 bucket, u32 cap, u32 lastRound)
+                    u64* __restrict__ Kout, u32* __restrict__ offOut, uint2* __restrict__ tasksLin,
+                    uint2* __restrict__ tasksSearch, u32 maxTasks, u64* lookback, u32 epoch, u32 r, u32 bucket, u32 cap,
+                    u32 lastRound)
 {
-    __shared__ u32 sTile, sPrefix, sDone, sTaskBase;
+    __shared__ u32 sTile, sPrefix, sDone, sLinBase, sSearchBase;
     __shared__ u32 warpSums[kLeafBlock / 32 + 1];
     __shared__ u32 warpSums2[kLeafBlock / 32 + 1];
     if (threadIdx.x == 0) sDone = ldVolatile(&ctrl->done);   // one read per CTA: the decision must be uniform
@@ -118,28 +121,34 @@ __global__ void __launch_bounds__(kLeafBlock)
             }
             O[k] = o;
             sum += o;
-            splits += (o == 8);
+            // split leaves become search tasks: short particle ranges are counted linearly, long ones searched
+            if (o == 8) splits += (off[k + 1] - off[k] <= kLinearMax) ? 1u : (1u << 16);
         }
         // g2: exclusive prefix sum (Eq. 6): tile scan + look-back
         u32 total, totalSplits;
         const u32 excl = blockExclusiveScan<kLeafBlock>(sum, warpSums, &total);
         u32 taskSlot = blockExclusiveScan<kLeafBlock>(splits, warpSums2, &totalSplits);
-        if (tid == 0) {
+        if (tid < 32) {                               // warp 0: publish, then warp-wide look-back
             u64* st = lookback + tile;
             u32 p = 0;
-            if (tile == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
-            else {
-                lbStore(st, lbPack(epoch, kLbAggregate, total));
-                p = lbLookBack(lookback, 1, 0, tile, epoch);
-                lbStore(st, lbPack(epoch, kLbPrefix, p + total));
+            if (tile == 0) {
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
+            } else {
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbAggregate, total));
+                p = lbLookBackWarp(lookback, tile, epoch);
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, p + total));
             }
-            sPrefix = p;
-            sTaskBase = totalSplits ? atomicAdd(&ctrl->taskCount[r], totalSplits) : 0u;
+            if (tid == 0) {
+                sPrefix = p;
+                const u32 nLin = totalSplits & 0xFFFFu, nSearch = totalSplits >> 16;
+                sLinBase = nLin ? atomicAdd(&ctrl->taskCount[r], nLin) : 0u;
+                sSearchBase = nSearch ? atomicAdd(&ctrl->searchCount[r], nSearch) : 0u;
+            }
         }
         const int tileChanged = __syncthreads_or(anyChange ? 1 : 0);
         // g3: node rebalancing (Eqs. 8, 9)
         u32 p = sPrefix + excl;
-        taskSlot += sTaskBase;
+        u32 linSlot = sLinBase + (taskSlot & 0xFFFFu), searchSlot = sSearchBase + (taskSlot >> 16);
 #pragma unroll
         for (int k = 0; k < kLeafItems; ++k) {
             if (O[k] == 1) {
@@ -154,9 +163,11 @@ __global__ void __launch_bounds__(kLeafBlock)
 #pragma unroll
                     for (u32 c = 0; c < 8; ++c) Kout[p + c] = K[k] + c * step;
                     offOut[p] = off[k];
-                    if (taskSlot < maxTasks) tasks[taskSlot] = make_uint2(p, off[k + 1]);
                 }
-                ++taskSlot;
+                const bool lin = off[k + 1] - off[k] <= kLinearMax;
+                u32& slot = lin ? linSlot : searchSlot;
+                if (p + 8 <= cap && slot < maxTasks) (lin ? tasksLin : tasksSearch)[slot] = make_uint2(p, off[k + 1]);
+                ++slot;
                 p += 8;
             }
         }
@@ -201,8 +212,6 @@ __global__ void __launch_bounds__(kLeafBlock)
 //     loads and counts, with 7 ballots per 32 keys, how many keys fall below each child boundary.
 //   * long ranges: a 32-ary search, 32 probes per step (5 bits of the range per dependent
 //     memory round trip instead of 1).
-constexpr u32 kLinearMax = 1024;
-
 __device__ __forceinline__ u32 warpLowerBound32(const u64* __restrict__ P, u32 lo, u32 hi, u64 key, u32 lane)
 {
     // invariant: answer in [lo, hi]; P[lo-1] < key (or lo is the range start), P[hi] >= key (or hi is the end)
@@ -223,46 +232,81 @@ __device__ __forceinline__ u32 warpLowerBound32(const u64* __restrict__ P, u32 l
 }
 
 __global__ void __launch_bounds__(256)
-    leafSearchKernel(const DeviceCtrl* ctrl, const u64* __restrict__ P, const u64* __restrict__ Kout,
-                     u32* __restrict__ offOut, const uint2* __restrict__ tasks, u32 maxTasks, u32 r)
+    leafSearchKernel(const DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const u64* __restrict__ Kout,
+                     u32* __restrict__ offOut, const uint2* __restrict__ tasksLin,
+                     const uint2* __restrict__ tasksSearch, u32 maxTasks, u32 r)
 {
-    if (ctrl->status == CS_ERR_CAPACITY || ctrl->status == CS_ERR_NOT_CORNERSTONE) return;   // task list incomplete
-    u32 numTasks = ctrl->taskCount[r];
-    if (numTasks > maxTasks) numTasks = maxTasks;
+    if (ctrl->status == CS_ERR_CAPACITY || ctrl->status == CS_ERR_NOT_CORNERSTONE) return;   // task lists incomplete
+    u32 numLin = ctrl->taskCount[r], numSearch = ctrl->searchCount[r];
+    if (numLin > maxTasks) numLin = maxTasks;
+    if (numSearch > maxTasks) numSearch = maxTasks;
     const u32 lane = laneId();
     const u32 warpsPerGrid = gridDim.x * (blockDim.x >> 5);
-    const u32 units = numTasks * 7u;
-    for (u32 u = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); u < units; u += warpsPerGrid) {
+    const u32 warpId = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+
+    // ---- short ranges: 8 lanes per task, 4 tasks per warp, 128-bit coalesced loads; every lane keeps
+    // a packed 8 x 16-bit histogram of the child octant of its keys, folded over the 8 lanes at the end
+    const u32 gl = lane & 7u;
+    for (u32 t0 = warpId * 4u; t0 < numLin; t0 += warpsPerGrid * 4u) {
+        const u32 t = t0 + (lane >> 3);
+        const bool valid = t < numLin;
+        u32 p = 0, lo = 0, hi = 0;
+        u64 base = 0;
+        int sh = 0;
+        if (valid) {
+            const uint2 task = tasksLin[t];
+            p = task.x;
+            hi = task.y;
+            lo = offOut[p];
+            base = Kout[p];
+            sh = __ffsll((long long)(Kout[p + 1] - base)) - 1;            // child length is a power of 8
+        }
+        const u32 a0 = lo & ~1u;                                          // 16-byte aligned start
+        u32 iters = valid ? (hi - a0 + 15u) / 16u : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) iters = max(iters, __shfl_xor_sync(kFull, iters, o));
+        u64 h0 = 0, h1 = 0;                                               // children 0-3 / 4-7, 16 bits each
+        auto add = [&](u64 key) {
+            const u32 c = (u32)((key - base) >> sh);                      // 0..7 inside the parent's range
+            const u64 one = 1ull << ((c & 3u) * 16u);
+            if (c & 4u) h1 += one;
+            else h0 += one;
+        };
+        for (u32 it = 0; it < iters; ++it) {
+            const u32 idx = a0 + it * 16u + gl * 2u;
+            if (idx + 1 < hi) {                                           // both elements inside [.., hi)
+                const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(P + idx);
+                if (idx >= lo) add(v.x);
+                add(v.y);
+            } else if (idx < hi && idx >= lo) {
+                add(__ldg(P + idx));
+            }
+        }
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) {
+            h0 += __shfl_xor_sync(kFull, h0, o);
+            h1 += __shfl_xor_sync(kFull, h1, o);
+        }
+        if (valid && gl >= 1) {                                           // lane c: keys in children < c
+            u32 below = 0;
+#pragma unroll
+            for (u32 c = 0; c < 7; ++c) {
+                const u32 cnt = (u32)(((c < 4 ? h0 : h1) >> ((c & 3u) * 16u)) & 0xFFFFu);
+                if (c < gl) below += cnt;
+            }
+            offOut[p + gl] = lo + below;
+        }
+    }
+
+    // ---- long ranges: one warp per (task, child boundary), 32-ary search -----------------------------
+    const u32 units = numSearch * 7u;
+    for (u32 u = warpId; u < units; u += warpsPerGrid) {
         const u32 t = u / 7u, c = u % 7u + 1u;
-        const uint2 task = tasks[t];
+        const uint2 task = tasksSearch[t];
         const u32 p = task.x, hi = task.y;
         const u32 lo = offOut[p];
-        if (hi - lo <= kLinearMax) {
-            if (c != 1u) continue;
-            const u64 base = Kout[p];
-            const int sh = __ffsll((long long)(Kout[p + 1] - base)) - 1;     // child length is a power of 8
-            u32 below = 0;                                                   // lane c: keys in children < c
-            for (u32 i0 = lo; i0 < hi; i0 += 128) {
-                u32 child[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const u32 i = i0 + q * 32 + lane;
-                    child[q] = i < hi ? (u32)((__ldg(P + i) - base) >> sh) : 8u;
-                }
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-#pragma unroll
-                    for (u32 cc = 1; cc < 8; ++cc) {
-                        const u32 b = __popc(__ballot_sync(kFull, child[q] < cc));
-                        if (lane == cc) below += b;
-                    }
-                }
-            }
-            if (lane >= 1 && lane < 8) offOut[p + lane] = lo + below;
-        } else {
-            const u32 pos = warpLowerBound32(P, lo, hi, Kout[p + c], lane);
-            if (lane == 0) offOut[p + c] = pos;
-        }
+        const u32 pos = warpLowerBound32(P, lo, hi, Kout[p + c], lane);
+        if (lane == 0) offOut[p + c] = pos;
     }
 }
 
@@ -318,8 +362,8 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
         }
         leafRoundKernel<<<g, kLeafBlock, 0, s>>>(ctrl, (u32)n, ctx->leafK[r & 1], ctx->leafOff[r & 1],
                                                  ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1], ctx->leafTasks,
-                                                 ctx->maxTasks, ctx->tileLookback, epoch, r, bucket, cap,
-                                                 roundsToLaunch - 1);
+                                                 ctx->leafTasks + ctx->maxTasks, ctx->maxTasks, ctx->tileLookback,
+                                                 epoch, r, bucket, cap, roundsToLaunch - 1);
         CS_LAUNCH_CHECK(ctx, "leafRoundKernel");
         // searches of this round's split leaves: at most 7 * 8^r warps of work in the early rounds
         u32 gs = persistentGrid;
@@ -327,8 +371,8 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
             u32 bound = divUp(7ull << (3 * r), 8);
             if (bound < gs) gs = bound;
         }
-        leafSearchKernel<<<gs, 256, 0, s>>>(ctrl, P, ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
-                                            ctx->leafTasks, ctx->maxTasks, r);
+        leafSearchKernel<<<gs, 256, 0, s>>>(ctrl, P, (u32)n, ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
+                                            ctx->leafTasks, ctx->leafTasks + ctx->maxTasks, ctx->maxTasks, r);
         CS_LAUNCH_CHECK(ctx, "leafSearchKernel");
     }
     leavesEmitKernel<<<grid, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafK[1], ctx->leafOff[0], ctx->leafOff[1],

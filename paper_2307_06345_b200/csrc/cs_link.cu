@@ -14,13 +14,15 @@
 //     inside one level it enumerates them in SFC order.
 //   * Hence index(node) = LO[level] + (number of level-`level` nodes starting at boundaries < j):
 //     a 22-bin stable split, done with per-level ballots inside a warp, a scan over the warps
-//     of a tile and a decoupled look-back over tiles.
+//     of a tile and a prefix sum over tiles.
 //   * The children of the k-th internal node of level l (SFC order) are the 8 nodes
 //     LO[l+1] + 8k .. + 8k + 7, because level l+1 consists of exactly those sibling groups in
 //     the same order.  So CO = LO[l+1] + 8 * (rank among the internal nodes of level l):
 //     a second set of 22 counters, no search.
 //
-// Pass A counts nodes per level (-> LO, numNodes) and validates Eq. 2; pass B ranks and writes.
+// Pass A counts nodes per level and tile and validates Eq. 2; pass A2 turns the counts into
+// exclusive prefixes over tiles (-> LO, numNodes); pass C ranks inside the tile and writes.
+// No pass waits on another CTA: tiles are assigned statically.
 #include "cs_device.cuh"
 
 namespace cs {
@@ -48,55 +50,125 @@ __device__ __forceinline__ u32 numLeavesOf(const u32* dNumLeaves, u32 hNumLeaves
     return dNumLeaves ? *dNumLeaves : hNumLeaves;
 }
 
-// ---- pass A: nodes per level --------------------------------------------------------------------
-__global__ void __launch_bounds__(kLinkBlock)
-    linkCountKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves)
+// ---- shared by passes A and C: this thread's boundaries and the warp's counts per level -----------
+struct TileItems {
+    int lo[kLinkItems], hi[kLinkItems];
+    u64 Kj[kLinkItems];
+    int wlo, whi;             // warp-uniform range of levels present
+};
+
+// Loads the kLinkItems boundaries of this thread (warp-striped: item order == boundary order).
+// Returns false if some gap violates Eq. 2.
+__device__ __forceinline__ bool loadTileItems(const u64* __restrict__ K, u32 nl, u32 warpBase, TileItems& it)
 {
-    __shared__ u32 sCnt[kLinkBins];
+    bool ok = true;
+    it.wlo = kLevels;
+    it.whi = -1;
+#pragma unroll
+    for (int k = 0; k < kLinkItems; ++k) {
+        const u32 j = warpBase + k * 32;
+        it.lo[k] = 1; it.hi[k] = 0; it.Kj[k] = 0;                      // empty range for j >= nl
+        if (j < nl) {
+            it.Kj[k] = K[j];
+            const u64 Kn = K[j + 1];
+            if (!boundaryLevels(it.Kj[k], Kn, j, it.lo[k], it.hi[k])) { ok = false; it.lo[k] = 1; it.hi[k] = 0; }
+            if (j == 0 && it.Kj[k] != 0) ok = false;
+            if (j == nl - 1 && Kn != kKeyEnd) ok = false;
+            if (it.lo[k] <= it.hi[k]) { it.wlo = min(it.wlo, it.lo[k]); it.whi = max(it.whi, it.hi[k]); }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        it.wlo = min(it.wlo, __shfl_xor_sync(kFull, it.wlo, o));
+        it.whi = max(it.whi, __shfl_xor_sync(kFull, it.whi, o));
+    }
+    return ok;
+}
+
+// per-warp node counts per level (all / internal) -> wc[0..kLinkBins), written by lane 0
+__device__ __forceinline__ void warpLevelCounts(const TileItems& it, u32* wc, u32 lane)
+{
+    for (int l = it.wlo; l <= it.whi; ++l) {
+        u32 cAll = 0, cInt = 0;
+#pragma unroll
+        for (int k = 0; k < kLinkItems; ++k) {
+            cAll += __popc(__ballot_sync(kFull, it.lo[k] <= l && l <= it.hi[k]));
+            cInt += __popc(__ballot_sync(kFull, it.lo[k] <= l && l < it.hi[k]));
+        }
+        if (lane == 0) { wc[l] = cAll; wc[kLevels + l] = cInt; }
+    }
+}
+
+// ---- pass A: nodes per level and tile; validates Eq. 2 -------------------------------------------------
+__global__ void __launch_bounds__(kLinkBlock)
+    linkCountKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves,
+                    u32* __restrict__ tileHist)
+{
+    __shared__ u32 sWarp[kLinkWarps][kLinkBins];
     __shared__ u32 sStop;
-    if (threadIdx.x == 0) {                                   // one read per CTA: uniform decision
+    const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
+    if (tid == 0) {                                           // one read per CTA: uniform decision
         const u32 st = *(const volatile u32*)&ctrl->status;
         sStop = (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) ? 1u : 0u;
     }
-    if (threadIdx.x < kLinkBins) sCnt[threadIdx.x] = 0;
     __syncthreads();
     if (sStop) return;
     const u32 nl = numLeavesOf(dNumLeaves, hNumLeaves);
-    const u32 lane = laneId();
-    bool bad = false;
-    const u32 stride = gridDim.x * kLinkBlock;
-    const u32 rounds = (nl + stride - 1) / stride;
-    for (u32 it = 0; it < rounds; ++it) {
-        const u32 j = it * stride + blockIdx.x * kLinkBlock + threadIdx.x;
-        int lo = 1, hi = 0;                                   // empty range for j >= nl
-        if (j < nl) {
-            const u64 Kj = K[j], Kn = K[j + 1];
-            if (!boundaryLevels(Kj, Kn, j, lo, hi)) { bad = true; lo = 1; hi = 0; }
-            if (j == 0 && Kj != 0) bad = true;
-            if (j == nl - 1 && Kn != kKeyEnd) bad = true;
-        }
-        int wlo = lo <= hi ? lo : kLevels, whi = lo <= hi ? hi : -1;
+    const u32 tiles = (nl + kLinkTile - 1) / kLinkTile;
+    bool bad = (nl == 0);
+    for (u32 tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
+        __syncthreads();
+        for (int i = tid; i < kLinkWarps * kLinkBins; i += kLinkBlock) (&sWarp[0][0])[i] = 0;
+        __syncthreads();
+        TileItems it;
+        if (!loadTileItems(K, nl, tile * kLinkTile + warp * (32 * kLinkItems) + lane, it)) bad = true;
+        warpLevelCounts(it, sWarp[warp], lane);
+        __syncthreads();
+        if (tid < kLinkBins) {
+            u32 sum = 0;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            wlo = min(wlo, __shfl_xor_sync(kFull, wlo, o));
-            whi = max(whi, __shfl_xor_sync(kFull, whi, o));
-        }
-        for (int l = wlo; l <= whi; ++l) {
-            const u32 bAll = __ballot_sync(kFull, lo <= l && l <= hi);
-            const u32 bInt = __ballot_sync(kFull, lo <= l && l < hi);
-            if (lane == 0) {
-                if (bAll) atomicAdd(&sCnt[l], __popc(bAll));
-                if (bInt) atomicAdd(&sCnt[kLevels + l], __popc(bInt));
-            }
+            for (int w = 0; w < kLinkWarps; ++w) sum += sWarp[w][tid];
+            tileHist[(size_t)tile * kLinkBins + tid] = sum;
         }
     }
-    if (nl == 0) bad = true;
-    __syncthreads();
-    if (threadIdx.x < kLinkBins && sCnt[threadIdx.x]) atomicAdd(&ctrl->levelTotals[threadIdx.x], sCnt[threadIdx.x]);
     if (bad) ctrl->status = CS_ERR_NOT_CORNERSTONE;
 }
 
-// ---- pass B: rank and write -------------------------------------------------------------------------
+// ---- pass A2: exclusive prefix over tiles of every (level, kind) column; column totals -----------------
+constexpr int kColItems = 4;
+__global__ void __launch_bounds__(256)
+    linkScanKernel(DeviceCtrl* ctrl, const u32* dNumLeaves, u32 hNumLeaves, u32* __restrict__ tileHist)
+{
+    __shared__ u32 warpSums[256 / 32 + 1];
+    const u32 st = ctrl->status;
+    if (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) return;
+    const u32 nl = numLeavesOf(dNumLeaves, hNumLeaves);
+    const u32 tiles = (nl + kLinkTile - 1) / kLinkTile;
+    const u32 bin = blockIdx.x;
+    u32 running = 0;
+    for (u32 t0 = 0; t0 < tiles; t0 += 256 * kColItems) {
+        u32 v[kColItems], sum = 0;
+#pragma unroll
+        for (int k = 0; k < kColItems; ++k) {
+            const u32 t = t0 + threadIdx.x * kColItems + k;
+            v[k] = t < tiles ? tileHist[(size_t)t * kLinkBins + bin] : 0u;
+            sum += v[k];
+        }
+        u32 total;
+        u32 run = running + blockExclusiveScan<256>(sum, warpSums, &total);
+#pragma unroll
+        for (int k = 0; k < kColItems; ++k) {
+            const u32 t = t0 + threadIdx.x * kColItems + k;
+            if (t < tiles) tileHist[(size_t)t * kLinkBins + bin] = run;
+            run += v[k];
+        }
+        running += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) ctrl->levelTotals[bin] = running;
+}
+
+// ---- pass C: rank and write ----------------------------------------------------------------------------
 struct LinkOut {
     u64* prefixes; u32* levels; u32* childOffsets; u32* parents; u32* levelRange; u32* leafToNode; u32* nodeToLeaf;
     u32 nodeCapacity;
@@ -128,12 +200,12 @@ __device__ __forceinline__ u32 subtreeEnd(const u64* __restrict__ K, u32 j, u32 
 
 __global__ void __launch_bounds__(kLinkBlock)
     linkEmitKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves, LinkOut out,
-                   u64* lookback, u32 epoch)
+                   const u32* __restrict__ tilePrefix)
 {
     __shared__ u32 sLO[kLevels + 2];                  // level offsets
     __shared__ u32 sWarp[kLinkWarps][kLinkBins];      // per-warp counts -> running exclusive prefix
     __shared__ u32 sBase[kLinkBins];                  // tile's exclusive prefix per bin
-    __shared__ u32 sTile, sStop;
+    __shared__ u32 sStop;
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
     const u32 nl = numLeavesOf(dNumLeaves, hNumLeaves);
     if (tid == 0) {
@@ -165,49 +237,18 @@ __global__ void __launch_bounds__(kLinkBlock)
     if (sStop) return;
     const u32 tiles = (nl + kLinkTile - 1) / kLinkTile;
     const u32 lt = laneMaskLt();
-    for (;;) {
+    for (u32 tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
         __syncthreads();
-        if (tid == 0) sTile = atomicAdd(&ctrl->linkTicket, 1u);
         for (int i = tid; i < kLinkWarps * kLinkBins; i += kLinkBlock) (&sWarp[0][0])[i] = 0;
+        if (tid < kLinkBins) sBase[tid] = tilePrefix[(size_t)tile * kLinkBins + tid];
         __syncthreads();
-        const u32 tile = sTile;
-        if (tile >= tiles) break;
         const u32 warpBase = tile * kLinkTile + warp * (32 * kLinkItems) + lane;
-
-        // boundary levels of this thread's items (warp-striped: item order == boundary order)
-        int lo[kLinkItems], hi[kLinkItems];
-        u64 Kj[kLinkItems];
-        int wlo = kLevels, whi = -1;
-#pragma unroll
-        for (int k = 0; k < kLinkItems; ++k) {
-            const u32 j = warpBase + k * 32;
-            lo[k] = 1; hi[k] = 0; Kj[k] = 0;
-            if (j < nl) {
-                Kj[k] = K[j];
-                boundaryLevels(Kj[k], K[j + 1], j, lo[k], hi[k]);   // validated in pass A
-                wlo = min(wlo, lo[k]);
-                whi = max(whi, hi[k]);
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            wlo = min(wlo, __shfl_xor_sync(kFull, wlo, o));
-            whi = max(whi, __shfl_xor_sync(kFull, whi, o));
-        }
-        // phase 1: per-warp counts per level
+        TileItems it;
+        loadTileItems(K, nl, warpBase, it);               // validated in pass A
         u32* wc = sWarp[warp];
-        for (int l = wlo; l <= whi; ++l) {
-            u32 cAll = 0, cInt = 0;
-#pragma unroll
-            for (int k = 0; k < kLinkItems; ++k) {
-                cAll += __popc(__ballot_sync(kFull, lo[k] <= l && l <= hi[k]));
-                cInt += __popc(__ballot_sync(kFull, lo[k] <= l && l < hi[k]));
-            }
-            if (lane == 0) { wc[l] = cAll; wc[kLevels + l] = cInt; }
-        }
+        warpLevelCounts(it, wc, lane);
         __syncthreads();
-        // exclusive prefix over warps, tile totals, look-back (one thread per bin)
-        if (tid < kLinkBins) {
+        if (tid < kLinkBins) {                            // exclusive prefix over the warps of the tile
             u32 run = 0;
 #pragma unroll
             for (int w = 0; w < kLinkWarps; ++w) {
@@ -215,39 +256,30 @@ __global__ void __launch_bounds__(kLinkBlock)
                 sWarp[w][tid] = run;
                 run += c;
             }
-            u64* st = lookback + (size_t)tile * kLinkBins + tid;
-            u32 excl = 0;
-            if (tile == 0) lbStore(st, lbPack(epoch, kLbPrefix, run));
-            else {
-                lbStore(st, lbPack(epoch, kLbAggregate, run));
-                excl = lbLookBack(lookback, kLinkBins, tid, tile, epoch);
-                lbStore(st, lbPack(epoch, kLbPrefix, excl + run));
-            }
-            sBase[tid] = excl;
         }
         __syncthreads();
-        // phase 2: positions and output
-        for (int l = wlo; l <= whi; ++l) {
+        // positions and output
+        for (int l = it.wlo; l <= it.whi; ++l) {
             u32 runAll = sBase[l] + wc[l];
             u32 runInt = sBase[kLevels + l] + wc[kLevels + l];
             const u32 levelStart = sLO[l];
             const u32 childStart = sLO[l + 1];
 #pragma unroll
             for (int k = 0; k < kLinkItems; ++k) {
-                const bool isNode = lo[k] <= l && l <= hi[k];
-                const bool isInt = isNode && l < hi[k];
+                const bool isNode = it.lo[k] <= l && l <= it.hi[k];
+                const bool isInt = isNode && l < it.hi[k];
                 const u32 bAll = __ballot_sync(kFull, isNode);
                 const u32 bInt = __ballot_sync(kFull, isInt);
                 if (isNode) {
                     const u32 j = warpBase + k * 32;
                     const u32 idx = levelStart + runAll + __popc(bAll & lt);
                     // placeholder-bit key: a 1 followed by l octal digits
-                    out.prefixes[idx] = l == 0 ? 1ull : ((1ull << (3 * l)) | (Kj[k] >> (3 * (kL - l))));
+                    out.prefixes[idx] = l == 0 ? 1ull : ((1ull << (3 * l)) | (it.Kj[k] >> (3 * (kL - l))));
                     if (out.levels) out.levels[idx] = (u32)l;
                     if (out.nodeFirst) {
                         const u32 firstP = out.leafOffsets[j];
                         u32 jEnd = j + 1;
-                        if (isInt) jEnd = l == 0 ? nl : subtreeEnd(K, j, nl, Kj[k] + (1ull << (3 * (kL - l))));
+                        if (isInt) jEnd = l == 0 ? nl : subtreeEnd(K, j, nl, it.Kj[k] + (1ull << (3 * (kL - l))));
                         out.nodeFirst[idx] = firstP;
                         out.nodeCount[idx] = out.leafOffsets[jEnd] - firstP;
                     }
@@ -256,13 +288,8 @@ __global__ void __launch_bounds__(kLinkBlock)
                         out.childOffsets[idx] = co;
                         if (out.nodeToLeaf) out.nodeToLeaf[idx] = CS_NO_LEAF;
                         if (out.parents) {
-                            uint4 p4 = make_uint4(idx, idx, idx, idx);
-                            uint4* dst = reinterpret_cast<uint4*>(out.parents + co);   // co = 1 + 8k: not 16B aligned
-                            if ((((uintptr_t)dst) & 15u) == 0) { dst[0] = p4; dst[1] = p4; }
-                            else {
 #pragma unroll
-                                for (int c = 0; c < 8; ++c) out.parents[co + c] = idx;
-                            }
+                            for (int c = 0; c < 8; ++c) out.parents[co + c] = idx;
                         }
                     } else {
                         out.childOffsets[idx] = 0;               // leaf
@@ -284,22 +311,18 @@ cs_status enqueueLink(cs_context* ctx, const u64* leaves, const u32* dNumLeaves,
 {
     StageTimer t(ctx, CS_STAGE_LINK, s);
     DeviceCtrl* ctrl = ctx->ctrl;
-    // reset the link part of the control block (levelTotals, ticket)
-    CS_CUDA(ctx, cudaMemsetAsync(&ctrl->linkTicket, 0, sizeof(u32), s));
-    CS_CUDA(ctx, cudaMemsetAsync(ctrl->levelTotals, 0, sizeof(u32) * kLinkBins, s));
+    u32* tileHist = ctx->linkTileHist;                              // [tiles][kLinkBins]
     const u32 persistentGrid = (u32)ctx->numSMs * 8;
-    u32 gridA = divUp((u64)leafBound, kLinkBlock);
-    if (gridA > persistentGrid) gridA = persistentGrid;
-    if (gridA == 0) gridA = 1;
-    linkCountKernel<<<gridA, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves);
+    u32 grid = divUp((u64)leafBound, kLinkTile);
+    if (grid > persistentGrid) grid = persistentGrid;
+    if (grid == 0) grid = 1;
+    linkCountKernel<<<grid, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkCountKernel");
-    u32 gridB = divUp((u64)leafBound, kLinkTile);
-    if (gridB > persistentGrid) gridB = persistentGrid;
-    if (gridB == 0) gridB = 1;
-    const u32 epoch = nextEpoch(ctx, s);
+    linkScanKernel<<<kLinkBins, 256, 0, s>>>(ctrl, dNumLeaves, hNumLeaves, tileHist);
+    CS_LAUNCH_CHECK(ctx, "linkScanKernel");
     LinkOut out{prefixes, levels, childOffsets, parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity,
                 leafOffsets, leafOffsets ? nodeFirst : nullptr, nodeCount};
-    linkEmitKernel<<<gridB, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, out, ctx->tileLookback, epoch);
+    linkEmitKernel<<<grid, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, out, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkEmitKernel");
     return CS_OK;
 }
