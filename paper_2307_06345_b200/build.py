@@ -21,6 +21,8 @@ HEADERS = ["cs_internal.cuh", "cs_device.cuh", os.path.join("..", "..", "include
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-Xptxas", "-warn-spills"]
+# tuning overrides for experiments, e.g. CS_DEFINES="-DCS_SORT_BLOCK=384 -DCS_SORT_ITEMS=20"
+FLAGS += os.environ.get("CS_DEFINES", "").split()
 
 
 def _newest_header() -> float:

@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, tileLookback, linkTileHist, ctrl, total;
+        leafOffFinal, leafTasks, divLevel, tileLookback, linkTileHist, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -41,7 +41,9 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = alignUp(o + bytes); return at; };
     const size_t sortTiles = (maxParticles + kSortTile - 1) / kSortTile + 1;
-    const size_t leafTiles = ((size_t)maxLeaves + 1 + kLeafTile - 1) / kLeafTile + 1;
+    const size_t leafTiles = ((size_t)maxLeaves + 1 + 1023) / 1024 + 1;   // covers kLeafTile, kScanTile >= 1024
+    const size_t linkTiles = ((size_t)maxLeaves + kLinkTile - 1) / kLinkTile + 1;
+    static_assert(kLeafTile >= 1024 && kScanTile >= 1024, "look-back array is sized for tiles of >= 1024");
     L.keysAlt = take(maxParticles * sizeof(u64));
     L.permAlt = take(maxParticles * sizeof(u32));
     L.sortHist = take((kSortPasses * kRadix + 64) * sizeof(u32));
@@ -54,8 +56,9 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafOff1 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOffFinal = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint2));   // linear list, search list
+    L.divLevel = take(maxParticles + 256);                                 // 1 byte per particle
     L.tileLookback = take(leafTiles * sizeof(u64));                        // one counter per tile (leaf rounds, scan)
-    L.linkTileHist = take(leafTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
+    L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
     return L;
@@ -205,6 +208,7 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->leafOff[1] = (u32*)(ctx->slab + L.leafOff1);
     ctx->leafOffFinal = (u32*)(ctx->slab + L.leafOffFinal);
     ctx->leafTasks = (uint2*)(ctx->slab + L.leafTasks);
+    ctx->divLevel = (unsigned char*)(ctx->slab + L.divLevel);
     ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);

@@ -23,14 +23,20 @@ constexpr int kRoundSlots = kMaxRounds + 2;
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = 8;               // 63 key bits, 8 bits per pass
-constexpr int kSortBlock = 512;
-constexpr int kSortItems = 15;
+#ifndef CS_SORT_BLOCK
+#define CS_SORT_BLOCK 512
+#endif
+#ifndef CS_SORT_ITEMS
+#define CS_SORT_ITEMS 15
+#endif
+constexpr int kSortBlock = CS_SORT_BLOCK;
+constexpr int kSortItems = CS_SORT_ITEMS;
 constexpr int kSortTile = kSortBlock * kSortItems;   // 7680 keys per tile
 
 // ---- leaf refinement / link geometry -------------------------------------------------
 constexpr int kLeafBlock = 256;
-constexpr int kLeafItems = 4;
-constexpr int kLeafTile = kLeafBlock * kLeafItems;   // 1024 leaves per tile
+constexpr int kLeafItems = 8;
+constexpr int kLeafTile = kLeafBlock * kLeafItems;   // 2048 leaves per tile
 
 constexpr int kLinkBlock = 256;
 constexpr int kLinkItems = 4;
@@ -94,6 +100,7 @@ struct cs_context {
     // leaves
     cs::u64* leafK[2] = {nullptr, nullptr};
     cs::u32* leafOff[2] = {nullptr, nullptr};
+    unsigned char* divLevel = nullptr; // D[i] = number of leading octal digits shared by P[i-1] and P[i] (D[0] = 0)
     uint2* leafTasks = nullptr;        // (first child slot, end of the parent's particle range) per split leaf
     cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries

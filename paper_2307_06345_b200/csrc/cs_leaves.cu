@@ -16,6 +16,38 @@ namespace cs {
 
 __device__ __forceinline__ u32 ldVolatile(const u32* p) { return *(const volatile u32*)p; }
 
+// ---- divergence levels ----------------------------------------------------------------------------
+// D[i] = number of leading octal digits that the sorted neighbours P[i-1] and P[i] share (21 for
+// equal keys; D[0] = 0).  Inside a node of level l every D is >= l, and the positions with
+// D == l are exactly the places where the node's particles change child octant.  One byte per
+// particle, written once per sorted array: the refinement rounds then locate the child
+// boundaries of short leaves by scanning bytes instead of re-reading 8-byte keys every round.
+__global__ void __launch_bounds__(256) divergenceKernel(const u64* __restrict__ P, u32 n, unsigned char* __restrict__ D)
+{
+    const u32 lane = laneId();
+    const u32 pairs = (n + 1) >> 1;
+    const u32 stride = gridDim.x * blockDim.x;
+    const u32 rounds = (pairs + stride - 1) / stride;            // warp-uniform trip count (shuffles inside)
+    for (u32 it = 0; it < rounds; ++it) {
+        const u32 t = it * stride + blockIdx.x * blockDim.x + threadIdx.x;
+        const u32 i = 2 * t;
+        u64 a = 0, b = 0;
+        if (i + 1 < n) {
+            const ulonglong2 v = ldStreamU2(P + i);
+            a = v.x;
+            b = v.y;
+        } else if (i < n) a = ldStreamU64(P + i);
+        u64 prev = __shfl_up_sync(kFull, b, 1);
+        if (lane == 0) prev = (i > 0 && i < n) ? P[i - 1] : a;
+        if (i < n) {
+            const u32 d0 = i == 0 ? 0u : (u32)(__clzll((long long)(prev ^ a)) - 1) / 3u;
+            const u32 d1 = (u32)(__clzll((long long)(a ^ b)) - 1) / 3u;
+            if (i + 1 < n) *reinterpret_cast<unsigned short*>(D + i) = (unsigned short)(d0 | (d1 << 8));
+            else D[i] = (unsigned char)d0;
+        }
+    }
+}
+
 // ---- start arrays -----------------------------------------------------------------------------
 __global__ void leavesInitRootKernel(DeviceCtrl* ctrl, u64* K0, u32* off0, u32 n)
 {
@@ -78,9 +110,12 @@ __global__ void __launch_bounds__(kLeafBlock)
     const u32 nl = ctrl->nl[r];
     const u32 tiles = (nl + kLeafTile - 1) / kLeafTile;
     const u32 tid = threadIdx.x;
+    // Tiles are handed out by an atomic ticket (a tile only waits for tiles that already run).  The
+    // ticket of the NEXT tile is drawn by the last thread while the current tile is in flight, so
+    // its round trip is off the critical path.
+    u32 nextTicket = 0;
+    if (tid == kLeafBlock - 1) sTile = atomicAdd(&ctrl->ticket[r], 1u);
     for (;;) {
-        __syncthreads();
-        if (tid == 0) sTile = atomicAdd(&ctrl->ticket[r], 1u);
         __syncthreads();
         const u32 tile = sTile;
         if (tile >= tiles) break;
@@ -94,6 +129,7 @@ __global__ void __launch_bounds__(kLeafBlock)
             K[k] = i <= nl ? Kin[i] : kKeyEnd;
             off[k] = i <= nl ? offIn[i] : n;
         }
+        if (tid == kLeafBlock - 1) nextTicket = atomicAdd(&ctrl->ticket[r], 1u);
         // g1: rebalance decision (Eq. 5)
         u32 O[kLeafItems];
         u32 sum = 0, splits = 0;
@@ -108,7 +144,7 @@ __global__ void __launch_bounds__(kLeafBlock)
                 o = 1;
                 if (cnt > bucket && delta > 1) o = 8;                    // split (A7: not at depth L)
                 else if (delta != kKeyEnd) {                             // the root never merges (A9)
-                    const u32 j = (u32)(K[k] / delta) & 7u;              // octant index among siblings
+                    const u32 j = (u32)(K[k] >> (__ffsll((long long)delta) - 1)) & 7u;   // octant among siblings (delta = 8^m)
                     if (j != 0 && i >= j && i - j + 8 <= nl) {
                         const u32 a = i - j;
                         if (Kin[a + 8] - Kin[a] == (delta << 3)) {       // all 8 siblings are leaves
@@ -202,14 +238,16 @@ __global__ void __launch_bounds__(kLeafBlock)
                 }
             }
         }
+        __syncthreads();                                     // everyone is done with sTile / sPrefix
+        if (tid == kLeafBlock - 1) sTile = nextTicket;
     }
 }
 
 // ---- one round, kernel 2: f for the new boundaries (Eq. 3) ------------------------------------------
 // A split leaf with particle range [lo, hi) needs lower_bound(P, K'[p + c]) for c = 1..7, all
 // inside [lo, hi).  Work unit = (task, c), one warp each:
-//   * short ranges (<= kLinearMax keys): the warp of c = 1 streams the range once with coalesced
-//     loads and counts, with 7 ballots per 32 keys, how many keys fall below each child boundary.
+//   * short ranges (<= kLinearMax keys): 8 lanes scan the range's divergence bytes (see
+//     divergenceKernel) for changes of child octant; only the hits touch the keys.
 //   * long ranges: a 32-ary search, 32 probes per step (5 bits of the range per dependent
 //     memory round trip instead of 1).
 __device__ __forceinline__ u32 warpLowerBound32(const u64* __restrict__ P, u32 lo, u32 hi, u64 key, u32 lane)
@@ -232,8 +270,8 @@ __device__ __forceinline__ u32 warpLowerBound32(const u64* __restrict__ P, u32 l
 }
 
 __global__ void __launch_bounds__(256)
-    leafSearchKernel(const DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const u64* __restrict__ Kout,
-                     u32* __restrict__ offOut, const uint2* __restrict__ tasksLin,
+    leafSearchKernel(const DeviceCtrl* ctrl, const u64* __restrict__ P, const unsigned char* __restrict__ D,
+                     const u64* __restrict__ Kout, u32* __restrict__ offOut, const uint2* __restrict__ tasksLin,
                      const uint2* __restrict__ tasksSearch, u32 maxTasks, u32 r)
 {
     if (ctrl->status == CS_ERR_CAPACITY || ctrl->status == CS_ERR_NOT_CORNERSTONE) return;   // task lists incomplete
@@ -244,57 +282,55 @@ __global__ void __launch_bounds__(256)
     const u32 warpsPerGrid = gridDim.x * (blockDim.x >> 5);
     const u32 warpId = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
 
-    // ---- short ranges: 8 lanes per task, 4 tasks per warp, 128-bit coalesced loads; every lane keeps
-    // a packed 8 x 16-bit histogram of the child octant of its keys, folded over the 8 lanes at the end
+    // ---- short ranges: 8 lanes per task, 4 tasks per warp.  The lanes scan the divergence bytes of
+    // the range, 16 per load, for D == level (a change of child octant); the few hits read the two
+    // neighbouring keys and record the boundary for every child index the change skips ------------
     const u32 gl = lane & 7u;
     for (u32 t0 = warpId * 4u; t0 < numLin; t0 += warpsPerGrid * 4u) {
         const u32 t = t0 + (lane >> 3);
         const bool valid = t < numLin;
-        u32 p = 0, lo = 0, hi = 0;
-        u64 base = 0;
+        u32 p = 0, lo = 0, hi = 0, level = 0;
         int sh = 0;
         if (valid) {
             const uint2 task = tasksLin[t];
             p = task.x;
             hi = task.y;
             lo = offOut[p];
-            base = Kout[p];
-            sh = __ffsll((long long)(Kout[p + 1] - base)) - 1;            // child length is a power of 8
+            sh = __ffsll((long long)(Kout[p + 1] - Kout[p])) - 1;         // child length = 8^(sh/3)
+            level = (u32)kL - 1u - (u32)sh / 3u;                          // level of the split leaf
         }
-        const u32 a0 = lo & ~1u;                                          // 16-byte aligned start
-        u32 iters = valid ? (hi - a0 + 15u) / 16u : 0u;
+        const bool nonEmpty = hi > lo;                                    // a split leaf always has particles
+        if (valid && nonEmpty && gl == 0) {                               // ends of the range
+            const u32 cf = (u32)(__ldg(P + lo) >> sh) & 7u;
+            const u32 cl = (u32)(__ldg(P + hi - 1) >> sh) & 7u;
+            for (u32 c = 1; c <= cf; ++c) offOut[p + c] = lo;
+            for (u32 c = cl + 1; c < 8; ++c) offOut[p + c] = hi;
+        }
+        // interior positions lo < i < hi with D[i] == level
+        const u32 a0 = (lo + 1u) & ~15u;                                  // 16-byte aligned start
+        u32 iters = (valid && hi > lo + 1u) ? (hi - a0 + 127u) / 128u : 0u;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) iters = max(iters, __shfl_xor_sync(kFull, iters, o));
-        u64 h0 = 0, h1 = 0;                                               // children 0-3 / 4-7, 16 bits each
-        auto add = [&](u64 key) {
-            const u32 c = (u32)((key - base) >> sh);                      // 0..7 inside the parent's range
-            const u64 one = 1ull << ((c & 3u) * 16u);
-            if (c & 4u) h1 += one;
-            else h0 += one;
-        };
+        const u32 want = level * 0x01010101u;
         for (u32 it = 0; it < iters; ++it) {
-            const u32 idx = a0 + it * 16u + gl * 2u;
-            if (idx + 1 < hi) {                                           // both elements inside [.., hi)
-                const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(P + idx);
-                if (idx >= lo) add(v.x);
-                add(v.y);
-            } else if (idx < hi && idx >= lo) {
-                add(__ldg(P + idx));
-            }
-        }
+            const u32 i0 = a0 + it * 128u + gl * 16u;
+            if (!valid || i0 >= hi) continue;
+            const uint4 v = *reinterpret_cast<const uint4*>(D + i0);
+            const u32 w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int o = 1; o < 8; o <<= 1) {
-            h0 += __shfl_xor_sync(kFull, h0, o);
-            h1 += __shfl_xor_sync(kFull, h1, o);
-        }
-        if (valid && gl >= 1) {                                           // lane c: keys in children < c
-            u32 below = 0;
-#pragma unroll
-            for (u32 c = 0; c < 7; ++c) {
-                const u32 cnt = (u32)(((c < 4 ? h0 : h1) >> ((c & 3u) * 16u)) & 0xFFFFu);
-                if (c < gl) below += cnt;
+            for (int q = 0; q < 4; ++q) {
+                u32 eq = __vcmpeq4(w[q], want);                           // 0xFF in every byte equal to level
+                while (eq) {
+                    const u32 byte = (__ffs((int)eq) - 1) >> 3;
+                    eq &= ~(0xFFu << (byte * 8));
+                    const u32 i = i0 + q * 4u + byte;
+                    if (i > lo && i < hi) {
+                        const u32 c0 = (u32)(__ldg(P + i - 1) >> sh) & 7u;
+                        const u32 c1 = (u32)(__ldg(P + i) >> sh) & 7u;
+                        for (u32 c = c0 + 1; c <= c1; ++c) offOut[p + c] = i;
+                    }
+                }
             }
-            offOut[p + gl] = lo + below;
         }
     }
 
@@ -338,6 +374,12 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
     DeviceCtrl* ctrl = ctx->ctrl;
     CS_CUDA(ctx, cudaMemsetAsync(ctrl, 0, sizeof(DeviceCtrl), s));
     const u32 persistentGrid = (u32)ctx->numSMs * 8;
+    if (n) {
+        u32 g = divUp((n + 1) / 2, 256);
+        if (g > persistentGrid) g = persistentGrid;
+        divergenceKernel<<<g, 256, 0, s>>>(P, (u32)n, ctx->divLevel);
+        CS_LAUNCH_CHECK(ctx, "divergenceKernel");
+    }
     if (prevLeaves) {
         u32 grid = divUp((u64)prevNumLeaves + 1, 256);
         if (grid > persistentGrid) grid = persistentGrid;
@@ -371,7 +413,7 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
             u32 bound = divUp(7ull << (3 * r), 8);
             if (bound < gs) gs = bound;
         }
-        leafSearchKernel<<<gs, 256, 0, s>>>(ctrl, P, (u32)n, ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
+        leafSearchKernel<<<gs, 256, 0, s>>>(ctrl, P, ctx->divLevel, ctx->leafK[(r + 1) & 1], ctx->leafOff[(r + 1) & 1],
                                             ctx->leafTasks, ctx->leafTasks + ctx->maxTasks, ctx->maxTasks, r);
         CS_LAUNCH_CHECK(ctx, "leafSearchKernel");
     }

@@ -80,6 +80,34 @@ struct SortSmem {
     u32 tile;
 };
 
+constexpr int kLookBatch = 4;            // predecessors fetched per look-back round trip
+
+// Exclusive prefix of counter c over tiles < tile.  The words of kLookBatch predecessors are
+// requested together, so one memory round trip covers kLookBatch tiles.
+__device__ __forceinline__ u32 lookBackBatched(const u64* state, u32 c, u32 tile, u32 epoch)
+{
+    u32 excl = 0;
+    int p = (int)tile - 1;
+    while (p >= 0) {
+        u64 w[kLookBatch];
+#pragma unroll
+        for (int i = 0; i < kLookBatch; ++i)
+            if (p - i >= 0) w[i] = lbLoad(state + (size_t)(p - i) * kRadix + c);
+#pragma unroll
+        for (int i = 0; i < kLookBatch; ++i) {
+            if (p - i < 0) return excl;
+            while ((u32)(w[i] >> 34) != (epoch & 0x3FFFFFFFu)) {
+                __nanosleep(32);
+                w[i] = lbLoad(state + (size_t)(p - i) * kRadix + c);
+            }
+            excl += (u32)w[i];
+            if (((u32)(w[i] >> 32) & 3u) == kLbPrefix) return excl;
+        }
+        p -= kLookBatch;
+    }
+    return excl;
+}
+
 template <bool FIRST>
 __global__ void __launch_bounds__(kSortBlock, 2)
     onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
@@ -110,7 +138,9 @@ __global__ void __launch_bounds__(kSortBlock, 2)
     // ---- rank inside the warp: peers holding the same digit are found with 8 ballots (one per digit
     // bit; the native match.any is far slower), every peer reads the warp's running count of its
     // digit (a shared-memory broadcast) and the lowest peer bumps it once ---------------------------
-    u32 rank[kSortItems];
+    u32 rankPk[(kSortItems + 1) / 2];                                        // two 16-bit ranks per register
+#pragma unroll
+    for (int j = 0; j < (kSortItems + 1) / 2; ++j) rankPk[j] = 0;
     u32* wh = sm.warpHist[warp];
     const u32 lt = laneMaskLt();
 #pragma unroll
@@ -128,7 +158,7 @@ __global__ void __launch_bounds__(kSortBlock, 2)
         __syncwarp();
         if (lower == 0) wh[d] = prev + __popc(peers);
         __syncwarp();
-        rank[j] = prev + lower;
+        rankPk[j >> 1] |= (prev + lower) << ((j & 1) * 16);
     }
     __syncthreads();
 
@@ -143,59 +173,58 @@ __global__ void __launch_bounds__(kSortBlock, 2)
             run += c;
         }
         count = run;
+        // publish this tile's count at once: the tiles behind it can start their look-back
+        const u32 real = tid == kRadix - 1 ? count - (kSortTile - valid) : count;     // pads are not elements
+        lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, tile == 0 ? kLbPrefix : kLbAggregate, real));
     }
     u32 total;
     u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
     if (tid < kRadix) {
         sm.digitStart[tid] = start;
-        if (tid == kRadix - 1) count -= (kSortTile - valid);    // pads are not real elements
-        // ---- decoupled look-back over preceding tiles, one thread per digit ------------------
-        u64* st = lookback + (size_t)tile * kRadix + tid;
+        // ---- decoupled look-back over preceding tiles, one thread per digit ----------------------
         u32 excl = 0;
-        if (tile == 0) lbStore(st, lbPack(epoch, kLbPrefix, count));
-        else {
-            lbStore(st, lbPack(epoch, kLbAggregate, count));
-            excl = lbLookBack(lookback, kRadix, tid, tile, epoch);
-            lbStore(st, lbPack(epoch, kLbPrefix, excl + count));
+        if (tile != 0) {
+            const u32 real = tid == kRadix - 1 ? count - (kSortTile - valid) : count;
+            excl = lookBackBatched(lookback, tid, tile, epoch);
+            lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, kLbPrefix, excl + real));
         }
         sm.globalBase[tid] = digitBase[tid] + excl - start;
     }
     __syncthreads();
 
-    // ---- scatter keys into digit order in shared memory -----------------------------------------
+    // ---- scatter keys, then values, into digit order in shared memory -----------------------------
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         u32 d = digitOf(key[j], shift);
-        u32 pos = sm.digitStart[d] + wh[d] + rank[j];
+        const u32 r = (rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
+        const u32 pos = sm.digitStart[d] + wh[d] + r;
         sm.keys[pos] = key[j];
-        rank[j] = pos;
+        if (j & 1) rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFFu) | (pos << 16);
+        else rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFF0000u) | pos;
     }
+    // values: pass 0 synthesises the identity permutation instead of reading it
+    asm volatile("" ::: "memory");        // keep the value loads behind the key scatter (register pressure)
+    u32 val[kSortItems];
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) {
+        u32 loc = warpOff + j * 32;
+        if (FIRST) val[j] = (u32)base + loc;
+        else val[j] = (full || loc < valid) ? ldStreamU32(valsIn + base + loc) : 0u;
+    }
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j) sm.vals[(rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu] = val[j];
     __syncthreads();
 
-    // ---- write keys: consecutive threads -> consecutive slots of a digit's run -------------------
+    // ---- write out: consecutive threads -> consecutive slots of a digit's run ----------------------
 #pragma unroll
     for (int k = 0; k < kSortItems; ++k) {
         u32 i = tid + k * kSortBlock;
         if (i < valid) {
-            u64 kk = sm.keys[i];
-            keysOut[sm.globalBase[digitOf(kk, shift)] + i] = kk;
+            const u64 kk = sm.keys[i];
+            const u32 dst = sm.globalBase[digitOf(kk, shift)] + i;
+            keysOut[dst] = kk;
+            valsOut[dst] = sm.vals[i];
         }
-    }
-
-    // ---- values: pass 0 synthesises the identity permutation instead of reading it -----------
-#pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
-        u32 loc = warpOff + j * 32;
-        u32 v;
-        if (FIRST) v = (u32)base + loc;
-        else v = (full || loc < valid) ? ldStreamU32(valsIn + base + loc) : 0u;
-        sm.vals[rank[j]] = v;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int k = 0; k < kSortItems; ++k) {
-        u32 i = tid + k * kSortBlock;
-        if (i < valid) valsOut[sm.globalBase[digitOf(sm.keys[i], shift)] + i] = sm.vals[i];
     }
 }
 
