@@ -108,36 +108,45 @@ __device__ __forceinline__ u32 lookBackBatched(const u64* state, u32 c, u32 tile
     return excl;
 }
 
-template <bool FIRST>
-__global__ void __launch_bounds__(kSortBlock, 2)
-    onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
-                   u32* __restrict__ valsOut, u32 n, int shift, const u32* __restrict__ digitBase /*scanned hist*/,
-                   u32* ticket, u64* lookback, u32 epoch)
+// Lanes of the warp whose 8-bit digit equals this lane's: one ballot per digit bit (the native match.any
+// is far slower).  Per bit: s = bit ? ~0 : 0 (bfe.s32), p = (s != 0), v = ballot(p), peers &= ~(v ^ s).
+__device__ __forceinline__ u32 matchDigit(u32 d)
 {
-    extern __shared__ __align__(16) unsigned char smemRaw[];
-    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
-    const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
+    u32 peers = kFull;
+#pragma unroll
+    for (int b = 0; b < kRadixBits; ++b) {
+        asm("{\n\t"
+            ".reg .pred p;\n\t"
+            ".reg .b32 s, v;\n\t"
+            "bfe.s32 s, %1, %2, 1;\n\t"
+            "setp.ne.s32 p, s, 0;\n\t"
+            "vote.sync.ballot.b32 v, p, 0xffffffff;\n\t"
+            "lop3.b32 %0, %0, v, s, 0x90;\n\t"
+            "}"
+            : "+r"(peers)
+            : "r"(d), "r"(b));
+    }
+    return peers;
+}
 
-    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < kSortWarps * kRadix; i += kSortBlock) (&sm.warpHist[0][0])[i] = 0;
-    __syncthreads();
-    const u32 tile = sm.tile;
+template <bool FIRST, bool FULL>
+__device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict__ keysIn, const u32* __restrict__ valsIn,
+                                             u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
+                                             int shift, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
+{
+    const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
     const u64 base = (u64)tile * kSortTile;
-    const u32 valid = (u32)((n - base) < (u64)kSortTile ? (n - base) : (u64)kSortTile);
-    const bool full = valid == kSortTile;
 
     // ---- load: warp-striped, so that (warp, item, lane) order == memory order (stability) ----
     u64 key[kSortItems];
     const u32 warpOff = warp * (32 * kSortItems) + lane;
+    const u64* src = keysIn + base + warpOff;
 #pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
-        u32 loc = warpOff + j * 32;
-        key[j] = (full || loc < valid) ? ldStreamU64(keysIn + base + loc) : ~0ull;   // pads sort last
-    }
+    for (int j = 0; j < kSortItems; ++j)
+        key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU64(src + j * 32) : ~0ull;   // pads sort last
 
-    // ---- rank inside the warp: peers holding the same digit are found with 8 ballots (one per digit
-    // bit; the native match.any is far slower), every peer reads the warp's running count of its
-    // digit (a shared-memory broadcast) and the lowest peer bumps it once ---------------------------
+    // ---- rank inside the warp: every peer reads the warp's running count of its digit (a
+    // shared-memory broadcast) and the lowest peer bumps it once ------------------------------------
     u32 rankPk[(kSortItems + 1) / 2];                                        // two 16-bit ranks per register
 #pragma unroll
     for (int j = 0; j < (kSortItems + 1) / 2; ++j) rankPk[j] = 0;
@@ -146,13 +155,7 @@ __global__ void __launch_bounds__(kSortBlock, 2)
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], shift);
-        u32 peers = kFull;
-#pragma unroll
-        for (int b = 0; b < kRadixBits; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const u32 vote = __ballot_sync(kFull, bit);
-            peers &= bit ? vote : ~vote;
-        }
+        const u32 peers = matchDigit(d);
         const u32 lower = __popc(peers & lt);
         const u32 prev = wh[d];
         __syncwarp();
@@ -174,7 +177,7 @@ __global__ void __launch_bounds__(kSortBlock, 2)
         }
         count = run;
         // publish this tile's count at once: the tiles behind it can start their look-back
-        const u32 real = tid == kRadix - 1 ? count - (kSortTile - valid) : count;     // pads are not elements
+        const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;   // pads are not elements
         lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, tile == 0 ? kLbPrefix : kLbAggregate, real));
     }
     u32 total;
@@ -184,7 +187,7 @@ __global__ void __launch_bounds__(kSortBlock, 2)
         // ---- decoupled look-back over preceding tiles, one thread per digit ----------------------
         u32 excl = 0;
         if (tile != 0) {
-            const u32 real = tid == kRadix - 1 ? count - (kSortTile - valid) : count;
+            const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;
             excl = lookBackBatched(lookback, tid, tile, epoch);
             lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, kLbPrefix, excl + real));
         }
@@ -205,11 +208,11 @@ __global__ void __launch_bounds__(kSortBlock, 2)
     // values: pass 0 synthesises the identity permutation instead of reading it
     asm volatile("" ::: "memory");        // keep the value loads behind the key scatter (register pressure)
     u32 val[kSortItems];
+    const u32* vsrc = valsIn + base + warpOff;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        u32 loc = warpOff + j * 32;
-        if (FIRST) val[j] = (u32)base + loc;
-        else val[j] = (full || loc < valid) ? ldStreamU32(valsIn + base + loc) : 0u;
+        if (FIRST) val[j] = (u32)base + warpOff + j * 32;
+        else val[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU32(vsrc + j * 32) : 0u;
     }
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) sm.vals[(rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu] = val[j];
@@ -218,14 +221,35 @@ __global__ void __launch_bounds__(kSortBlock, 2)
     // ---- write out: consecutive threads -> consecutive slots of a digit's run ----------------------
 #pragma unroll
     for (int k = 0; k < kSortItems; ++k) {
-        u32 i = tid + k * kSortBlock;
-        if (i < valid) {
+        const u32 i = tid + k * kSortBlock;
+        if (FULL || i < valid) {
             const u64 kk = sm.keys[i];
             const u32 dst = sm.globalBase[digitOf(kk, shift)] + i;
             keysOut[dst] = kk;
             valsOut[dst] = sm.vals[i];
         }
     }
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(kSortBlock, 2)
+    onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
+                   u32* __restrict__ valsOut, u32 n, int shift, const u32* __restrict__ digitBase /*scanned hist*/,
+                   u32* ticket, u64* lookback, u32 epoch)
+{
+    extern __shared__ __align__(16) unsigned char smemRaw[];
+    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    const u32 tid = threadIdx.x;
+    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+    for (int i = tid; i < kSortWarps * kRadix; i += kSortBlock) (&sm.warpHist[0][0])[i] = 0;
+    __syncthreads();
+    const u32 tile = sm.tile;
+    const u64 base = (u64)tile * kSortTile;
+    const u32 valid = (u32)((n - base) < (u64)kSortTile ? (n - base) : (u64)kSortTile);
+    if (valid == kSortTile)
+        onesweepTile<FIRST, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, shift, digitBase, lookback, epoch);
+    else
+        onesweepTile<FIRST, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, shift, digitBase, lookback, epoch);
 }
 
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
