@@ -158,41 +158,47 @@ cs_status enqueueBox(cs_context* ctx, const double* x, const double* y, const do
 // ---------------------------------------------------------------------------------------------
 // H2: Morton keys.  g = clamp(floor(((c - lo) / e) * 2^21), 0, 2^21 - 1) with explicitly
 // rounded intrinsics (__dsub_rn, __ddiv_rn, __dmul_rn are never contracted into FMAs), then
-// the 21 bits of each coordinate are spread to every third bit with 5 shift-or-mask steps.
-// cvt.rmi.s64.f64 saturates and maps NaN (0/0 of a flat box) to 0, which is reading A1.
+// the 21 bits of each coordinate are spread to every third bit with shift-or-mask steps on
+// 32-bit halves.  cvt.rmi.s32.f64 saturates and maps NaN (0/0 of a flat box) to 0: reading A1.
 // Optionally (HIST) the 8 radix-digit histograms of the sort are accumulated on the fly,
 // saving the sort a pass over the keys.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ u64 spread21(u64 v)
+// 11 bits -> every third bit of a 32-bit word (bit b -> bit 3b)
+__device__ __forceinline__ u32 spread11(u32 v)
 {
-    v &= 0x1fffffull;
-    v = (v | (v << 32)) & 0x001f00000000ffffull;
-    v = (v | (v << 16)) & 0x001f0000ff0000ffull;
-    v = (v | (v << 8)) & 0x100f00f00f00f00full;
-    v = (v | (v << 4)) & 0x10c30c30c30c30c3ull;
-    v = (v | (v << 2)) & 0x1249249249249249ull;
+    v &= 0x7FFu;
+    v = (v | (v << 16)) & 0x070000FFu;
+    v = (v | (v << 8)) & 0x0700F00Fu;
+    v = (v | (v << 4)) & 0x430C30C3u;
+    v = (v | (v << 2)) & 0x49249249u;
     return v;
 }
 
-__device__ __forceinline__ u64 gridCoordinate(double c, double lo, double e)
+// floor and clamp in 32-bit: cvt.rmi.s32.f64 saturates (+-inf, huge) and maps NaN to 0
+__device__ __forceinline__ u32 gridCoordinate(double c, double lo, double e)
 {
-    double t = __dmul_rn(__ddiv_rn(__dsub_rn(c, lo), e), 2097152.0);
-    long long g = __double2ll_rd(t);
-    g = g < 0 ? 0 : g;
-    g = g > 2097151 ? 2097151 : g;
-    return (u64)g;
+    const double t = __dmul_rn(__ddiv_rn(__dsub_rn(c, lo), e), 2097152.0);
+    int g = __double2int_rd(t);
+    g = max(g, 0);
+    g = min(g, 2097151);
+    return (u32)g;
 }
 
 struct BoxParams {
     double lo[3], e[3];
 };
 
+// Interleave as two 32-bit words (all spreading in 32-bit arithmetic):
+//   key bit 3b+2 = x bit b, 3b+1 = y bit b, 3b = z bit b   (digit = 4x + 2y + z, A3)
+//   low word : x bits 0..9, y bits 0..10, z bits 0..10;  high word: x bits 10..20, y and z bits 11..20
 __device__ __forceinline__ u64 mortonKey(double x, double y, double z, const BoxParams& b)
 {
-    u64 gx = gridCoordinate(x, b.lo[0], b.e[0]);
-    u64 gy = gridCoordinate(y, b.lo[1], b.e[1]);
-    u64 gz = gridCoordinate(z, b.lo[2], b.e[2]);
-    return (spread21(gx) << 2) | (spread21(gy) << 1) | spread21(gz);   // digit = 4x + 2y + z (A3)
+    const u32 gx = gridCoordinate(x, b.lo[0], b.e[0]);
+    const u32 gy = gridCoordinate(y, b.lo[1], b.e[1]);
+    const u32 gz = gridCoordinate(z, b.lo[2], b.e[2]);
+    const u32 lo = (spread11(gx & 0x3FFu) << 2) | (spread11(gy) << 1) | spread11(gz);
+    const u32 hi = spread11(gx >> 10) | (spread11(gy >> 11) << 2) | (spread11(gz >> 11) << 1);
+    return ((u64)hi << 32) | lo;
 }
 
 template <bool HIST>
