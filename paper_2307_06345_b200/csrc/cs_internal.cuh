@@ -29,7 +29,11 @@ constexpr int kSortPasses = 8;               // 63 key bits, 8 bits per pass
 #ifndef CS_SORT_ITEMS
 #define CS_SORT_ITEMS 15
 #endif
+#ifndef CS_SORT_MINBLOCKS
+#define CS_SORT_MINBLOCKS 2
+#endif
 constexpr int kSortBlock = CS_SORT_BLOCK;
+constexpr int kSortMinBlocks = CS_SORT_MINBLOCKS;   // resident CTAs per SM the radix pass is compiled for
 constexpr int kSortItems = CS_SORT_ITEMS;
 constexpr int kSortTile = kSortBlock * kSortItems;   // 7680 keys per tile
 

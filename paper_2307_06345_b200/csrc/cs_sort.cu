@@ -232,7 +232,7 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
 }
 
 template <bool FIRST>
-__global__ void __launch_bounds__(kSortBlock, 2)
+__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
                    u32* __restrict__ valsOut, u32 n, int shift, const u32* __restrict__ digitBase /*scanned hist*/,
                    u32* ticket, u64* lookback, u32 epoch)
