@@ -129,6 +129,20 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
                          uint64_t* leaves, uint32_t* counts, uint32_t leafCapacity,
                          uint32_t* numLeaves, uint32_t* rounds, void* stream);
 
+/* cs_setLeafMode -- how cs_buildLeaves / cs_buildOctree reach the converged array when they
+ *   start from the root (prevLeaves == NULL, maxRounds == 0).  From {0, 8^21} the rounds of
+ *   PAPER.md:120-126 only ever split, so their fixpoint is the top-down tree "a node above
+ *   depth L is internal iff it holds more than bucketSize particles".
+ *   CS_LEAVES_AUTO (default): that fixpoint is computed in ONE pass over the sorted keys (a
+ *   node holds more than b particles iff it contains b+1 consecutive keys of P); leaves,
+ *   counts and `rounds` (deepest leaf level + 1) are identical to what the rounds return.
+ *   bucketSize > 1024 falls back to the rounds.
+ *   CS_LEAVES_ITERATIVE: always run the rounds f, g1, g2, g3 (Eqs. 3-9) literally.
+ *   Incremental starts (prevLeaves) and bounded round counts (maxRounds > 0) always use the
+ *   rounds.  Errors: INVALID_ARG. */
+enum { CS_LEAVES_AUTO = 0, CS_LEAVES_ITERATIVE = 1 };
+cs_status cs_setLeafMode(cs_context* ctx, int mode);
+
 /* cs_linkOctree -- the fully linked octree of Sec. 5, all levels in
  *   parallel, in the paper's format: node keys NK in Warren-Salmon placeholder-bit form
  *   (a 1 bit followed by `level` octal digits), connectivity CO (index of

@@ -107,6 +107,15 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
     return statusFromCtrl(ctx, "cs_buildLeaves");
 }
 
+cs_status cs_setLeafMode(cs_context* ctx, int mode)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setLeafMode: ctx is null");
+    if (mode != CS_LEAVES_AUTO && mode != CS_LEAVES_ITERATIVE)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_setLeafMode: unknown mode %d", mode);
+    ctx->leafMode = mode;
+    return CS_OK;
+}
+
 cs_status cs_linkOctree(cs_context* ctx, const uint64_t* leaves, uint32_t numLeaves, uint64_t* prefixes,
                         uint32_t* levels, uint32_t* childOffsets, uint32_t* parents, uint32_t* levelRange,
                         uint32_t* leafToNode, uint32_t* nodeToLeaf, uint32_t nodeCapacity, uint32_t* numNodes,

@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, divLevel, tileLookback, linkTileHist, ctrl, total;
+        leafOffFinal, leafTasks, divLevel, tileLookback, leafLookback, linkTileHist, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -58,6 +58,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint2));   // linear list, search list
     L.divLevel = take(maxParticles + 256);                                 // 1 byte per particle
     L.tileLookback = take(leafTiles * sizeof(u64));                        // one counter per tile (leaf rounds, scan)
+    L.leafLookback = take(((maxParticles >> kDirectTileLog2) + 2) * sizeof(u64));   // one-pass leaf build
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
@@ -211,6 +212,7 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->divLevel = (unsigned char*)(ctx->slab + L.divLevel);
     ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
+    ctx->leafLookback = (u64*)(ctx->slab + L.leafLookback);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
     *out = ctx;

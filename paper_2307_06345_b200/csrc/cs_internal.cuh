@@ -47,6 +47,10 @@ constexpr int kLinkItems = 4;
 constexpr int kLinkTile = kLinkBlock * kLinkItems;   // 1024 leaf boundaries per tile
 constexpr int kLinkBins = 2 * (kL + 1);              // per level: all nodes, internal nodes
 
+// one-pass leaf build (cs_leaves_direct.cu): particle boundaries per tile, largest bucketSize it takes
+constexpr int kDirectTileLog2 = 11;
+constexpr int kDirectMaxBucket = 1024;
+
 constexpr int kScanBlock = 256;
 constexpr int kScanItems = 8;
 constexpr int kScanTile = kScanBlock * kScanItems;
@@ -70,7 +74,8 @@ struct DeviceCtrl {
     u32 scanTicket;
     u32 levelTotals[kLinkBins];  // link: nodes per level (all / internal)
     u32 levelRange[kL + 2];
-    u32 pad[7];
+    u32 directBuild;             // the leaves in leafK[0] come from the one-pass build (cs_leaves_direct.cu)
+    u32 pad[6];
 };
 
 struct HostCtrl {                // pinned mirror read back once per call
@@ -109,6 +114,8 @@ struct cs_context {
     cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
     cs::u64* tileLookback = nullptr;   // [tiles] look-back words of the leaf rounds and the scan
+    cs::u64* leafLookback = nullptr;   // [maxParticles / 2^kDirectTileLog2 + 2] look-back words of the one-pass leaf build
+    int leafMode = 0;                  // cs_setLeafMode
     cs::u32* linkTileHist = nullptr;   // [tiles][kLinkBins] node counts per tile, level and kind
     cs::DeviceCtrl* ctrl = nullptr;
     cs::HostCtrl* hostCtrl = nullptr;  // pinned
@@ -175,6 +182,8 @@ cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool histReady, 
 cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
                         u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity,
                         cudaStream_t);
+bool leavesDirectSupported(const cs_context*, u32 bucketSize);
+cs_status enqueueLeavesDirect(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, u32 cap, cudaStream_t);
 // leaves/numLeaves: if dNumLeaves is null the host value is used
 cs_status enqueueLink(cs_context*, const u64* leaves, const u32* dNumLeaves, u32 hNumLeaves, u32 leafBound,
                       u64* prefixes, u32* levels, u32* childOffsets, u32* parents, u32* levelRange,

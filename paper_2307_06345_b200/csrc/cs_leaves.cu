@@ -355,8 +355,9 @@ __global__ void __launch_bounds__(256) leavesEmitKernel(const DeviceCtrl* ctrl, 
     if (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) return;   // outputs untouched
     const u32 rounds = ctrl->rounds;
     const u32 nl = ctrl->nl[rounds];
-    const u64* K = (rounds & 1) ? K1 : K0;
-    const u32* off = (rounds & 1) ? off1 : off0;
+    const bool second = (rounds & 1) && !ctrl->directBuild;      // the one-pass build always writes K0 / off0
+    const u64* K = second ? K1 : K0;
+    const u32* off = second ? off1 : off0;
     const u32 stride = gridDim.x * blockDim.x;
     for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i <= nl; i += stride) {
         const u32 o = off[i];
@@ -374,6 +375,17 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
     DeviceCtrl* ctrl = ctx->ctrl;
     CS_CUDA(ctx, cudaMemsetAsync(ctrl, 0, sizeof(DeviceCtrl), s));
     const u32 persistentGrid = (u32)ctx->numSMs * 8;
+    // From the root and to convergence the fixpoint is built in one pass over P (cs_leaves_direct.cu);
+    // the rounds below serve incremental starts, bounded round counts and cs_setLeafMode(ITERATIVE).
+    if (!prevLeaves && maxRounds == 0 && ctx->leafMode != CS_LEAVES_ITERATIVE && leavesDirectSupported(ctx, bucket)) {
+        CS_TRY(enqueueLeavesDirect(ctx, P, n, bucket, cap, s));
+        u32 g = divUp((u64)cap + 1, 256);
+        if (g > persistentGrid) g = persistentGrid;
+        leavesEmitKernel<<<g, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafK[1], ctx->leafOff[0], ctx->leafOff[1], leaves,
+                                           counts, ctx->leafOffFinal);
+        CS_LAUNCH_CHECK(ctx, "leavesEmitKernel");
+        return CS_OK;
+    }
     if (n) {
         u32 g = divUp((n + 1) / 2, 256);
         if (g > persistentGrid) g = persistentGrid;

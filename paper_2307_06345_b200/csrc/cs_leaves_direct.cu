@@ -1,0 +1,384 @@
+// H4-H8, start {0, 8^21}, run to convergence: the fixpoint of f and g in ONE pass over P.
+//
+// The iteration of PAPER.md:62-128 from the root only ever splits (a node is split iff it holds
+// more than N_crit particles and lies above depth L, and then its 8 children together hold more
+// than N_crit, so they never merge back: DESIGN.md A8), hence its fixpoint is the top-down tree:
+//   node (level l < L, prefix p) is internal  <=>  count(l, p) > N_crit                      (*)
+// and the leaves are the children of internal nodes that are not internal (plus the root if it
+// is not).  Because P is sorted, (*) can be decided from windows of b+1 = N_crit+1 consecutive
+// keys: a node holds more than b particles iff it contains such a window, so with
+//   w_i = min(#leading octal digits shared by P[i] and P[i+b], L-1)       (0 <= i < n-b)
+// the deepest internal node on the path of particle j has level
+//   d_j = max{ w_i : j-b <= i <= j }                                       (sliding maximum)
+// and the leaf that holds particle j has level D_j = d_j + 1 (D_j = 0, the root, if n <= b).
+// Between two neighbours a = P[j-1] < c = P[j] that fall into different leaves (they share
+// s < D_j digits) the leaf array K contains, in key order:
+//   the empty siblings to the right of a's ancestors on levels D_{j-1} .. s+2,
+//   the empty children of the common ancestor strictly between the two branches (level s+1),
+//   the empty siblings to the left of c's ancestors on levels s+2 .. D_j,
+//   the leaf of c.
+// All of them have lower_bound position j in P (Eq. 3), so N_i follows from the off[] array
+// like in the iterative path.  One kernel: per-tile counts, decoupled look-back across tiles,
+// emission.  Per tile: window levels and the sliding maximum run on bytes, four per 32-bit SIMD
+// operation; the positions where a leaf starts (one in ~18) are compacted with a block scan, so
+// the digit arithmetic of the counts and the emission run on a dense list.
+// rounds := (deepest leaf level) + 1 is what the iteration would have reported (one round per
+// level, plus the confirming one: DESIGN.md A12).
+#include "cs_device.cuh"
+
+namespace cs {
+
+#ifndef CS_DIR_MINBLOCKS
+#define CS_DIR_MINBLOCKS 4
+#endif
+constexpr int kDirBlock = 256;
+constexpr int kDirItems = 8;
+constexpr int kDirTile = kDirBlock * kDirItems;          // 2048 particle boundaries per tile
+static_assert(kDirTile == (1 << kDirectTileLog2), "look-back array of the context is sized for this tile");
+
+constexpr u64 kOct1 = 0x1249249249249249ull;             // bit 0 of every octal digit (bits 0, 3, ..., 60)
+
+// sum of the octal digits of key on levels lo..hi (1-based, digit l = bits [3(L-l), 3(L-l)+2]); 0 if lo > hi
+__device__ __forceinline__ u32 digitSum(u64 key, int lo, int hi)
+{
+    if (lo > hi) return 0;
+    const u64 upper = (lo <= 1) ? ~0ull >> 1 : ((1ull << (3 * (kL + 1 - lo))) - 1);
+    const u64 lower = (1ull << (3 * (kL - hi))) - 1;
+    const u64 m = key & upper & ~lower;
+    return __popcll(m & kOct1) + 2 * __popcll(m & (kOct1 << 1)) + 4 * __popcll(m & (kOct1 << 2));
+}
+__device__ __forceinline__ u32 digitAt(u64 key, int l) { return (u32)(key >> (3 * (kL - l))) & 7u; }
+__device__ __forceinline__ int sharedDigits(u64 a, u64 c) { return (__clzll((long long)(a ^ c)) - 1) / 3; }   // 21 if equal
+// the same from x = a ^ c (bit 63 clear): (clz - 1) / 3 for clz in 1..64, by multiplication
+__device__ __forceinline__ u32 sharedDigitsX(u64 x) { return ((u32)__clzll((long long)x) - 1u) * 43u >> 7; }
+
+// number of K entries owned by position j.  Da = D_{j-1}, Dc = D_j.
+__device__ __forceinline__ u32 dirCount(u64 a, u64 c, int Da, int Dc, u32 j, u32 n)
+{
+    if (j > n) return 0;
+    if (j == n) return (n ? 7u * Da - digitSum(a, 1, Da) : 1u) + 1u;      // right flank of the last particle, 8^21
+    if (j == 0) return digitSum(c, 1, Dc) + 1u;                            // left flank of the first particle, its leaf
+    const int s = sharedDigits(a, c);
+    if (s >= Dc) return 0;                                                 // same leaf
+    const u32 up = 7u * (u32)(Da - s - 1) - digitSum(a, s + 2, Da);
+    const u32 mid = digitAt(c, s + 1) - digitAt(a, s + 1) - 1u;
+    return up + mid + digitSum(c, s + 2, Dc) + 1u;
+}
+
+// write the K entries owned by position j to K[pos ..], off[pos ..] = j
+__device__ __noinline__ void dirEmit(u64 a, u64 c, int Da, int Dc, u32 j, u32 n, u32 pos, u64* __restrict__ K,
+                                        u32* __restrict__ off, u32 cap)
+{
+    auto put = [&](u64 key) {
+        if (pos <= cap) {
+            K[pos] = key;
+            off[pos] = j;
+        }
+        ++pos;
+    };
+    int s = -1;
+    if (j != 0 && j != n) s = sharedDigits(a, c);
+    if (j != 0) {                                          // siblings to the right of a's ancestors, deepest first
+        for (int l = Da; l >= s + 2; --l) {
+            const u64 step = 1ull << (3 * (kL - l));
+            const u64 parent = a & ~((step << 3) - 1);     // (step << 3) = 2^63 at l = 1: still a valid mask
+            for (u32 q = digitAt(a, l) + 1; q < 8; ++q) put(parent + q * step);
+        }
+    }
+    if (j == n) {
+        put(kKeyEnd);                                      // A11: terminal element
+        return;
+    }
+    if (j != 0) {                                          // empty children of the common ancestor between the branches
+        const int l = s + 1;
+        const u64 step = 1ull << (3 * (kL - l));
+        const u64 parent = a & ~((step << 3) - 1);
+        for (u32 q = digitAt(a, l) + 1; q < digitAt(c, l); ++q) put(parent + q * step);
+    }
+    for (int l = s + 2; l <= Dc; ++l) {                    // siblings to the left of c's ancestors, shallowest first
+        const u64 step = 1ull << (3 * (kL - l));
+        const u64 parent = c & ~((step << 3) - 1);
+        for (u32 q = 0; q < digitAt(c, l); ++q) put(parent + q * step);
+    }
+    put(Dc == 0 ? 0ull : c & ~((1ull << (3 * (kL - Dc))) - 1));   // the leaf of c
+}
+
+// dynamic shared memory: keys of [T0 - b - 1, T0 + T + b), window levels (two byte arrays for the
+// doubling steps of the sliding maximum), neighbour levels s[p], list of leaf-start positions
+struct DirLayout {
+    u32 nKeys, wWords, offW0, offW1, offS, offList, total;
+};
+__host__ __device__ inline DirLayout dirLayout(u32 b)
+{
+    DirLayout L;
+    L.nKeys = kDirTile + 2 * b + 1;
+    u32 p2 = 1;
+    while (p2 * 2 <= b + 1) p2 *= 2;                       // largest power of two <= window length b+1
+    L.wWords = (kDirTile + b + 1 + p2 + 8 + 3) / 4 + 2;    // window levels + read-ahead of the last doubling step
+    L.offW0 = L.nKeys * 8;
+    L.offW1 = L.offW0 + L.wWords * 4;
+    L.offS = (L.offW1 + L.wWords * 4 + 15u) & ~15u;
+    L.offList = L.offS + kDirTile + 16;
+    L.total = L.offList + kDirTile * 2;
+    return L;
+}
+
+struct DirSmem {
+    u64* K;                   // K[q] <-> particle G0 + q, G0 = T0 - b - 1
+    u32* W0;                  // byte i <-> window start G0 + i
+    u32* W1;
+    unsigned char* S;         // S[p] = digits shared by the neighbours left and right of position T0 + p
+    unsigned short* list;     // positions p (tile-local) that own K entries, ascending
+};
+
+// Phases 1-3 for one tile: keys -> window levels -> sliding maximum.  Returns the byte array
+// dmax with dmax[q'] = d of particle T0 - 1 + q'.  EDGE: the tile touches the ends of P.
+template <bool EDGE>
+__device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm, const DirLayout& L,
+                                                              const u64* __restrict__ P, u32 n, u32 b, long long T0)
+{
+    const u32 tid = threadIdx.x;
+    const long long G0 = T0 - (long long)b - 1;
+    const u64* Pt = P + G0;                                // only dereferenced where G0 + q is inside P
+    auto valid = [&](u32 q) { const long long g = G0 + q; return g >= 0 && g < (long long)n; };
+    // ---- keys of the tile and its halo: all loads of a thread are in flight together -------------
+    {
+        u64 kr[kDirItems];
+#pragma unroll
+        for (int k = 0; k < kDirItems; ++k) {
+            const u32 q = k * kDirBlock + tid;
+            kr[k] = (!EDGE || valid(q)) ? ldStreamU64(Pt + q) : 0ull;
+        }
+        for (u32 q = kDirTile + tid; q < L.nKeys; q += kDirBlock) sm.K[q] = (!EDGE || valid(q)) ? ldStreamU64(Pt + q) : 0ull;
+#pragma unroll
+        for (int k = 0; k < kDirItems; ++k) sm.K[k * kDirBlock + tid] = kr[k];
+    }
+    __syncthreads();
+    // ---- window levels w[i] = min(digits shared by P[g], P[g + b], L - 1), g = G0 + i; 0 where the
+    // window does not fit into P (and in the read-ahead of the doubling steps) ----------------------
+    unsigned char* w0 = reinterpret_cast<unsigned char*>(sm.W0);
+    for (u32 i = tid; i < L.wWords * 4; i += kDirBlock) {
+        u32 w = 0;
+        if (i <= kDirTile + b && (!EDGE || (G0 + i >= 0 && G0 + i + b < (long long)n))) {
+            w = sharedDigitsX(sm.K[i] ^ sm.K[i + b]);
+            w = w < (u32)kL - 1 ? w : (u32)kL - 1;
+        }
+        w0[i] = (unsigned char)w;
+    }
+    // ---- neighbour levels: a leaf starts at position p iff S[p] <= d of particle T0 + p ----------
+#pragma unroll
+    for (int k = 0; k < kDirItems; ++k) {
+        const u32 p = k * kDirBlock + tid;
+        u32 sv = sharedDigitsX(sm.K[p + b] ^ sm.K[p + b + 1]);
+        if (EDGE) {
+            const u64 j = (u64)T0 + p;
+            if (j == 0 || j == n) sv = 0;                  // first particle / tail of the array: always owns entries
+            else if (j > n) sv = 255;                      // beyond the tail: never
+        }
+        sm.S[p] = (unsigned char)sv;
+    }
+    __syncthreads();
+    // ---- sliding maximum over b+1 consecutive windows: doubling, 4 bytes per operation -----------
+    u32* src = sm.W0;
+    u32* dst = sm.W1;
+    const u32 W = b + 1;
+    const u32 words = (kDirTile + 1 + W + 3) / 4;          // covers every byte a later step or the result needs
+    auto shifted = [](const u32* a, u32 q, u32 o) {        // bytes [4q + o, 4q + o + 4) of array a
+        const u32 w = q + (o >> 2);
+        return __funnelshift_r(a[w], a[w + 1], 8 * (o & 3u));
+    };
+    u32 len = 1;
+    while (len * 2 <= W) {                                 // afterwards byte i = max of w over [i, i + 2 len)
+        for (u32 q = tid; q < words; q += kDirBlock)
+            if (q + (len >> 2) + 1 < L.wWords) dst[q] = __vmaxu4(src[q], shifted(src, q, len));
+        __syncthreads();
+        u32* t = src; src = dst; dst = t;
+        len *= 2;
+    }
+    if (len < W) {                                         // two overlapping windows of length len cover b+1
+        for (u32 q = tid; q < (kDirTile + 1 + 3) / 4; q += kDirBlock) dst[q] = __vmaxu4(src[q], shifted(src, q, W - len));
+        __syncthreads();
+        src = dst;
+    }
+    return reinterpret_cast<const unsigned char*>(src);
+}
+
+__global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
+    leavesDirectKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 b, u64* __restrict__ K,
+                       u32* __restrict__ off, u32 cap, u64* lookback, u32 epoch, u32 tiles)
+{
+    extern __shared__ __align__(16) unsigned char dsm[];
+    __shared__ u32 sTile, sPrefix, sMaxLevel;
+    __shared__ u32 warpSums[kDirBlock / 32 + 1];
+    const DirLayout L = dirLayout(b);
+    DirSmem sm;
+    sm.K = reinterpret_cast<u64*>(dsm);
+    sm.W0 = reinterpret_cast<u32*>(dsm + L.offW0);
+    sm.W1 = reinterpret_cast<u32*>(dsm + L.offW1);
+    sm.S = dsm + L.offS;
+    sm.list = reinterpret_cast<unsigned short*>(dsm + L.offList);
+    const u32 tid = threadIdx.x;
+    if (tid == 0) sMaxLevel = 0;
+    u32 published = 0;                                     // thread 0: deepest level already sent to ctrl
+
+    // Tiles are handed out by an atomic ticket, so a tile only ever waits for tiles that already run.
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) sTile = atomicAdd(&ctrl->ticket[0], 1u);
+        __syncthreads();
+        const u32 tile = sTile;
+        if (tile >= tiles) break;
+        const long long T0 = (long long)tile * kDirTile;
+        const long long G0 = T0 - (long long)b - 1;
+        const bool edge = G0 < 0 || G0 + (long long)L.nKeys > (long long)n;
+        const unsigned char* dmax = edge ? dirTileLevels<true>(sm, L, P, n, b, T0) : dirTileLevels<false>(sm, L, P, n, b, T0);
+        const u32* dm = reinterpret_cast<const u32*>(dmax);
+
+        // ---- which positions own K entries: S[p] <= d_{T0+p}, 8 consecutive positions per thread ----
+        const u32* s32 = reinterpret_cast<const u32*>(sm.S);
+        const u32 sA = s32[2 * tid], sB = s32[2 * tid + 1];
+        const u32 d0 = dm[2 * tid], d1 = dm[2 * tid + 1], d2 = dm[2 * tid + 2];
+        const u32 dA = __funnelshift_r(d0, d1, 8), dB = __funnelshift_r(d1, d2, 8);   // d of positions 8 tid .. 8 tid + 7
+        const u32 fA = __vcmpleu4(sA, dA), fB = __vcmpleu4(sB, dB);                   // 0xFF per owning position
+        const u32 mine = (__popc(fA) + __popc(fB)) >> 3;
+        u32 mx = __vmaxu4(dA, dB);
+        mx = __vmaxu4(mx, mx >> 16);
+        mx = __vmaxu4(mx, mx >> 8) & 0xFFu;                 // deepest internal level d on this thread's positions
+        u32 nb;
+        u32 slot = blockExclusiveScan<kDirBlock>(mine, warpSums, &nb);
+        if (mine) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (((k < 4 ? fA : fB) >> (8 * (k & 3))) & 1u) sm.list[slot++] = (unsigned short)(8 * tid + k);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, o));
+        if ((tid & 31u) == 0 && mx + 1 > sMaxLevel) atomicMax(&sMaxLevel, mx + 1);   // leaf level D = d + 1
+        __syncthreads();
+
+        // ---- counts of the listed positions (chunks of one entry per thread), tile total ---------------
+        auto countOf = [&](u32 m) -> u32 {
+            if (m >= nb) return 0u;
+            const u32 p = sm.list[m];
+            return dirCount(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n);
+        };
+        u32 total = 0, cnt0 = 0, excl0 = 0;
+        for (u32 base = 0; base < nb; base += kDirBlock) {
+            const u32 cnt = countOf(base + tid);
+            u32 t;
+            const u32 e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
+            if (base == 0) {
+                cnt0 = cnt;
+                excl0 = e;
+            }
+            total += t;
+            __syncthreads();                                // warpSums is reused by the next chunk
+        }
+        // ---- look-back across tiles -----------------------------------------------------------------
+        if (tid < 32) {
+            u64* st = lookback + tile;
+            u32 pfx = 0;
+            if (tile == 0) {
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
+            } else {
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbAggregate, total));
+                pfx = lbLookBackWarp(lookback, tile, epoch);
+                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, pfx + total));
+            }
+            if (tid == 0) sPrefix = pfx;
+        }
+        __syncthreads();
+        // ---- emission ----------------------------------------------------------------------------------
+        u32 carry = sPrefix;
+        for (u32 base = 0; base < nb; base += kDirBlock) {
+            u32 cnt = cnt0, e = excl0, t = 0;
+            if (nb > kDirBlock) {                           // rare: more than 256 leaf starts in 2048 positions
+                cnt = countOf(base + tid);
+                e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
+                __syncthreads();
+            }
+            if (cnt) {
+                const u32 p = sm.list[base + tid];
+                dirEmit(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n, carry + e, K, off, cap);
+            }
+            carry += t;
+        }
+        if (tid == 0) {
+            if (sMaxLevel > published) {                    // changed[0] doubles as the deepest leaf level
+                published = sMaxLevel;
+                atomicMax(&ctrl->changed[0], published);
+            }
+            if (tile == tiles - 1) ctrl->nl[0] = sPrefix + total - 1;   // K entries minus the terminal 8^21
+            __threadfence();
+            const u32 finished = atomicAdd(&ctrl->tilesDone[0], 1u) + 1u;
+            if (finished == tiles) {                         // last tile to finish closes the build
+                __threadfence();
+                const u32 nl = *(volatile u32*)&ctrl->nl[0];
+                const u32 deepest = *(volatile u32*)&ctrl->changed[0];
+                const u32 rounds = deepest + 1;              // one round per level + the confirming one (A12)
+                ctrl->rounds = rounds;
+                ctrl->nl[rounds] = nl;
+                ctrl->directBuild = 1;
+                if (nl > cap) ctrl->status = CS_ERR_CAPACITY;
+                else {
+                    ctrl->numLeaves = nl;
+                    ctrl->converged = 1;
+                }
+                ctrl->done = 1;
+            }
+        }
+    }
+}
+
+// n <= bucketSize (A15 for n == 0): the root is the only leaf, K = {0, 8^21}, one (confirming) round
+__global__ void leavesDirectRootKernel(DeviceCtrl* ctrl, u64* K, u32* off, u32 n)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        K[0] = 0;
+        K[1] = kKeyEnd;
+        off[0] = 0;
+        off[1] = n;
+        ctrl->nl[0] = 1;
+        ctrl->nl[1] = 1;
+        ctrl->rounds = 1;
+        ctrl->numLeaves = 1;
+        ctrl->converged = 1;
+        ctrl->directBuild = 1;
+        ctrl->done = 1;
+    }
+}
+
+bool leavesDirectSupported(const cs_context* ctx, u32 bucket)
+{
+    return bucket <= (u32)kDirectMaxBucket && dirLayout(bucket).total <= 200u * 1024u && ctx->leafLookback != nullptr;
+}
+
+// enqueue the one-pass build into the workspace arrays leafK[0] / leafOff[0]; ctrl must be zeroed
+cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, u32 cap, cudaStream_t s)
+{
+    DeviceCtrl* ctrl = ctx->ctrl;
+    if (n <= bucket) {                                     // no window of bucket+1 keys: the root is not split
+        leavesDirectRootKernel<<<1, 32, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafOff[0], (u32)n);
+        CS_LAUNCH_CHECK(ctx, "leavesDirectRootKernel");
+        return CS_OK;
+    }
+    const DirLayout L = dirLayout(bucket);
+    static u32 attrBytes = 0;
+    if (L.total > 48u * 1024u && L.total > attrBytes) {
+        CS_CUDA(ctx, cudaFuncSetAttribute(leavesDirectKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        attrBytes = L.total;
+    }
+    const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
+    const u32 epoch = nextEpoch(ctx, s);
+    int perSM = 1;
+    CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, leavesDirectKernel, kDirBlock, L.total));
+    if (perSM < 1) perSM = 1;
+    u32 grid = (u32)ctx->numSMs * (u32)perSM;
+    if (grid > tiles) grid = tiles;
+    leavesDirectKernel<<<grid, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->leafK[0], ctx->leafOff[0], cap,
+                                                        ctx->leafLookback, epoch, tiles);
+    CS_LAUNCH_CHECK(ctx, "leavesDirectKernel");
+    return CS_OK;
+}
+
+}  // namespace cs

@@ -80,7 +80,16 @@ struct SortSmem {
     u32 tile;
 };
 
-constexpr int kLookBatch = 4;            // predecessors fetched per look-back round trip
+#ifndef CS_SORT_LOOKBATCH
+#define CS_SORT_LOOKBATCH 4
+#endif
+#ifndef CS_SORT_LATELB
+#define CS_SORT_LATELB 0
+#endif
+#ifndef CS_SORT_PREFETCH
+#define CS_SORT_PREFETCH 0
+#endif
+constexpr int kLookBatch = CS_SORT_LOOKBATCH;   // predecessors fetched per look-back round trip
 
 // Exclusive prefix of counter c over tiles < tile.  The words of kLookBatch predecessors are
 // requested together, so one memory round trip covers kLookBatch tiles.
@@ -140,6 +149,10 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     // ---- load: warp-striped, so that (warp, item, lane) order == memory order (stability) ----
     u64 key[kSortItems];
     const u32 warpOff = warp * (32 * kSortItems) + lane;
+#if CS_SORT_PREFETCH
+    if (!FIRST && tid < kSortTile * 4 / 128)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(valsIn + base + tid * 32));
+#endif
     const u64* src = keysIn + base + warpOff;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j)
@@ -184,6 +197,7 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
     if (tid < kRadix) {
         sm.digitStart[tid] = start;
+#if !CS_SORT_LATELB
         // ---- decoupled look-back over preceding tiles, one thread per digit ----------------------
         u32 excl = 0;
         if (tile != 0) {
@@ -192,6 +206,7 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
             lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, kLbPrefix, excl + real));
         }
         sm.globalBase[tid] = digitBase[tid] + excl - start;
+#endif
     }
     __syncthreads();
 
@@ -216,6 +231,19 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     }
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) sm.vals[(rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu] = val[j];
+#if CS_SORT_LATELB
+    // ---- decoupled look-back, after the shared-memory scatter: the predecessors have had that much
+    // longer to publish their prefixes, and the other warps are not kept waiting at a barrier ---------
+    if (tid < kRadix) {
+        u32 excl = 0;
+        if (tile != 0) {
+            const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;
+            excl = lookBackBatched(lookback, tid, tile, epoch);
+            lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, kLbPrefix, excl + real));
+        }
+        sm.globalBase[tid] = digitBase[tid] + excl - start;
+    }
+#endif
     __syncthreads();
 
     // ---- write out: consecutive threads -> consecutive slots of a digit's run ----------------------
