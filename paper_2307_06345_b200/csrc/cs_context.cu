@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, divLevel, tileLookback, leafLookback, linkTileHist, ctrl, total;
+        leafOffFinal, leafTasks, divLevel, tileLookback, dirFlags, dirTotals, dirBases, linkTileHist, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -41,7 +41,9 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = alignUp(o + bytes); return at; };
     const size_t sortTiles = (maxParticles + kSortTile - 1) / kSortTile + 1;
-    const size_t leafTiles = ((size_t)maxLeaves + 1 + 1023) / 1024 + 1;   // covers kLeafTile, kScanTile >= 1024
+    const size_t dirTiles = (maxParticles >> kDirectTileLog2) + 2;          // one-pass leaf build: positions 0 .. n
+    size_t leafTiles = ((size_t)maxLeaves + 1 + 1023) / 1024 + 1;          // covers kLeafTile, kScanTile >= 1024
+    if (leafTiles < dirTiles / 1024 + 2) leafTiles = dirTiles / 1024 + 2;  // the scan of the one-pass build's tile totals
     const size_t linkTiles = ((size_t)maxLeaves + kLinkTile - 1) / kLinkTile + 1;
     static_assert(kLeafTile >= 1024 && kScanTile >= 1024, "look-back array is sized for tiles of >= 1024");
     L.keysAlt = take(maxParticles * sizeof(u64));
@@ -56,9 +58,11 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafOff1 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOffFinal = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint2));   // linear list, search list
-    L.divLevel = take(maxParticles + 256);                                 // 1 byte per particle
+    L.divLevel = take(dirTiles << kDirectTileLog2);                        // 1 byte per particle, whole tiles
     L.tileLookback = take(leafTiles * sizeof(u64));                        // one counter per tile (leaf rounds, scan)
-    L.leafLookback = take(((maxParticles >> kDirectTileLog2) + 2) * sizeof(u64));   // one-pass leaf build
+    L.dirFlags = take(dirTiles << (kDirectTileLog2 - 3));                  // one-pass leaf build: 1 bit per position
+    L.dirTotals = take((dirTiles + 2) * sizeof(u32));                      // K entries per tile
+    L.dirBases = take((dirTiles + 2) * sizeof(u32));                       // exclusive prefix of dirTotals
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
@@ -212,7 +216,9 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->divLevel = (unsigned char*)(ctx->slab + L.divLevel);
     ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
-    ctx->leafLookback = (u64*)(ctx->slab + L.leafLookback);
+    ctx->dirFlags = (unsigned char*)(ctx->slab + L.dirFlags);
+    ctx->dirTotals = (u32*)(ctx->slab + L.dirTotals);
+    ctx->dirBases = (u32*)(ctx->slab + L.dirBases);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
     *out = ctx;

@@ -109,12 +109,15 @@ struct cs_context {
     // leaves
     cs::u64* leafK[2] = {nullptr, nullptr};
     cs::u32* leafOff[2] = {nullptr, nullptr};
-    unsigned char* divLevel = nullptr; // D[i] = number of leading octal digits shared by P[i-1] and P[i] (D[0] = 0)
+    unsigned char* divLevel = nullptr; // iterative path: D[i] = (digits shared by P[i-1], P[i]) << 3 | next digit;
+                                       // one-pass build: d_j = level of the deepest internal node above particle j
     uint2* leafTasks = nullptr;        // (first child slot, end of the parent's particle range) per split leaf
     cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
     cs::u64* tileLookback = nullptr;   // [tiles] look-back words of the leaf rounds and the scan
-    cs::u64* leafLookback = nullptr;   // [maxParticles / 2^kDirectTileLog2 + 2] look-back words of the one-pass leaf build
+    unsigned char* dirFlags = nullptr; // one-pass leaf build: bit j set <=> position j owns entries of K
+    cs::u32* dirTotals = nullptr;      // [tiles] K entries owned by the positions of a tile
+    cs::u32* dirBases = nullptr;       // [tiles + 1] exclusive prefix of dirTotals
     int leafMode = 0;                  // cs_setLeafMode
     cs::u32* linkTileHist = nullptr;   // [tiles][kLinkBins] node counts per tile, level and kind
     cs::DeviceCtrl* ctrl = nullptr;

@@ -103,18 +103,19 @@ __device__ __noinline__ void dirEmit(u64 a, u64 c, int Da, int Dc, u32 j, u32 n,
     put(Dc == 0 ? 0ull : c & ~((1ull << (3 * (kL - Dc))) - 1));   // the leaf of c
 }
 
-// dynamic shared memory: keys of [T0 - b - 1, T0 + T + b), window levels (two byte arrays for the
-// doubling steps of the sliding maximum), neighbour levels s[p], list of leaf-start positions
+// ---- kernel 1: levels ---------------------------------------------------------------------------
+// dynamic shared memory: keys of [T0 - b - 1, T0 + T + b), window levels (two word arrays for the
+// steps of the sliding maximum), neighbour levels s[p], list of leaf-start positions
 struct DirLayout {
-    u32 nKeys, wWords, offW0, offW1, offS, offList, total;
+    u32 nKeys, words, wWords, offW0, offW1, offS, offList, total;
 };
 __host__ __device__ inline DirLayout dirLayout(u32 b)
 {
     DirLayout L;
+    const u32 W = b + 1;
     L.nKeys = kDirTile + 2 * b + 1;
-    u32 p2 = 1;
-    while (p2 * 2 <= b + 1) p2 *= 2;                       // largest power of two <= window length b+1
-    L.wWords = (kDirTile + b + 1 + p2 + 8 + 3) / 4 + 2;    // window levels + read-ahead of the last doubling step
+    L.words = (kDirTile + 1 + W + 3) / 4 + 1;              // covers every byte a later step or the result needs
+    L.wWords = L.words + W / 4 + 4;                        // + read-ahead of a step (at most 3/4 W bytes) + slack
     L.offW0 = L.nKeys * 8;
     L.offW1 = L.offW0 + L.wWords * 4;
     L.offS = (L.offW1 + L.wWords * 4 + 15u) & ~15u;
@@ -131,8 +132,15 @@ struct DirSmem {
     unsigned short* list;     // positions p (tile-local) that own K entries, ascending
 };
 
-// Phases 1-3 for one tile: keys -> window levels -> sliding maximum.  Returns the byte array
-// dmax with dmax[q'] = d of particle T0 - 1 + q'.  EDGE: the tile touches the ends of P.
+// bytes [4q + o, 4q + o + 4) of the word array a
+__device__ __forceinline__ u32 dirShifted(const u32* a, u32 q, u32 o)
+{
+    const u32 w = q + (o >> 2);
+    return __funnelshift_r(a[w], a[w + 1], 8 * (o & 3u));
+}
+
+// Keys -> window levels -> sliding maximum for one tile.  Returns the byte array dmax with
+// dmax[q'] = d of particle T0 - 1 + q'.  EDGE: the tile touches the ends of P.
 template <bool EDGE>
 __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm, const DirLayout& L,
                                                               const u64* __restrict__ P, u32 n, u32 b, long long T0)
@@ -152,63 +160,76 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
         for (u32 q = kDirTile + tid; q < L.nKeys; q += kDirBlock) sm.K[q] = (!EDGE || valid(q)) ? ldStreamU64(Pt + q) : 0ull;
 #pragma unroll
         for (int k = 0; k < kDirItems; ++k) sm.K[k * kDirBlock + tid] = kr[k];
+        // the parts of the level arrays that no thread computes read as level 0
+        for (u32 q = (kDirTile + b + 1) / 4 + tid; q < L.wWords; q += kDirBlock) sm.W0[q] = 0;
+        for (u32 q = L.words + tid; q < L.wWords; q += kDirBlock) sm.W1[q] = 0;
     }
     __syncthreads();
-    // ---- window levels w[i] = min(digits shared by P[g], P[g + b], L - 1), g = G0 + i; 0 where the
-    // window does not fit into P (and in the read-ahead of the doubling steps) ----------------------
+    // ---- window levels w[i] = min(digits shared by P[g], P[g + b], L - 1), g = G0 + i (0 where the
+    // window does not fit into P), and neighbour levels: a leaf starts at position p iff
+    // S[p] <= d of particle T0 + p.  One pass, the key K[i + b] serves both ------------------------
     unsigned char* w0 = reinterpret_cast<unsigned char*>(sm.W0);
-    for (u32 i = tid; i < L.wWords * 4; i += kDirBlock) {
-        u32 w = 0;
-        if (i <= kDirTile + b && (!EDGE || (G0 + i >= 0 && G0 + i + b < (long long)n))) {
-            w = sharedDigitsX(sm.K[i] ^ sm.K[i + b]);
-            w = w < (u32)kL - 1 ? w : (u32)kL - 1;
-        }
-        w0[i] = (unsigned char)w;
-    }
-    // ---- neighbour levels: a leaf starts at position p iff S[p] <= d of particle T0 + p ----------
 #pragma unroll
     for (int k = 0; k < kDirItems; ++k) {
-        const u32 p = k * kDirBlock + tid;
-        u32 sv = sharedDigitsX(sm.K[p + b] ^ sm.K[p + b + 1]);
+        const u32 i = k * kDirBlock + tid;
+        const u64 kb = sm.K[i + b];
+        u32 w = sharedDigitsX(sm.K[i] ^ kb);
+        w = w < (u32)kL - 1 ? w : (u32)kL - 1;
+        u32 sv = sharedDigitsX(kb ^ sm.K[i + b + 1]);
         if (EDGE) {
-            const u64 j = (u64)T0 + p;
+            if (!(G0 + i >= 0 && G0 + i + b < (long long)n)) w = 0;
+            const u64 j = (u64)T0 + i;
             if (j == 0 || j == n) sv = 0;                  // first particle / tail of the array: always owns entries
             else if (j > n) sv = 255;                      // beyond the tail: never
         }
-        sm.S[p] = (unsigned char)sv;
+        w0[i] = (unsigned char)w;
+        sm.S[i] = (unsigned char)sv;
+    }
+    for (u32 i = kDirTile + tid; i <= kDirTile + b; i += kDirBlock) {
+        u32 w = sharedDigitsX(sm.K[i] ^ sm.K[i + b]);
+        w = w < (u32)kL - 1 ? w : (u32)kL - 1;
+        if (EDGE && !(G0 + i >= 0 && G0 + i + b < (long long)n)) w = 0;
+        w0[i] = (unsigned char)w;
     }
     __syncthreads();
-    // ---- sliding maximum over b+1 consecutive windows: doubling, 4 bytes per operation -----------
+    // ---- sliding maximum over b+1 consecutive windows, 4 bytes per operation: the window length
+    // covered by a byte grows 4-fold per step (then 2-fold, then the two overlapping windows) --------
     u32* src = sm.W0;
     u32* dst = sm.W1;
     const u32 W = b + 1;
-    const u32 words = (kDirTile + 1 + W + 3) / 4;          // covers every byte a later step or the result needs
-    auto shifted = [](const u32* a, u32 q, u32 o) {        // bytes [4q + o, 4q + o + 4) of array a
-        const u32 w = q + (o >> 2);
-        return __funnelshift_r(a[w], a[w + 1], 8 * (o & 3u));
-    };
-    u32 len = 1;
-    while (len * 2 <= W) {                                 // afterwards byte i = max of w over [i, i + 2 len)
-        for (u32 q = tid; q < words; q += kDirBlock)
-            if (q + (len >> 2) + 1 < L.wWords) dst[q] = __vmaxu4(src[q], shifted(src, q, len));
+    u32 len = 1;                                           // byte i = max of w over [i, i + len)
+    while (len * 4 <= W) {
+        for (u32 q = tid; q < L.words; q += kDirBlock) {
+            const u32 a = __vmaxu4(src[q], dirShifted(src, q, len));
+            const u32 c = __vmaxu4(dirShifted(src, q, 2 * len), dirShifted(src, q, 3 * len));
+            dst[q] = __vmaxu4(a, c);
+        }
+        __syncthreads();
+        u32* t = src; src = dst; dst = t;
+        len *= 4;
+    }
+    if (len * 2 <= W) {
+        for (u32 q = tid; q < L.words; q += kDirBlock) dst[q] = __vmaxu4(src[q], dirShifted(src, q, len));
         __syncthreads();
         u32* t = src; src = dst; dst = t;
         len *= 2;
     }
     if (len < W) {                                         // two overlapping windows of length len cover b+1
-        for (u32 q = tid; q < (kDirTile + 1 + 3) / 4; q += kDirBlock) dst[q] = __vmaxu4(src[q], shifted(src, q, W - len));
+        for (u32 q = tid; q < (kDirTile + 1 + 3) / 4 + 1; q += kDirBlock) dst[q] = __vmaxu4(src[q], dirShifted(src, q, W - len));
         __syncthreads();
         src = dst;
     }
     return reinterpret_cast<const unsigned char*>(src);
 }
 
+// One tile of kDirTile positions per CTA: d of every particle (dArr), which positions own K entries
+// (flags, one bit per position) and how many entries the tile owns (totals).  No CTA waits for another.
 __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
-    leavesDirectKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 b, u64* __restrict__ K,
-                       u32* __restrict__ off, u32 cap, u64* lookback, u32 epoch, u32 tiles)
+    leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 b, unsigned char* __restrict__ dArr,
+                       unsigned char* __restrict__ flags, u32* __restrict__ totals)
 {
     extern __shared__ __align__(16) unsigned char dsm[];
-    __shared__ u32 sTile, sPrefix, sMaxLevel;
+    __shared__ u32 sTotal, sMaxLevel;
     __shared__ u32 warpSums[kDirBlock / 32 + 1];
     const DirLayout L = dirLayout(b);
     DirSmem sm;
@@ -218,115 +239,110 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
     sm.S = dsm + L.offS;
     sm.list = reinterpret_cast<unsigned short*>(dsm + L.offList);
     const u32 tid = threadIdx.x;
-    if (tid == 0) sMaxLevel = 0;
-    u32 published = 0;                                     // thread 0: deepest level already sent to ctrl
+    const u32 tile = blockIdx.x;
+    if (tid == 0) {
+        sTotal = 0;
+        sMaxLevel = 0;
+    }
+    const long long T0 = (long long)tile * kDirTile;
+    const long long G0 = T0 - (long long)b - 1;
+    const bool edge = G0 < 0 || G0 + (long long)L.nKeys > (long long)n;
+    const unsigned char* dmax = edge ? dirTileLevels<true>(sm, L, P, n, b, T0) : dirTileLevels<false>(sm, L, P, n, b, T0);
+    const u32* dm = reinterpret_cast<const u32*>(dmax);
 
-    // Tiles are handed out by an atomic ticket, so a tile only ever waits for tiles that already run.
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) sTile = atomicAdd(&ctrl->ticket[0], 1u);
-        __syncthreads();
-        const u32 tile = sTile;
-        if (tile >= tiles) break;
-        const long long T0 = (long long)tile * kDirTile;
-        const long long G0 = T0 - (long long)b - 1;
-        const bool edge = G0 < 0 || G0 + (long long)L.nKeys > (long long)n;
-        const unsigned char* dmax = edge ? dirTileLevels<true>(sm, L, P, n, b, T0) : dirTileLevels<false>(sm, L, P, n, b, T0);
-        const u32* dm = reinterpret_cast<const u32*>(dmax);
-
-        // ---- which positions own K entries: S[p] <= d_{T0+p}, 8 consecutive positions per thread ----
-        const u32* s32 = reinterpret_cast<const u32*>(sm.S);
-        const u32 sA = s32[2 * tid], sB = s32[2 * tid + 1];
-        const u32 d0 = dm[2 * tid], d1 = dm[2 * tid + 1], d2 = dm[2 * tid + 2];
-        const u32 dA = __funnelshift_r(d0, d1, 8), dB = __funnelshift_r(d1, d2, 8);   // d of positions 8 tid .. 8 tid + 7
-        const u32 fA = __vcmpleu4(sA, dA), fB = __vcmpleu4(sB, dB);                   // 0xFF per owning position
-        const u32 mine = (__popc(fA) + __popc(fB)) >> 3;
-        u32 mx = __vmaxu4(dA, dB);
-        mx = __vmaxu4(mx, mx >> 16);
-        mx = __vmaxu4(mx, mx >> 8) & 0xFFu;                 // deepest internal level d on this thread's positions
-        u32 nb;
-        u32 slot = blockExclusiveScan<kDirBlock>(mine, warpSums, &nb);
-        if (mine) {
+    // ---- which positions own K entries: S[p] <= d_{T0+p}, 8 consecutive positions per thread ----
+    const u32* s32 = reinterpret_cast<const u32*>(sm.S);
+    const u32 sA = s32[2 * tid], sB = s32[2 * tid + 1];
+    const u32 d0 = dm[2 * tid], d1 = dm[2 * tid + 1], d2 = dm[2 * tid + 2];
+    const u32 dA = __funnelshift_r(d0, d1, 8), dB = __funnelshift_r(d1, d2, 8);   // d of particles T0 + 8 tid .. + 7
+    const u32 fA = __vcmpleu4(sA, dA), fB = __vcmpleu4(sB, dB);                   // 0xFF per owning position
+    // one bit per position: bit k of the byte <-> position 8 tid + k
+    const u32 bitsA = ((fA & 0x01010101u) * 0x10204080u) >> 28, bitsB = ((fB & 0x01010101u) * 0x10204080u) >> 28;
+    const u32 fbyte = bitsA | (bitsB << 4);
+    flags[(size_t)tile * kDirBlock + tid] = (unsigned char)fbyte;
+    *reinterpret_cast<uint2*>(dArr + (size_t)T0 + 8 * tid) = make_uint2(dA, dB);
+    const u32 mine = __popc(fbyte);
+    u32 mx = __vmaxu4(dA, dB);
+    mx = __vmaxu4(mx, mx >> 16);
+    mx = __vmaxu4(mx, mx >> 8) & 0xFFu;                     // deepest internal level d on this thread's particles (0 past the tail)
+    u32 nb;
+    u32 slot = blockExclusiveScan<kDirBlock>(mine, warpSums, &nb);
+    for (u32 f = fbyte; f; f &= f - 1) sm.list[slot++] = (unsigned short)(8 * tid + __ffs((int)f) - 1);
 #pragma unroll
-            for (int k = 0; k < 8; ++k)
-                if (((k < 4 ? fA : fB) >> (8 * (k & 3))) & 1u) sm.list[slot++] = (unsigned short)(8 * tid + k);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, o));
-        if ((tid & 31u) == 0 && mx + 1 > sMaxLevel) atomicMax(&sMaxLevel, mx + 1);   // leaf level D = d + 1
-        __syncthreads();
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, o));
+    if ((tid & 31u) == 0 && mx + 1 > sMaxLevel) atomicMax(&sMaxLevel, mx + 1);   // leaf level D = d + 1
+    __syncthreads();
 
-        // ---- counts of the listed positions (chunks of one entry per thread), tile total ---------------
-        auto countOf = [&](u32 m) -> u32 {
-            if (m >= nb) return 0u;
-            const u32 p = sm.list[m];
-            return dirCount(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n);
-        };
-        u32 total = 0, cnt0 = 0, excl0 = 0;
-        for (u32 base = 0; base < nb; base += kDirBlock) {
-            const u32 cnt = countOf(base + tid);
-            u32 t;
-            const u32 e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
-            if (base == 0) {
-                cnt0 = cnt;
-                excl0 = e;
+    // ---- K entries owned by the tile --------------------------------------------------------------
+    u32 cnt = 0;
+    for (u32 m = tid; m < nb; m += kDirBlock) {
+        const u32 p = sm.list[m];
+        cnt += dirCount(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n);
+    }
+    cnt = warpReduceSum(cnt);
+    if ((tid & 31u) == 0 && cnt) atomicAdd(&sTotal, cnt);
+    __syncthreads();
+    if (tid == 0) {
+        totals[tile] = sTotal;
+        atomicMax(&ctrl->changed[0], sMaxLevel);           // changed[0] doubles as the deepest leaf level
+    }
+}
+
+// ---- kernel 2: emission ---------------------------------------------------------------------------
+// The same tiles; bases = exclusive prefix of totals over tiles (bases[tiles] = all K entries).  The
+// listed positions fetch their two keys and levels from global memory; everything else is a bit scan.
+__global__ void __launch_bounds__(kDirBlock)
+    leavesEmitDirectKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const unsigned char* __restrict__ dArr,
+                           const unsigned char* __restrict__ flags, const u32* __restrict__ bases, u32 tiles,
+                           u64* __restrict__ K, u32* __restrict__ off, u32 cap)
+{
+    __shared__ unsigned short list[kDirTile];
+    __shared__ u32 warpSums[kDirBlock / 32 + 1];
+    const u32 tid = threadIdx.x;
+    const u32 tile = blockIdx.x;
+    const u64 T0 = (u64)tile * kDirTile;
+    const u32 fbyte = flags[(size_t)tile * kDirBlock + tid];
+    u32 nb;
+    u32 slot = blockExclusiveScan<kDirBlock>(__popc(fbyte), warpSums, &nb);
+    for (u32 f = fbyte; f; f &= f - 1) list[slot++] = (unsigned short)(8 * tid + __ffs((int)f) - 1);
+    __syncthreads();
+    u32 carry = bases[tile];
+    for (u32 base = 0; base < nb; base += kDirBlock) {
+        const u32 m = base + tid;
+        u64 a = 0, c = 0;
+        int Da = 0, Dc = 0;
+        u32 j = 0, cnt = 0;
+        if (m < nb) {
+            j = (u32)(T0 + list[m]);
+            if (j > 0) {
+                a = __ldg(P + j - 1);
+                Da = dArr[j - 1] + 1;
             }
-            total += t;
-            __syncthreads();                                // warpSums is reused by the next chunk
+            if (j < n) {
+                c = __ldg(P + j);
+                Dc = dArr[j] + 1;
+            }
+            cnt = dirCount(a, c, Da, Dc, j, n);
         }
-        // ---- look-back across tiles -----------------------------------------------------------------
-        if (tid < 32) {
-            u64* st = lookback + tile;
-            u32 pfx = 0;
-            if (tile == 0) {
-                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, total));
-            } else {
-                if (tid == 0) lbStore(st, lbPack(epoch, kLbAggregate, total));
-                pfx = lbLookBackWarp(lookback, tile, epoch);
-                if (tid == 0) lbStore(st, lbPack(epoch, kLbPrefix, pfx + total));
-            }
-            if (tid == 0) sPrefix = pfx;
+        u32 t;
+        const u32 e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
+        if (cnt) dirEmit(a, c, Da, Dc, j, n, carry + e, K, off, cap);
+        carry += t;
+        __syncthreads();                                    // warpSums is reused by the next chunk
+    }
+    if (tile == 0 && tid == 0) {                            // close the build
+        const u32 nl = bases[tiles] - 1;                    // K entries minus the terminal 8^21
+        const u32 rounds = ctrl->changed[0] + 1;            // one round per level + the confirming one (A12)
+        ctrl->nl[0] = nl;
+        ctrl->rounds = rounds;
+        ctrl->nl[rounds] = nl;
+        ctrl->directBuild = 1;
+        if (nl > cap) ctrl->status = CS_ERR_CAPACITY;
+        else {
+            ctrl->numLeaves = nl;
+            ctrl->converged = 1;
         }
-        __syncthreads();
-        // ---- emission ----------------------------------------------------------------------------------
-        u32 carry = sPrefix;
-        for (u32 base = 0; base < nb; base += kDirBlock) {
-            u32 cnt = cnt0, e = excl0, t = 0;
-            if (nb > kDirBlock) {                           // rare: more than 256 leaf starts in 2048 positions
-                cnt = countOf(base + tid);
-                e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
-                __syncthreads();
-            }
-            if (cnt) {
-                const u32 p = sm.list[base + tid];
-                dirEmit(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n, carry + e, K, off, cap);
-            }
-            carry += t;
-        }
-        if (tid == 0) {
-            if (sMaxLevel > published) {                    // changed[0] doubles as the deepest leaf level
-                published = sMaxLevel;
-                atomicMax(&ctrl->changed[0], published);
-            }
-            if (tile == tiles - 1) ctrl->nl[0] = sPrefix + total - 1;   // K entries minus the terminal 8^21
-            __threadfence();
-            const u32 finished = atomicAdd(&ctrl->tilesDone[0], 1u) + 1u;
-            if (finished == tiles) {                         // last tile to finish closes the build
-                __threadfence();
-                const u32 nl = *(volatile u32*)&ctrl->nl[0];
-                const u32 deepest = *(volatile u32*)&ctrl->changed[0];
-                const u32 rounds = deepest + 1;              // one round per level + the confirming one (A12)
-                ctrl->rounds = rounds;
-                ctrl->nl[rounds] = nl;
-                ctrl->directBuild = 1;
-                if (nl > cap) ctrl->status = CS_ERR_CAPACITY;
-                else {
-                    ctrl->numLeaves = nl;
-                    ctrl->converged = 1;
-                }
-                ctrl->done = 1;
-            }
-        }
+        ctrl->done = 1;
     }
 }
 
@@ -350,7 +366,7 @@ __global__ void leavesDirectRootKernel(DeviceCtrl* ctrl, u64* K, u32* off, u32 n
 
 bool leavesDirectSupported(const cs_context* ctx, u32 bucket)
 {
-    return bucket <= (u32)kDirectMaxBucket && dirLayout(bucket).total <= 200u * 1024u && ctx->leafLookback != nullptr;
+    return bucket <= (u32)kDirectMaxBucket && dirLayout(bucket).total <= 200u * 1024u && ctx->dirFlags != nullptr;
 }
 
 // enqueue the one-pass build into the workspace arrays leafK[0] / leafOff[0]; ctrl must be zeroed
@@ -365,19 +381,17 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
     const DirLayout L = dirLayout(bucket);
     static u32 attrBytes = 0;
     if (L.total > 48u * 1024u && L.total > attrBytes) {
-        CS_CUDA(ctx, cudaFuncSetAttribute(leavesDirectKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        CS_CUDA(ctx, cudaFuncSetAttribute(leavesLevelsKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
         attrBytes = L.total;
     }
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
-    const u32 epoch = nextEpoch(ctx, s);
-    int perSM = 1;
-    CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, leavesDirectKernel, kDirBlock, L.total));
-    if (perSM < 1) perSM = 1;
-    u32 grid = (u32)ctx->numSMs * (u32)perSM;
-    if (grid > tiles) grid = tiles;
-    leavesDirectKernel<<<grid, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->leafK[0], ctx->leafOff[0], cap,
-                                                        ctx->leafLookback, epoch, tiles);
-    CS_LAUNCH_CHECK(ctx, "leavesDirectKernel");
+    leavesLevelsKernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags,
+                                                         ctx->dirTotals);
+    CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
+    CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));
+    leavesEmitDirectKernel<<<tiles, kDirBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
+                                                       ctx->leafK[0], ctx->leafOff[0], cap);
+    CS_LAUNCH_CHECK(ctx, "leavesEmitDirectKernel");
     return CS_OK;
 }
 
