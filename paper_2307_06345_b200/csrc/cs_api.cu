@@ -190,8 +190,9 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
 
     CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
-    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, (u64*)b->keys, /*withHist=*/true, s));
-    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*histReady=*/true, s));
+    // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), /*withHist=*/true, s));
+    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
                          (u64*)b->leaves, b->counts, leafCap, s));
     // link and node counts in one pass: the leaves' particle offsets are still in the workspace

@@ -20,9 +20,12 @@ constexpr int kMaxRounds = kL + 1;           // DESIGN.md A12
 constexpr int kRoundSlots = kMaxRounds + 2;
 
 // ---- radix sort geometry -------------------------------------------------------------
-constexpr int kRadixBits = 8;
+#ifndef CS_RADIX_BITS
+#define CS_RADIX_BITS 9
+#endif
+constexpr int kRadixBits = CS_RADIX_BITS;
 constexpr int kRadix = 1 << kRadixBits;
-constexpr int kSortPasses = 8;               // 63 key bits, 8 bits per pass
+constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits: 7 passes of 9 bits
 #ifndef CS_SORT_BLOCK
 #define CS_SORT_BLOCK 512
 #endif
@@ -181,7 +184,8 @@ cs_status enqueueBox(cs_context*, const double* x, const double* y, const double
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
                       u64* keys, bool withHist, cudaStream_t);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
-cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool histReady, cudaStream_t);
+u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
+cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t);
 cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
                         u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity,
                         cudaStream_t);

@@ -1,25 +1,31 @@
 // H3: stable LSD radix sort of (u64 key, u32 index) pairs -- PAPER.md:70, 168; A5.
 //
 // "Onesweep" organisation: one histogram pass over the keys gives the global digit counts of
-// all 8 passes; every pass then reads each element once and writes it once.  A pass tile is
-// ranked inside the CTA (warp-level match + per-warp digit counters), the tile's position in
-// each digit's output run comes from a decoupled look-back over the preceding tiles' digit
-// counts, and the tile is written out through shared memory so that each digit's run is a
+// all passes; every pass then reads each element once and writes it once.  63 key bits in 7
+// passes of 9 bits.  A pass tile is ranked inside the CTA (warp-level ballot matching + per-warp
+// digit counters), the tile's position in each digit's output run comes from a decoupled
+// look-back over the preceding tiles' digit counts (one thread per digit, all 512 threads of the
+// CTA), and the tile is written out through shared memory so that each digit's run is a
 // contiguous burst.  Tiles take their index from an atomic ticket, so a tile only ever waits
 // for tiles that are already running (forward progress).
 //
-// Model bytes per particle: histogram 8 + pass 0 (8 read, 12 written) + 7 x 24 = 196.
+// Model bytes per particle (SURVEY 8d, 8 passes): 196; moved by this 7-pass sort:
+// histogram 0 (fused into the key kernel, else 8) + pass 0 (8 read, 12 written) + 6 x 24 = 164.
 #include "cs_device.cuh"
 
 namespace cs {
 
 constexpr int kHistBlock = 512;
 constexpr int kSortWarps = kSortBlock / 32;
+static_assert(kSortBlock >= kRadix, "one thread per digit in the per-digit phases of a radix pass");
+static_assert(kSortItems * 32 < 65536 && kSortTile < 65536, "16-bit per-warp digit counters and tile-local slots");
 
 __device__ __forceinline__ u32 digitOf(u64 key, int shift) { return (u32)(key >> shift) & (kRadix - 1); }
 
 // ---- global digit histograms of all passes ----------------------------------------------------
-__global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restrict__ keys, u64 n, u32* gHist)
+// copyTo (nullable): the keys are also copied there (the buffer the first pass reads, see sortSource)
+__global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restrict__ keys, u64 n, u32* gHist,
+                                                             u64* __restrict__ copyTo)
 {
     __shared__ u32 sh[kSortPasses * kRadix];
     for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kHistBlock) sh[i] = 0;
@@ -40,14 +46,28 @@ __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restri
             ulonglong2 c = ldStreamU2(keys + 2 * (i + 2 * nthreads));
             ulonglong2 d = ldStreamU2(keys + 2 * (i + 3 * nthreads));
             add(a.x); add(a.y); add(b.x); add(b.y); add(c.x); add(c.y); add(d.x); add(d.y);
+            if (copyTo) {
+                stStreamU2(copyTo + 2 * i, a.x, a.y);
+                stStreamU2(copyTo + 2 * (i + nthreads), b.x, b.y);
+                stStreamU2(copyTo + 2 * (i + 2 * nthreads), c.x, c.y);
+                stStreamU2(copyTo + 2 * (i + 3 * nthreads), d.x, d.y);
+            }
         }
         for (; i < pairs; i += nthreads) {
             ulonglong2 a = ldStreamU2(keys + 2 * i);
             add(a.x); add(a.y);
+            if (copyTo) stStreamU2(copyTo + 2 * i, a.x, a.y);
         }
-        if ((n & 1) && tid == 0) add(keys[n - 1]);
+        if ((n & 1) && tid == 0) {
+            add(keys[n - 1]);
+            if (copyTo) copyTo[n - 1] = keys[n - 1];
+        }
     } else {
-        for (u64 i = tid; i < n; i += nthreads) add(ldStreamU64(keys + i));
+        for (u64 i = tid; i < n; i += nthreads) {
+            const u64 k = ldStreamU64(keys + i);
+            add(k);
+            if (copyTo) copyTo[i] = k;
+        }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kHistBlock) {
@@ -56,7 +76,7 @@ __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restri
     }
 }
 
-// exclusive scan of each pass's 256 digit counts, in place (one CTA)
+// exclusive scan of each pass's digit counts, in place (one CTA)
 __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 {
     __shared__ u32 warpSums[kRadix / 32 + 1];
@@ -71,77 +91,72 @@ __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 
 // ---- one radix pass ------------------------------------------------------------------------------
 struct SortSmem {
-    u64 keys[kSortTile];                 // tile in digit order
+    u64 keys[kSortTile];                           // tile in digit order
     u32 vals[kSortTile];
-    u32 warpHist[kSortWarps][kRadix];    // per-warp digit counts, then exclusive prefix over warps
-    u32 digitStart[kRadix];              // first tile-local slot of each digit
-    u32 globalBase[kRadix];              // global slot of (digit d, tile-local slot i) = globalBase[d] + i
+    unsigned short warpHist[kSortWarps][kRadix];   // per-warp digit counts, then first tile-local slot of (warp, digit)
+    u32 globalBase[kRadix];                        // global slot of (digit d, tile-local slot i) = globalBase[d] + i
     u32 warpSums[kSortWarps + 1];
     u32 tile;
 };
 
 #ifndef CS_SORT_LOOKBATCH
-#define CS_SORT_LOOKBATCH 4
-#endif
-#ifndef CS_SORT_LATELB
-#define CS_SORT_LATELB 0
-#endif
-#ifndef CS_SORT_PREFETCH
-#define CS_SORT_PREFETCH 0
+#define CS_SORT_LOOKBATCH 8
 #endif
 constexpr int kLookBatch = CS_SORT_LOOKBATCH;   // predecessors fetched per look-back round trip
 
-// Exclusive prefix of counter c over tiles < tile.  The words of kLookBatch predecessors are
-// requested together, so one memory round trip covers kLookBatch tiles.
+// Exclusive prefix of counter c over tiles < tile (tile > 0).  The words of kLookBatch predecessors
+// are requested together, so one memory round trip covers kLookBatch tiles.  Tile 0 always holds a
+// prefix word, so indices clamped to 0 are never summed twice.
 __device__ __forceinline__ u32 lookBackBatched(const u64* state, u32 c, u32 tile, u32 epoch)
 {
+    const u32 want = epoch & 0x3FFFFFFFu;
     u32 excl = 0;
     int p = (int)tile - 1;
-    while (p >= 0) {
+    for (;;) {
         u64 w[kLookBatch];
 #pragma unroll
-        for (int i = 0; i < kLookBatch; ++i)
-            if (p - i >= 0) w[i] = lbLoad(state + (size_t)(p - i) * kRadix + c);
+        for (int i = 0; i < kLookBatch; ++i) w[i] = lbLoad(state + (size_t)max(p - i, 0) * kRadix + c);
 #pragma unroll
         for (int i = 0; i < kLookBatch; ++i) {
-            if (p - i < 0) return excl;
-            while ((u32)(w[i] >> 34) != (epoch & 0x3FFFFFFFu)) {
+            u64 x = w[i];
+            while ((u32)(x >> 34) != want) {
                 __nanosleep(32);
-                w[i] = lbLoad(state + (size_t)(p - i) * kRadix + c);
+                x = lbLoad(state + (size_t)max(p - i, 0) * kRadix + c);
             }
-            excl += (u32)w[i];
-            if (((u32)(w[i] >> 32) & 3u) == kLbPrefix) return excl;
+            excl += (u32)x;
+            if (((u32)(x >> 32) & 3u) == kLbPrefix) return excl;
         }
         p -= kLookBatch;
     }
-    return excl;
 }
 
-// Lanes of the warp whose 8-bit digit equals this lane's: one ballot per digit bit (the native match.any
-// is far slower).  Per bit: s = bit ? ~0 : 0 (bfe.s32), p = (s != 0), v = ballot(p), peers &= ~(v ^ s).
+// Lanes of the warp whose digit equals this lane's: one ballot per digit bit (the native match.any is far
+// slower).  Per bit: p = bit set, v = ballot(p); a &= v where p, o |= v where !p; peers = a & ~o.
+// SASS per bit: VOTE + 2 predicated LOP3; the predicates of 7 bits come from one R2P.
 __device__ __forceinline__ u32 matchDigit(u32 d)
 {
-    u32 peers = kFull;
+    u32 a = kFull, o = 0;
 #pragma unroll
     for (int b = 0; b < kRadixBits; ++b) {
         asm("{\n\t"
             ".reg .pred p;\n\t"
-            ".reg .b32 s, v;\n\t"
-            "bfe.s32 s, %1, %2, 1;\n\t"
-            "setp.ne.s32 p, s, 0;\n\t"
+            ".reg .b32 t, v;\n\t"
+            "and.b32 t, %2, %3;\n\t"
+            "setp.ne.u32 p, t, 0;\n\t"
             "vote.sync.ballot.b32 v, p, 0xffffffff;\n\t"
-            "lop3.b32 %0, %0, v, s, 0x90;\n\t"
+            "@p and.b32 %0, %0, v;\n\t"
+            "@!p or.b32 %1, %1, v;\n\t"
             "}"
-            : "+r"(peers)
-            : "r"(d), "r"(b));
+            : "+r"(a), "+r"(o)
+            : "r"(d), "r"(1u << b));
     }
-    return peers;
+    return a & ~o;
 }
 
-template <bool FIRST, bool FULL>
+template <int SHIFT, bool FIRST, bool FULL>
 __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict__ keysIn, const u32* __restrict__ valsIn,
                                              u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
-                                             int shift, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
+                                             const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
     const u64 base = (u64)tile * kSortTile;
@@ -149,10 +164,6 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     // ---- load: warp-striped, so that (warp, item, lane) order == memory order (stability) ----
     u64 key[kSortItems];
     const u32 warpOff = warp * (32 * kSortItems) + lane;
-#if CS_SORT_PREFETCH
-    if (!FIRST && tid < kSortTile * 4 / 128)
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(valsIn + base + tid * 32));
-#endif
     const u64* src = keysIn + base + warpOff;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j)
@@ -163,59 +174,49 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     u32 rankPk[(kSortItems + 1) / 2];                                        // two 16-bit ranks per register
 #pragma unroll
     for (int j = 0; j < (kSortItems + 1) / 2; ++j) rankPk[j] = 0;
-    u32* wh = sm.warpHist[warp];
+    unsigned short* wh = sm.warpHist[warp];
     const u32 lt = laneMaskLt();
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        const u32 d = digitOf(key[j], shift);
+        const u32 d = digitOf(key[j], SHIFT);
         const u32 peers = matchDigit(d);
         const u32 lower = __popc(peers & lt);
         const u32 prev = wh[d];
         __syncwarp();
-        if (lower == 0) wh[d] = prev + __popc(peers);
+        if (lower == 0) wh[d] = (unsigned short)(prev + __popc(peers));
         __syncwarp();
         rankPk[j >> 1] |= (prev + lower) << ((j & 1) * 16);
     }
     __syncthreads();
 
-    // ---- per digit: exclusive prefix over warps, tile count, tile-local start ------------------
+    // ---- per digit (one thread each): tile count, tile-local start, first slot of every warp ------
     u32 count = 0;
     if (tid < kRadix) {
-        u32 run = 0;
 #pragma unroll
-        for (int w = 0; w < kSortWarps; ++w) {
-            u32 c = sm.warpHist[w][tid];
-            sm.warpHist[w][tid] = run;
-            run += c;
-        }
-        count = run;
+        for (int w = 0; w < kSortWarps; ++w) count += sm.warpHist[w][tid];
         // publish this tile's count at once: the tiles behind it can start their look-back
         const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;   // pads are not elements
         lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, tile == 0 ? kLbPrefix : kLbAggregate, real));
     }
     u32 total;
-    u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
+    const u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
     if (tid < kRadix) {
-        sm.digitStart[tid] = start;
-#if !CS_SORT_LATELB
-        // ---- decoupled look-back over preceding tiles, one thread per digit ----------------------
-        u32 excl = 0;
-        if (tile != 0) {
-            const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;
-            excl = lookBackBatched(lookback, tid, tile, epoch);
-            lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, kLbPrefix, excl + real));
+        u32 run = start;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w) {
+            const u32 c = sm.warpHist[w][tid];
+            sm.warpHist[w][tid] = (unsigned short)run;
+            run += c;
         }
-        sm.globalBase[tid] = digitBase[tid] + excl - start;
-#endif
     }
     __syncthreads();
 
     // ---- scatter keys, then values, into digit order in shared memory -----------------------------
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
-        u32 d = digitOf(key[j], shift);
+        const u32 d = digitOf(key[j], SHIFT);
         const u32 r = (rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
-        const u32 pos = sm.digitStart[d] + wh[d] + r;
+        const u32 pos = wh[d] + r;
         sm.keys[pos] = key[j];
         if (j & 1) rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFFu) | (pos << 16);
         else rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFF0000u) | pos;
@@ -231,9 +232,9 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     }
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) sm.vals[(rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu] = val[j];
-#if CS_SORT_LATELB
+
     // ---- decoupled look-back, after the shared-memory scatter: the predecessors have had that much
-    // longer to publish their prefixes, and the other warps are not kept waiting at a barrier ---------
+    // longer to publish their prefixes ---------------------------------------------------------------
     if (tid < kRadix) {
         u32 excl = 0;
         if (tile != 0) {
@@ -243,7 +244,6 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
         }
         sm.globalBase[tid] = digitBase[tid] + excl - start;
     }
-#endif
     __syncthreads();
 
     // ---- write out: consecutive threads -> consecutive slots of a digit's run ----------------------
@@ -252,32 +252,35 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
         const u32 i = tid + k * kSortBlock;
         if (FULL || i < valid) {
             const u64 kk = sm.keys[i];
-            const u32 dst = sm.globalBase[digitOf(kk, shift)] + i;
+            const u32 dst = sm.globalBase[digitOf(kk, SHIFT)] + i;
             keysOut[dst] = kk;
             valsOut[dst] = sm.vals[i];
         }
     }
 }
 
-template <bool FIRST>
+template <int PASS>
 __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
-                   u32* __restrict__ valsOut, u32 n, int shift, const u32* __restrict__ digitBase /*scanned hist*/,
-                   u32* ticket, u64* lookback, u32 epoch)
+                   u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase /*scanned hist*/, u32* ticket,
+                   u64* lookback, u32 epoch)
 {
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    constexpr int SHIFT = PASS * kRadixBits;
+    constexpr bool FIRST = PASS == 0;
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < kSortWarps * kRadix; i += kSortBlock) (&sm.warpHist[0][0])[i] = 0;
+    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
+    for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
     const u32 tile = sm.tile;
     const u64 base = (u64)tile * kSortTile;
     const u32 valid = (u32)((n - base) < (u64)kSortTile ? (n - base) : (u64)kSortTile);
     if (valid == kSortTile)
-        onesweepTile<FIRST, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, shift, digitBase, lookback, epoch);
+        onesweepTile<SHIFT, FIRST, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
     else
-        onesweepTile<FIRST, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, shift, digitBase, lookback, epoch);
+        onesweepTile<SHIFT, FIRST, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
 }
 
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
@@ -286,26 +289,47 @@ cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
     return CS_OK;
 }
 
-cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool histReady, cudaStream_t s)
+template <int PASS>
+static cs_status launchPasses(cs_context* ctx, u64* const* kbuf, u32* const* vbuf, u32 n, u32 tiles, cudaStream_t s)
+{
+    if constexpr (PASS < kSortPasses) {
+        static bool attrSet = false;
+        if (!attrSet) {
+            CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)sizeof(SortSmem)));
+            attrSet = true;
+        }
+        const u32 epoch = nextEpoch(ctx, s);
+        const int in = PASS & 1, out = in ^ 1;
+        onesweepKernel<PASS><<<tiles, kSortBlock, sizeof(SortSmem), s>>>(
+            kbuf[in], PASS == 0 ? nullptr : vbuf[in], kbuf[out], vbuf[out], n, ctx->sortHist + PASS * kRadix,
+            ctx->sortTickets + PASS, ctx->sortLookback, epoch);
+        CS_LAUNCH_CHECK(ctx, "onesweepKernel");
+        return launchPasses<PASS + 1>(ctx, kbuf, vbuf, n, tiles, s);
+    } else {
+        return CS_OK;
+    }
+}
+
+// The passes alternate between the caller's arrays and the workspace's; an odd number of passes
+// ends in `keys` only if the first pass reads the alternate buffer.
+u64* sortSource(cs_context* ctx, u64* keys) { return (kSortPasses & 1) ? ctx->keysAlt : keys; }
+
+// fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
+// (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
+cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_SORT, s);
     if (n == 0) return CS_OK;
-    static bool attrSet = false;
-    if (!attrSet) {
-        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)sizeof(SortSmem)));
-        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)sizeof(SortSmem)));
-        attrSet = true;
-    }
+    u64* first = sortSource(ctx, keys);
     {
         StageTimer th(ctx, CS_STAGE_SORT_HIST, s);
-        if (!histReady) {
+        if (!fused) {
             CS_TRY(enqueueSortReset(ctx, s));
             u32 grid = (u32)ctx->numSMs * 4;
             u32 need = divUp((n + 1) / 2, kHistBlock);
             if (need < grid) grid = need ? need : 1;
-            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist);
+            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first);
             CS_LAUNCH_CHECK(ctx, "sortHistKernel");
         }
         sortScanHistKernel<<<1, kRadix, 0, s>>>(ctx->sortHist);
@@ -313,22 +337,10 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool histRea
     }
     StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
     const u32 tiles = divUp(n, kSortTile);
-    u64* kbuf[2] = {keys, ctx->keysAlt};
-    u32* vbuf[2] = {perm, ctx->permAlt};
-    for (int p = 0; p < kSortPasses; ++p) {
-        const u32 epoch = nextEpoch(ctx, s);
-        const int in = p & 1, out = in ^ 1;
-        if (p == 0)
-            onesweepKernel<true><<<tiles, kSortBlock, sizeof(SortSmem), s>>>(
-                kbuf[in], nullptr, kbuf[out], vbuf[out], (u32)n, p * kRadixBits, ctx->sortHist + p * kRadix,
-                ctx->sortTickets + p, ctx->sortLookback, epoch);
-        else
-            onesweepKernel<false><<<tiles, kSortBlock, sizeof(SortSmem), s>>>(
-                kbuf[in], vbuf[in], kbuf[out], vbuf[out], (u32)n, p * kRadixBits, ctx->sortHist + p * kRadix,
-                ctx->sortTickets + p, ctx->sortLookback, epoch);
-        CS_LAUNCH_CHECK(ctx, "onesweepKernel");
-    }
-    return CS_OK;
+    u64* other = first == keys ? ctx->keysAlt : keys;
+    u64* kbuf[2] = {first, other};
+    u32* vbuf[2] = {first == keys ? perm : ctx->permAlt, first == keys ? ctx->permAlt : perm};
+    return launchPasses<0>(ctx, kbuf, vbuf, (u32)n, tiles, s);
 }
 
 }  // namespace cs
