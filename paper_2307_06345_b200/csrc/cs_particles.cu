@@ -8,7 +8,7 @@ namespace cs {
 constexpr int kBoxBlock = 512;
 constexpr int kBoxBlocksPerSM = 4;
 constexpr int kKeysBlock = 256;
-constexpr int kKeysBlocksPerSM = 8;
+constexpr int kKeysBlocksPerSM = 4;
 
 // ---------------------------------------------------------------------------------------------
 // H1: per-dimension min / max.  Each CTA reduces a grid-strided slice, writes 6 partials, and
@@ -174,28 +174,58 @@ __device__ __forceinline__ u32 spread11(u32 v)
     return v;
 }
 
-// floor and clamp in 32-bit: cvt.rmi.s32.f64 saturates (+-inf, huge) and maps NaN to 0
-__device__ __forceinline__ u32 gridCoordinate(double c, double lo, double e)
+// floor and clamp in 32-bit: cvt.rmi.s32.f64 saturates (+-inf, huge) and maps NaN to 0.
+//
+// The IEEE division of reading A2 costs ~25 instructions; its result is only needed to the integer
+// below it.  With r21 = RN(1/e) * 2^21 (exact scaling), t' = RN(a * r21) differs from the reference
+// t = RN(a / e) * 2^21 by at most 3 roundings, |t' - t| <= 3.01 * 2^-53 * 2^21 < 7.1e-10 for every
+// |a / e| <= 1 (coordinates outside that range clamp to the same grid cell on both paths).  So if
+// floor(t' - eps) == floor(t' + eps) with eps = 2^-27 = 7.45e-9 (the additions round by <= 2.4e-10),
+// no integer lies between t and t' and floor(t) == floor(t').  Otherwise (about 1.5e-8 of the
+// coordinates, or grid-aligned inputs) the reference expression itself is evaluated: exact on all inputs.
+struct BoxParams {
+    double lo[3], e[3], r21[3];   // r21 = 0 marks a dimension that always takes the reference expression
+};
+
+__device__ __forceinline__ u32 gridCoordinate(double c, double lo, double e, double r21)
 {
-    const double t = __dmul_rn(__ddiv_rn(__dsub_rn(c, lo), e), 2097152.0);
-    int g = __double2int_rd(t);
+    const double a = __dsub_rn(c, lo);
+    int g;
+    bool exact = true;
+    if (r21 != 0.0) {
+        const double t = __dmul_rn(a, r21);
+        const int g0 = __double2int_rd(__dadd_rn(t, -0x1p-27));
+        g = __double2int_rd(__dadd_rn(t, 0x1p-27));
+        exact = g0 != g;
+    }
+    if (exact) g = __double2int_rd(__dmul_rn(__ddiv_rn(a, e), 2097152.0));
     g = max(g, 0);
     g = min(g, 2097151);
     return (u32)g;
 }
 
-struct BoxParams {
-    double lo[3], e[3];
-};
+__device__ __forceinline__ BoxParams loadBox(const double* __restrict__ box6)
+{
+    BoxParams b;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        b.lo[d] = box6[2 * d];
+        b.e[d] = __dsub_rn(box6[2 * d + 1], box6[2 * d]);
+        // the bound above needs a normal reciprocal that can be scaled by 2^21 exactly
+        const bool ok = b.e[d] >= 0x1p-500 && b.e[d] <= 0x1p500;
+        b.r21[d] = ok ? __dmul_rn(__drcp_rn(b.e[d]), 2097152.0) : 0.0;
+    }
+    return b;
+}
 
 // Interleave as two 32-bit words (all spreading in 32-bit arithmetic):
 //   key bit 3b+2 = x bit b, 3b+1 = y bit b, 3b = z bit b   (digit = 4x + 2y + z, A3)
 //   low word : x bits 0..9, y bits 0..10, z bits 0..10;  high word: x bits 10..20, y and z bits 11..20
 __device__ __forceinline__ u64 mortonKey(double x, double y, double z, const BoxParams& b)
 {
-    const u32 gx = gridCoordinate(x, b.lo[0], b.e[0]);
-    const u32 gy = gridCoordinate(y, b.lo[1], b.e[1]);
-    const u32 gz = gridCoordinate(z, b.lo[2], b.e[2]);
+    const u32 gx = gridCoordinate(x, b.lo[0], b.e[0], b.r21[0]);
+    const u32 gy = gridCoordinate(y, b.lo[1], b.e[1], b.r21[1]);
+    const u32 gz = gridCoordinate(z, b.lo[2], b.e[2], b.r21[2]);
     const u32 lo = (spread11(gx & 0x3FFu) << 2) | (spread11(gy) << 1) | spread11(gz);
     const u32 hi = spread11(gx >> 10) | (spread11(gy >> 11) << 2) | (spread11(gz >> 11) << 1);
     return ((u64)hi << 32) | lo;
@@ -212,7 +242,7 @@ __device__ __forceinline__ void histAdd(u32* sh, u64 key)
 }
 
 template <bool VEC, bool HIST>
-__global__ void __launch_bounds__(kKeysBlock) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
+__global__ void __launch_bounds__(kKeysBlock, 4) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
                                                          const double* __restrict__ z, u64 n,
                                                          const double* __restrict__ box6, u64* __restrict__ keys,
                                                          u32* gHist)
@@ -222,17 +252,29 @@ __global__ void __launch_bounds__(kKeysBlock) keysKernel(const double* __restric
         for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) sh[i] = 0;
         __syncthreads();
     }
-    BoxParams b;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        b.lo[d] = box6[2 * d];
-        b.e[d] = __dsub_rn(box6[2 * d + 1], box6[2 * d]);
-    }
+    const BoxParams b = loadBox(box6);
     const u64 tid = (u64)blockIdx.x * kKeysBlock + threadIdx.x;
     const u64 nthreads = (u64)gridDim.x * kKeysBlock;
     if (VEC) {
         const u64 pairs = n >> 1;
-        for (u64 i = tid; i < pairs; i += nthreads) {
+        u64 i = tid;
+        // two iterations of loads in flight per thread (96 B)
+        for (; i + nthreads < pairs; i += 2 * nthreads) {
+            const u64 i2 = i + nthreads;
+            double2 ax = ldStreamD2(x + 2 * i), ay = ldStreamD2(y + 2 * i), az = ldStreamD2(z + 2 * i);
+            double2 bx = ldStreamD2(x + 2 * i2), by = ldStreamD2(y + 2 * i2), bz = ldStreamD2(z + 2 * i2);
+            u64 k0 = mortonKey(ax.x, ay.x, az.x, b);
+            u64 k1 = mortonKey(ax.y, ay.y, az.y, b);
+            stStreamU2(keys + 2 * i, k0, k1);
+            histAdd<HIST>(sh, k0);
+            histAdd<HIST>(sh, k1);
+            k0 = mortonKey(bx.x, by.x, bz.x, b);
+            k1 = mortonKey(bx.y, by.y, bz.y, b);
+            stStreamU2(keys + 2 * i2, k0, k1);
+            histAdd<HIST>(sh, k0);
+            histAdd<HIST>(sh, k1);
+        }
+        for (; i < pairs; i += nthreads) {
             double2 vx = ldStreamD2(x + 2 * i);
             double2 vy = ldStreamD2(y + 2 * i);
             double2 vz = ldStreamD2(z + 2 * i);
