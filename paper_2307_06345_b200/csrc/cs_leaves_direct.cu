@@ -199,10 +199,16 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
     const u32 W = b + 1;
     u32 len = 1;                                           // byte i = max of w over [i, i + len)
     while (len * 4 <= W) {
-        for (u32 q = tid; q < L.words; q += kDirBlock) {
-            const u32 a = __vmaxu4(src[q], dirShifted(src, q, len));
-            const u32 c = __vmaxu4(dirShifted(src, q, 2 * len), dirShifted(src, q, 3 * len));
-            dst[q] = __vmaxu4(a, c);
+        if ((len & 3u) == 0) {                             // whole-word offsets: no funnel shifts
+            const u32 o = len >> 2;
+            for (u32 q = tid; q < L.words; q += kDirBlock)
+                dst[q] = __vmaxu4(__vmaxu4(src[q], src[q + o]), __vmaxu4(src[q + 2 * o], src[q + 3 * o]));
+        } else {
+            for (u32 q = tid; q < L.words; q += kDirBlock) {
+                const u32 a = __vmaxu4(src[q], dirShifted(src, q, len));
+                const u32 c = __vmaxu4(dirShifted(src, q, 2 * len), dirShifted(src, q, 3 * len));
+                dst[q] = __vmaxu4(a, c);
+            }
         }
         __syncthreads();
         u32* t = src; src = dst; dst = t;
@@ -291,23 +297,24 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
 // ---- kernel 2: emission ---------------------------------------------------------------------------
 // The same tiles; bases = exclusive prefix of totals over tiles (bases[tiles] = all K entries).  The
 // listed positions fetch their two keys and levels from global memory; everything else is a bit scan.
-__global__ void __launch_bounds__(kDirBlock)
+constexpr int kEmitBlock = kDirBlock / 2;                 // 16 positions per thread: most threads hold a listed position
+__global__ void __launch_bounds__(kEmitBlock)
     leavesEmitDirectKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const unsigned char* __restrict__ dArr,
                            const unsigned char* __restrict__ flags, const u32* __restrict__ bases, u32 tiles,
                            u64* __restrict__ K, u32* __restrict__ off, u32 cap)
 {
     __shared__ unsigned short list[kDirTile];
-    __shared__ u32 warpSums[kDirBlock / 32 + 1];
+    __shared__ u32 warpSums[kEmitBlock / 32 + 1];
     const u32 tid = threadIdx.x;
     const u32 tile = blockIdx.x;
     const u64 T0 = (u64)tile * kDirTile;
-    const u32 fbyte = flags[(size_t)tile * kDirBlock + tid];
-    u32 nb;
-    u32 slot = blockExclusiveScan<kDirBlock>(__popc(fbyte), warpSums, &nb);
-    for (u32 f = fbyte; f; f &= f - 1) list[slot++] = (unsigned short)(8 * tid + __ffs((int)f) - 1);
-    __syncthreads();
+    const u32 fbits = reinterpret_cast<const unsigned short*>(flags)[(size_t)tile * kEmitBlock + tid];
     u32 carry = bases[tile];
-    for (u32 base = 0; base < nb; base += kDirBlock) {
+    u32 nb;
+    u32 slot = blockExclusiveScan<kEmitBlock>(__popc(fbits), warpSums, &nb);
+    for (u32 f = fbits; f; f &= f - 1) list[slot++] = (unsigned short)(16 * tid + __ffs((int)f) - 1);
+    __syncthreads();
+    for (u32 base = 0; base < nb; base += kEmitBlock) {
         const u32 m = base + tid;
         u64 a = 0, c = 0;
         int Da = 0, Dc = 0;
@@ -325,7 +332,7 @@ __global__ void __launch_bounds__(kDirBlock)
             cnt = dirCount(a, c, Da, Dc, j, n);
         }
         u32 t;
-        const u32 e = blockExclusiveScan<kDirBlock>(cnt, warpSums, &t);
+        const u32 e = blockExclusiveScan<kEmitBlock>(cnt, warpSums, &t);
         if (cnt) dirEmit(a, c, Da, Dc, j, n, carry + e, K, off, cap);
         carry += t;
         __syncthreads();                                    // warpSums is reused by the next chunk
@@ -389,7 +396,7 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
                                                          ctx->dirTotals);
     CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
     CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));
-    leavesEmitDirectKernel<<<tiles, kDirBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
+    leavesEmitDirectKernel<<<tiles, kEmitBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
                                                        ctx->leafK[0], ctx->leafOff[0], cap);
     CS_LAUNCH_CHECK(ctx, "leavesEmitDirectKernel");
     return CS_OK;
