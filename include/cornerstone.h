@@ -106,6 +106,17 @@ cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, cons
  */
 cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream);
 
+/* cs_setSortMode -- how cs_sortKeys / cs_buildOctree reach the (unique) stable order.
+ *   CS_SORT_AUTO (default): 5 radix passes over the 5 leading 9-bit digits, then the low 18
+ *   bits are ordered inside every run of equal leading digits; if some run is longer than
+ *   257 elements (particles deeper than octree level 15 in bulk) the 7 plain passes are run
+ *   behind it instead, decided on the device with no host round trip.  cs_buildOctree
+ *   remembers that outcome and uses the plain passes directly from then on.
+ *   CS_SORT_PLAIN: always the 7 plain LSD passes (9 bits each).
+ *   The sorted keys and perm are identical in both modes.  Errors: INVALID_ARG. */
+enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1 };
+cs_status cs_setSortMode(cs_context* ctx, int mode);
+
 /* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1
  *   (Eqs. 4-9), until a round reports O_i = 1 for all i.
  *   sortedKeys: dev, n ascending keys < 2^63 (the array P).  bucketSize = N_crit >= 1.

@@ -28,6 +28,7 @@ NUM_STAGES = 8
 STAGE_NAMES = ("box", "keys", "sort", "leaves", "link", "counts", "sort_hist", "sort_passes")
 
 LEAVES_AUTO, LEAVES_ITERATIVE = 0, 1
+SORT_AUTO, SORT_PLAIN = 0, 1
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_NOT_CORNERSTONE, ERR_NOT_CONVERGED, ERR_CUDA = range(6)
 _STATUS_NAMES = {0: "CS_OK", 1: "CS_ERR_INVALID_ARG", 2: "CS_ERR_CAPACITY", 3: "CS_ERR_NOT_CORNERSTONE",
                  4: "CS_ERR_NOT_CONVERGED", 5: "CS_ERR_CUDA"}
@@ -76,6 +77,7 @@ def lib():
         "cs_setProfiling": (C.c_int, [vp, C.c_int]),
         "cs_stageTimes": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(u64)]),
         "cs_setLeafMode": (C.c_int, [vp, C.c_int]),
+        "cs_setSortMode": (C.c_int, [vp, C.c_int]),
         "cs_computeBox": (C.c_int, [vp, vp, vp, vp, u64, vp, vp]),
         "cs_computeKeys": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
         "cs_sortKeys": (C.c_int, [vp, vp, vp, u64, vp]),
@@ -171,6 +173,10 @@ class Context:
     def setLeafMode(self, mode: int):
         """LEAVES_AUTO (one-pass fixpoint from the root) or LEAVES_ITERATIVE (always the rounds f, g)."""
         self.check(lib().cs_setLeafMode(self.handle, int(mode)))
+
+    def setSortMode(self, mode: int):
+        """SORT_AUTO (5 passes + fix-up of the low bits, plain passes behind it if needed) or SORT_PLAIN."""
+        self.check(lib().cs_setSortMode(self.handle, int(mode)))
 
     def stageTimes(self):
         ms = (C.c_float * NUM_STAGES)()

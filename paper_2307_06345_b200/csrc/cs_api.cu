@@ -107,6 +107,15 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
     return statusFromCtrl(ctx, "cs_buildLeaves");
 }
 
+cs_status cs_setSortMode(cs_context* ctx, int mode)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setSortMode: ctx is null");
+    if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_setSortMode: unknown mode %d", mode);
+    ctx->sortPlain = mode == CS_SORT_PLAIN;
+    return CS_OK;
+}
+
 cs_status cs_setLeafMode(cs_context* ctx, int mode)
 {
     if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setLeafMode: ctx is null");
@@ -200,6 +209,7 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
                        b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,
                        ctx->leafOffFinal, b->nodeFirst, b->nodeCount, s));
     CS_TRY(readCtrl(ctx, s));
+    if (ctx->hostCtrl->sortRedo) ctx->sortPlain = true;   // deep clustering: skip the short cut from now on
     const DeviceCtrl& c = ctx->hostCtrl->c;
     sizes->rounds = c.rounds;
     sizes->converged = c.converged;

@@ -86,6 +86,8 @@ u32 nextEpoch(cs_context* ctx, cudaStream_t s)
 cs_status readCtrl(cs_context* ctx, cudaStream_t s)
 {
     CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->c, ctx->ctrl, sizeof(DeviceCtrl), cudaMemcpyDeviceToHost, s));
+    CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedo, ctx->sortTickets + kSortRedoSlot, sizeof(u32),
+                                 cudaMemcpyDeviceToHost, s));
     CS_CUDA(ctx, cudaStreamSynchronize(s));
     return CS_OK;
 }

@@ -83,7 +83,9 @@ struct DeviceCtrl {
 
 struct HostCtrl {                // pinned mirror read back once per call
     DeviceCtrl c;
+    u32 sortRedo;                // the sort's fix-up gave up and the plain passes ran (cs_sort.cu)
 };
+constexpr int kSortRedoSlot = 63;   // ctx->sortTickets[kSortRedoSlot]: that flag on the device
 
 }  // namespace cs
 
@@ -104,6 +106,7 @@ struct cs_context {
     cs::u32* sortTickets = nullptr;
     cs::u64* sortLookback = nullptr;   // [tiles][kRadix]
     cs::u32 epoch = 0;                 // look-back epoch, bumped per launch that uses a look-back array
+    bool sortPlain = false;            // run the 7 plain radix passes (set once a build needed the redo, or by cs_setSortMode)
 
     // box
     double* boxPartials = nullptr;     // [grid][6]

@@ -1,16 +1,24 @@
 // H3: stable LSD radix sort of (u64 key, u32 index) pairs -- PAPER.md:70, 168; A5.
 //
 // "Onesweep" organisation: one histogram pass over the keys gives the global digit counts of
-// all passes; every pass then reads each element once and writes it once.  63 key bits in 7
-// passes of 9 bits.  A pass tile is ranked inside the CTA (warp-level ballot matching + per-warp
+// all passes; every pass then reads each element once and writes it once.  63 key bits = 7
+// digits of 9 bits.  A pass tile is ranked inside the CTA (warp-level ballot matching + per-warp
 // digit counters), the tile's position in each digit's output run comes from a decoupled
 // look-back over the preceding tiles' digit counts (one thread per digit, all 512 threads of the
 // CTA), and the tile is written out through shared memory so that each digit's run is a
 // contiguous burst.  Tiles take their index from an atomic ticket, so a tile only ever waits
-// for tiles that are already running (forward progress).
+// for tiles that are already running (forward progress); the CTAs are persistent.
 //
-// Model bytes per particle (SURVEY 8d, 8 passes): 196; moved by this 7-pass sort:
-// histogram 0 (fused into the key kernel, else 8) + pass 0 (8 read, 12 written) + 6 x 24 = 164.
+// Short cut: SFC keys of N particles are all but decided by their leading
+// digits.  The default path sorts by the 5 leading digits (bits 18..62) with 5 passes and then
+// orders the low 18 bits inside every run of equal leading digits directly (sortFixupKernel:
+// rank = elements of the run that must precede, counted by scanning the run, O(run length) per
+// element).  A run longer than kFixupMaxRun + 1 raises a device flag instead; the 7 plain passes
+// that follow in the stream are gated on that flag and redo the sort from the (still complete)
+// output of pass 5.  Either way the result is the stable sort: parity does not depend on the path.
+//
+// Model bytes per particle (SURVEY 8d, 8 passes of 8 bits): 196; moved by the default path:
+// pass 0 (8 read, 12 written) + 4 x 24 + fix-up 24 = 140 (histograms come from the key kernel).
 #include "cs_device.cuh"
 
 namespace cs {
@@ -259,7 +267,8 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     }
 }
 
-template <int PASS>
+// One tile per CTA (grid = tiles): the passes of the default path and of cs_setSortMode(PLAIN).
+template <int SHIFT, bool FIRST>
 __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
                    u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase /*scanned hist*/, u32* ticket,
@@ -267,8 +276,6 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
 {
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
-    constexpr int SHIFT = PASS * kRadixBits;
-    constexpr bool FIRST = PASS == 0;
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
     u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
@@ -283,37 +290,157 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
         onesweepTile<SHIFT, FIRST, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
 }
 
+// The redo passes behind the fix-up: persistent CTAs that leave at once unless *gate != 0, so that
+// the default path pays a few microseconds for them, not a wave of empty CTAs per pass.
+template <int SHIFT>
+__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
+    onesweepGatedKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
+                        u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase, u32* ticket, u64* lookback,
+                        u32 epoch, const u32* gate)
+{
+    extern __shared__ __align__(16) unsigned char smemRaw[];
+    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    const u32 tid = threadIdx.x;
+    if (*reinterpret_cast<const volatile u32*>(gate) == 0) return;
+    const u32 tiles = (n + kSortTile - 1) / kSortTile;
+    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
+    for (;;) {
+        __syncthreads();                                   // the previous tile is written out
+        if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+        for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
+        __syncthreads();
+        const u32 tile = sm.tile;
+        if (tile >= tiles) break;
+        const u64 base = (u64)tile * kSortTile;
+        const u32 valid = (u32)((n - base) < (u64)kSortTile ? (n - base) : (u64)kSortTile);
+        if (valid == kSortTile)
+            onesweepTile<SHIFT, false, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
+        else
+            onesweepTile<SHIFT, false, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
+    }
+}
+
+// ---- fix-up of the low bits inside runs of equal leading digits ----------------------------------------
+// In: elements stably sorted by key >> LOW.  Out: stably sorted by the whole key.  An element moves
+// inside its run only: to runStart + (elements of the run with smaller low bits) + (elements of the run
+// before it with equal low bits).  Neighbours are read through L1 (the lines were just loaded by the
+// adjacent threads).  Runs longer than kFixupMaxRun + 1: *redo = 1 and the kernel gives up.
+constexpr int kFixupBlock = 256;
+constexpr u32 kFixupMaxRun = 256;
+
+template <int LOW>
+__global__ void __launch_bounds__(kFixupBlock)
+    sortFixupKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
+                    u32* __restrict__ valsOut, u32 n, u32* redo)
+{
+    const u32 stride = gridDim.x * kFixupBlock;
+    u32 it = 0;
+    for (u32 i = blockIdx.x * kFixupBlock + threadIdx.x; i < n; i += stride, ++it) {
+        const u64 key = keysIn[i];
+        const u32 val = ldStreamU32(valsIn + i);
+        // same run <=> the keys agree above bit LOW; inside a run the key order is the order of the low bits
+        const u64 kl = keysIn[i > 0 ? i - 1 : 0], kr = keysIn[i + 1 < n ? i + 1 : i];
+        const bool runL = i > 0 && ((kl ^ key) >> LOW) == 0, runR = i + 1 < n && ((kr ^ key) >> LOW) == 0;
+        u32 dst = i;
+        if (runL || runR) {                                 // not alone in its run: count what precedes it
+            u32 before = 0, j = i, e = i + 1;               // the run is [j, e)
+            bool tooLong = false;
+            if (runL) {
+                before += kl <= key;                        // to the left: smaller or equal low bits precede
+                --j;
+                while (j > 0) {
+                    const u64 k = keysIn[j - 1];
+                    if (((k ^ key) >> LOW) != 0) break;
+                    before += k <= key;
+                    --j;
+                    if (i - j > kFixupMaxRun) { tooLong = true; break; }
+                }
+            }
+            if (runR && !tooLong) {
+                before += kr < key;                         // to the right: strictly smaller low bits precede
+                ++e;
+                while (e < n) {
+                    const u64 k = keysIn[e];
+                    if (((k ^ key) >> LOW) != 0) break;
+                    before += k < key;
+                    ++e;
+                    if (e - i > kFixupMaxRun) { tooLong = true; break; }
+                }
+            }
+            if (tooLong) {                                  // the gated passes redo the sort
+                *reinterpret_cast<volatile u32*>(redo) = 1u;
+                return;
+            }
+            dst = j + before;
+        }
+        keysOut[dst] = key;
+        valsOut[dst] = val;
+        // now and then: no point in finishing once another thread has given up
+        if ((it & 15u) == 15u && *reinterpret_cast<const volatile u32*>(redo)) return;
+    }
+}
+
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
 {
     CS_CUDA(ctx, cudaMemsetAsync(ctx->sortHist, 0, (kSortPasses * kRadix + 64) * sizeof(u32), s));
     return CS_OK;
 }
 
-template <int PASS>
-static cs_status launchPasses(cs_context* ctx, u64* const* kbuf, u32* const* vbuf, u32 n, u32 tiles, cudaStream_t s)
+constexpr int kTopPasses = 5;                               // digits 2..6 (bits 18..62) before the fix-up
+constexpr int kFixupLow = (kSortPasses - kTopPasses) * kRadixBits;
+static_assert(kSortPasses == 7 && kRadixBits == 9, "the pass plan below is written for 7 digits of 9 bits");
+
+struct PassPlan {
+    u64* k[2];
+    u32* v[2];
+    int cur;                                                // buffers holding the current order
+    u32 n, tiles;
+    int ticketSlot;
+};
+
+template <int SHIFT, bool FIRST>
+static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 {
-    if constexpr (PASS < kSortPasses) {
-        static bool attrSet = false;
-        if (!attrSet) {
-            CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SortSmem)));
-            attrSet = true;
-        }
-        const u32 epoch = nextEpoch(ctx, s);
-        const int in = PASS & 1, out = in ^ 1;
-        onesweepKernel<PASS><<<tiles, kSortBlock, sizeof(SortSmem), s>>>(
-            kbuf[in], PASS == 0 ? nullptr : vbuf[in], kbuf[out], vbuf[out], n, ctx->sortHist + PASS * kRadix,
-            ctx->sortTickets + PASS, ctx->sortLookback, epoch);
-        CS_LAUNCH_CHECK(ctx, "onesweepKernel");
-        return launchPasses<PASS + 1>(ctx, kbuf, vbuf, n, tiles, s);
-    } else {
-        return CS_OK;
+    static bool attrSet = false;
+    if (!attrSet) {
+        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<SHIFT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)sizeof(SortSmem)));
+        attrSet = true;
     }
+    const u32 epoch = nextEpoch(ctx, s);
+    const int in = pl.cur, out = in ^ 1;
+    onesweepKernel<SHIFT, FIRST><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
+        pl.k[in], FIRST ? nullptr : pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
+        ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch);
+    CS_LAUNCH_CHECK(ctx, "onesweepKernel");
+    pl.cur = out;
+    return CS_OK;
 }
 
-// The passes alternate between the caller's arrays and the workspace's; an odd number of passes
-// ends in `keys` only if the first pass reads the alternate buffer.
-u64* sortSource(cs_context* ctx, u64* keys) { return (kSortPasses & 1) ? ctx->keysAlt : keys; }
+template <int SHIFT>
+static cs_status launchGatedPass(cs_context* ctx, PassPlan& pl, const u32* gate, cudaStream_t s)
+{
+    static bool attrSet = false;
+    if (!attrSet) {
+        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepGatedKernel<SHIFT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)sizeof(SortSmem)));
+        attrSet = true;
+    }
+    const u32 epoch = nextEpoch(ctx, s);
+    const int in = pl.cur, out = in ^ 1;
+    const u32 resident = (u32)ctx->numSMs * kSortMinBlocks;
+    onesweepGatedKernel<SHIFT><<<pl.tiles < resident ? pl.tiles : resident, kSortBlock, sizeof(SortSmem), s>>>(
+        pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
+        ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, gate);
+    CS_LAUNCH_CHECK(ctx, "onesweepGatedKernel");
+    pl.cur = out;
+    return CS_OK;
+}
+
+// Where the first radix pass reads the unsorted keys.  The passes alternate between the caller's
+// arrays and the workspace's: the default path (5 passes + fix-up, and 7 more if redone) ends where
+// it started; the plain 7 passes end in the other pair.
+u64* sortSource(cs_context* ctx, u64* keys) { return ctx->sortPlain ? ctx->keysAlt : keys; }
 
 // fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
 // (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
@@ -336,11 +463,48 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
     }
     StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
-    const u32 tiles = divUp(n, kSortTile);
-    u64* other = first == keys ? ctx->keysAlt : keys;
-    u64* kbuf[2] = {first, other};
-    u32* vbuf[2] = {first == keys ? perm : ctx->permAlt, first == keys ? ctx->permAlt : perm};
-    return launchPasses<0>(ctx, kbuf, vbuf, (u32)n, tiles, s);
+    PassPlan pl;
+    const bool own = first == keys;
+    pl.k[0] = first; pl.k[1] = own ? ctx->keysAlt : keys;
+    pl.v[0] = own ? perm : ctx->permAlt; pl.v[1] = own ? ctx->permAlt : perm;
+    pl.cur = 0;
+    pl.n = (u32)n;
+    pl.tiles = divUp(n, kSortTile);
+    pl.ticketSlot = 0;
+    if (ctx->sortPlain) {                                   // all 7 digits, least significant first
+        CS_TRY((launchPass<0, true>(ctx, pl, s)));
+        CS_TRY((launchPass<9, false>(ctx, pl, s)));
+        CS_TRY((launchPass<18, false>(ctx, pl, s)));
+        CS_TRY((launchPass<27, false>(ctx, pl, s)));
+        CS_TRY((launchPass<36, false>(ctx, pl, s)));
+        CS_TRY((launchPass<45, false>(ctx, pl, s)));
+        return launchPass<54, false>(ctx, pl, s);
+    }
+    // leading digits, most of the order
+    CS_TRY((launchPass<18, true>(ctx, pl, s)));
+    CS_TRY((launchPass<27, false>(ctx, pl, s)));
+    CS_TRY((launchPass<36, false>(ctx, pl, s)));
+    CS_TRY((launchPass<45, false>(ctx, pl, s)));
+    CS_TRY((launchPass<54, false>(ctx, pl, s)));
+    // low bits inside the runs; out of place, so the input stays intact for a redo
+    u32* redo = ctx->sortTickets + kSortRedoSlot;
+    {
+        u32 grid = divUp(n, kFixupBlock);
+        const u32 cap = (u32)ctx->numSMs * 32;
+        if (grid > cap) grid = cap;
+        const int in = pl.cur, out = in ^ 1;
+        sortFixupKernel<kFixupLow><<<grid, kFixupBlock, 0, s>>>(pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, redo);
+        CS_LAUNCH_CHECK(ctx, "sortFixupKernel");
+    }
+    // gated redo from the output of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
+    // which is where the fix-up wrote
+    CS_TRY((launchGatedPass<0>(ctx, pl, redo, s)));
+    CS_TRY((launchGatedPass<9>(ctx, pl, redo, s)));
+    CS_TRY((launchGatedPass<18>(ctx, pl, redo, s)));
+    CS_TRY((launchGatedPass<27>(ctx, pl, redo, s)));
+    CS_TRY((launchGatedPass<36>(ctx, pl, redo, s)));
+    CS_TRY((launchGatedPass<45>(ctx, pl, redo, s)));
+    return launchGatedPass<54>(ctx, pl, redo, s);
 }
 
 }  // namespace cs
