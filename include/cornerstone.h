@@ -52,7 +52,10 @@ typedef enum cs_status {
 /* Stage identifiers for cs_stageTimes (milliseconds of device time, CUDA events). */
 enum {
     CS_STAGE_BOX = 0, CS_STAGE_KEYS = 1, CS_STAGE_SORT = 2, CS_STAGE_LEAVES = 3, CS_STAGE_LINK = 4,
-    CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6, CS_STAGE_SORT_PASSES = 7, CS_NUM_STAGES = 8
+    CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6,
+    CS_STAGE_SORT_PASSES = 7,    /* the radix passes that always run: 5 (CS_SORT_AUTO) or 7 (CS_SORT_PLAIN) */
+    CS_STAGE_SORT_FIXUP = 8,     /* CS_SORT_AUTO: fix-up of the low 18 bits + the gated redo passes behind it */
+    CS_NUM_STAGES = 9
 };
 
 /* ---- context ------------------------------------------------------------------------ */
@@ -116,6 +119,8 @@ cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t 
  *   The sorted keys and perm are identical in both modes.  Errors: INVALID_ARG. */
 enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1 };
 cs_status cs_setSortMode(cs_context* ctx, int mode);
+/* Radix passes the next sort on this context launches unconditionally: 5 or 7 (0 if ctx is NULL). */
+int cs_sortPasses(const cs_context* ctx);
 
 /* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1
  *   (Eqs. 4-9), until a round reports O_i = 1 for all i.

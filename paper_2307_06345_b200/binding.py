@@ -24,8 +24,8 @@ L = 21
 KEY_END = 1 << 63
 NUM_LEVEL_OFFSETS = 23
 NO_LEAF = 0xFFFFFFFF
-NUM_STAGES = 8
-STAGE_NAMES = ("box", "keys", "sort", "leaves", "link", "counts", "sort_hist", "sort_passes")
+NUM_STAGES = 9
+STAGE_NAMES = ("box", "keys", "sort", "leaves", "link", "counts", "sort_hist", "sort_passes", "sort_fixup")
 
 LEAVES_AUTO, LEAVES_ITERATIVE = 0, 1
 SORT_AUTO, SORT_PLAIN = 0, 1
@@ -78,6 +78,7 @@ def lib():
         "cs_stageTimes": (C.c_int, [vp, C.POINTER(C.c_float), C.POINTER(u64)]),
         "cs_setLeafMode": (C.c_int, [vp, C.c_int]),
         "cs_setSortMode": (C.c_int, [vp, C.c_int]),
+        "cs_sortPasses": (C.c_int, [vp]),
         "cs_computeBox": (C.c_int, [vp, vp, vp, vp, u64, vp, vp]),
         "cs_computeKeys": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
         "cs_sortKeys": (C.c_int, [vp, vp, vp, u64, vp]),
@@ -177,6 +178,10 @@ class Context:
     def setSortMode(self, mode: int):
         """SORT_AUTO (5 passes + fix-up of the low bits, plain passes behind it if needed) or SORT_PLAIN."""
         self.check(lib().cs_setSortMode(self.handle, int(mode)))
+
+    def sortPasses(self) -> int:
+        """Radix passes the next sort launches unconditionally (5 with the fix-up, 7 plain)."""
+        return int(lib().cs_sortPasses(self.handle))
 
     def stageTimes(self):
         ms = (C.c_float * NUM_STAGES)()

@@ -116,6 +116,8 @@ cs_status cs_setSortMode(cs_context* ctx, int mode)
     return CS_OK;
 }
 
+int cs_sortPasses(const cs_context* ctx) { return ctx ? (ctx->sortPlain ? 7 : 5) : 0; }
+
 cs_status cs_setLeafMode(cs_context* ctx, int mode)
 {
     if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setLeafMode: ctx is null");

@@ -343,35 +343,41 @@ __global__ void __launch_bounds__(kFixupBlock)
         const bool runL = i > 0 && ((kl ^ key) >> LOW) == 0, runR = i + 1 < n && ((kr ^ key) >> LOW) == 0;
         u32 dst = i;
         if (runL || runR) {                                 // not alone in its run: count what precedes it
-            u32 before = 0, j = i, e = i + 1;               // the run is [j, e)
-            bool tooLong = false;
-            if (runL) {
-                before += kl <= key;                        // to the left: smaller or equal low bits precede
-                --j;
-                while (j > 0) {
-                    const u64 k = keysIn[j - 1];
-                    if (((k ^ key) >> LOW) != 0) break;
+            // the input is ordered by the leading bits, so the run is where runLo <= k < runHi
+            const u64 runLo = key & ~((1ull << LOW) - 1), runHi = runLo + (1ull << LOW);
+            u32 before = 0;
+            const u64* p = keysIn + i;                      // walks to the start of the run
+            if (runL) {                                     // to the left: smaller or equal low bits precede
+                const u64* stop = keysIn + (i > kFixupMaxRun ? i - kFixupMaxRun : 0);   // at most kFixupMaxRun to the left
+                before += kl <= key;
+                --p;
+                while (p > stop) {
+                    const u64 k = p[-1];
+                    if (k < runLo) break;
                     before += k <= key;
-                    --j;
-                    if (i - j > kFixupMaxRun) { tooLong = true; break; }
+                    --p;
+                }
+                if (p == stop && p > keysIn && p[-1] >= runLo) {   // longer than the limit: the gated passes redo the sort
+                    *reinterpret_cast<volatile u32*>(redo) = 1u;
+                    return;
                 }
             }
-            if (runR && !tooLong) {
-                before += kr < key;                         // to the right: strictly smaller low bits precede
-                ++e;
-                while (e < n) {
-                    const u64 k = keysIn[e];
-                    if (((k ^ key) >> LOW) != 0) break;
+            if (runR) {                                     // to the right: strictly smaller low bits precede
+                const u64* q = keysIn + i + 2;
+                const u64* stop = keysIn + (n - i > kFixupMaxRun + 1 ? i + kFixupMaxRun + 1 : n);   // and to the right
+                before += kr < key;
+                while (q < stop) {
+                    const u64 k = *q;
+                    if (k >= runHi) break;
                     before += k < key;
-                    ++e;
-                    if (e - i > kFixupMaxRun) { tooLong = true; break; }
+                    ++q;
+                }
+                if (q == stop && q < keysIn + n && *q < runHi) {
+                    *reinterpret_cast<volatile u32*>(redo) = 1u;
+                    return;
                 }
             }
-            if (tooLong) {                                  // the gated passes redo the sort
-                *reinterpret_cast<volatile u32*>(redo) = 1u;
-                return;
-            }
-            dst = j + before;
+            dst = (u32)(p - keysIn) + before;
         }
         keysOut[dst] = key;
         valsOut[dst] = val;
@@ -462,7 +468,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         sortScanHistKernel<<<1, kRadix, 0, s>>>(ctx->sortHist);
         CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
     }
-    StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
+    ctx->evUsed[CS_STAGE_SORT_FIXUP] = false;
     PassPlan pl;
     const bool own = first == keys;
     pl.k[0] = first; pl.k[1] = own ? ctx->keysAlt : keys;
@@ -472,6 +478,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     pl.tiles = divUp(n, kSortTile);
     pl.ticketSlot = 0;
     if (ctx->sortPlain) {                                   // all 7 digits, least significant first
+        StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
         CS_TRY((launchPass<0, true>(ctx, pl, s)));
         CS_TRY((launchPass<9, false>(ctx, pl, s)));
         CS_TRY((launchPass<18, false>(ctx, pl, s)));
@@ -480,12 +487,15 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         CS_TRY((launchPass<45, false>(ctx, pl, s)));
         return launchPass<54, false>(ctx, pl, s);
     }
-    // leading digits, most of the order
-    CS_TRY((launchPass<18, true>(ctx, pl, s)));
-    CS_TRY((launchPass<27, false>(ctx, pl, s)));
-    CS_TRY((launchPass<36, false>(ctx, pl, s)));
-    CS_TRY((launchPass<45, false>(ctx, pl, s)));
-    CS_TRY((launchPass<54, false>(ctx, pl, s)));
+    {   // leading digits, most of the order
+        StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
+        CS_TRY((launchPass<18, true>(ctx, pl, s)));
+        CS_TRY((launchPass<27, false>(ctx, pl, s)));
+        CS_TRY((launchPass<36, false>(ctx, pl, s)));
+        CS_TRY((launchPass<45, false>(ctx, pl, s)));
+        CS_TRY((launchPass<54, false>(ctx, pl, s)));
+    }
+    StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     // low bits inside the runs; out of place, so the input stays intact for a redo
     u32* redo = ctx->sortTickets + kSortRedoSlot;
     {

@@ -1,0 +1,145 @@
+"""GPU parity of cs_sortKeys on every path of cs_sort.cu against the oracle's stable sort (O3).
+
+Default path: 5 radix passes over the leading 45 bits + fix-up of the low 18 bits inside runs of
+equal leading bits; a run longer than 257 elements raises the device flag and the 7 gated plain
+passes redo the sort.  cs_setSortMode(PLAIN) runs the 7 plain passes directly.  All of them must
+return the same (unique) keys and permutation, bit for bit.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2307_06345_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+LOW = 18            # bits ordered by the fix-up
+MAX_RUN = 257       # longest run the fix-up takes (kFixupMaxRun + 1)
+
+
+@pytest.fixture(scope="module")
+def cs():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2307_06345_b200 import binding
+    return binding
+
+
+@pytest.fixture()
+def ctx(cs):
+    c = cs.Context(max_particles=1 << 21, max_leaves=1 << 18)
+    yield c
+    c.close()
+
+
+def check(cs, ctx, k):
+    P, perm = oracle.sort(k)
+    dk = cs.from_u64(k, ctx.device)
+    dperm = cs.sortKeys(ctx, dk)
+    assert np.array_equal(cs.u64(dk), P), "sorted keys"
+    assert np.array_equal(cs.u32(dperm), perm), "perm"
+
+
+def keys_with_runs(rng, run_lengths, low_mode="random"):
+    """Keys whose leading 45 bits form runs of the given lengths, shuffled."""
+    tops = rng.choice(1 << 40, size=len(run_lengths), replace=False).astype(np.uint64)
+    parts = []
+    for t, r in zip(tops, run_lengths):
+        if low_mode == "random":
+            lo = rng.integers(0, 1 << LOW, r, dtype=np.uint64)
+        elif low_mode == "few":                      # many equal whole keys inside the run
+            lo = rng.integers(0, 3, r, dtype=np.uint64)
+        else:                                        # all equal: only stability orders them
+            lo = np.zeros(r, dtype=np.uint64)
+        parts.append((t << np.uint64(LOW)) | lo)
+    k = np.concatenate(parts)
+    rng.shuffle(k)
+    return k
+
+
+@pytest.mark.parametrize("low_mode", ["random", "few", "equal"])
+def test_fixup_orders_short_runs(cs, ctx, low_mode):
+    rng = np.random.default_rng(11)
+    runs = list(rng.integers(1, 40, 3000)) + [MAX_RUN - 1, MAX_RUN, 200, 256]
+    check(cs, ctx, keys_with_runs(rng, runs, low_mode))
+
+
+@pytest.mark.parametrize("longest", [MAX_RUN, MAX_RUN + 1, MAX_RUN + 2, 300, 513, 5000])
+def test_run_length_boundary_and_gated_redo(cs, ctx, longest):
+    """Runs of exactly the limit stay on the fix-up; one element more takes the gated 7 passes."""
+    rng = np.random.default_rng(longest)
+    runs = [1] * 20000 + [longest] + list(rng.integers(1, 9, 2000))
+    check(cs, ctx, keys_with_runs(rng, runs))
+    # the context is reusable afterwards (flag and tickets are reset per call)
+    check(cs, ctx, keys_with_runs(rng, [1] * 9000 + [17, 3]))
+
+
+def test_runs_at_the_ends_and_across_blocks(cs, ctx):
+    rng = np.random.default_rng(3)
+    n_runs = 600
+    tops = np.sort(rng.choice(1 << 40, size=n_runs, replace=False).astype(np.uint64))
+    lens = rng.integers(100, MAX_RUN + 1, n_runs)            # long runs straddle every 256-thread block
+    lens[0] = MAX_RUN
+    lens[-1] = MAX_RUN
+    k = np.concatenate([(t << np.uint64(LOW)) | rng.integers(0, 1 << LOW, r, dtype=np.uint64)
+                        for t, r in zip(tops, lens)])
+    rng.shuffle(k)
+    check(cs, ctx, k)
+
+
+def test_one_giant_run_and_all_equal_keys(cs, ctx):
+    rng = np.random.default_rng(4)
+    k = (np.uint64(12345) << np.uint64(LOW)) | rng.integers(0, 1 << LOW, 50000, dtype=np.uint64)
+    check(cs, ctx, k)
+    check(cs, ctx, np.full(30001, 0x7FFFFFFFFFFFFFFF, dtype=np.uint64))
+    check(cs, ctx, np.zeros(777, dtype=np.uint64))
+
+
+def test_plain_mode_equals_default(cs, ctx):
+    rng = np.random.default_rng(8)
+    for n in (1, 257, 7680, 7681, 123457):
+        k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
+        ctx.setSortMode(cs.SORT_PLAIN)
+        check(cs, ctx, k)
+        ctx.setSortMode(cs.SORT_AUTO)
+        check(cs, ctx, k)
+    with pytest.raises(cs.CornerstoneError):
+        ctx.setSortMode(7)
+
+
+def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
+    """Deeply clustered particles (more than 257 per level-15 cell): the full build still matches
+    the oracle, through the gated redo the first time and through the plain passes afterwards."""
+    rng = np.random.default_rng(21)
+    n = 60000
+    x = np.concatenate([rng.random(n - 4000), 0.5 + 1e-7 * rng.random(4000)])
+    y = np.concatenate([rng.random(n - 4000), 0.5 + 1e-7 * rng.random(4000)])
+    z = np.concatenate([rng.random(n - 4000), 0.5 + 1e-7 * rng.random(4000)])
+    ref = oracle.full_build(x, y, z, 64)
+    d = [torch.from_numpy(a).cuda() for a in (x, y, z)]
+    for _ in range(3):
+        got = cs.buildOctree(ctx, d[0], d[1], d[2], 64)
+        assert np.array_equal(cs.u64(got["keys"]), ref["sortedKeys"])
+        assert np.array_equal(cs.u32(got["perm"]), ref["perm"])
+        assert np.array_equal(cs.u64(got["leaves"]), ref["leaves"])
+        assert np.array_equal(cs.u32(got["nodeCount"]), ref["nodeCount"])
+
+
+def test_workload_shapes(cs, ctx):
+    for gen in (lambda: W.blobs(300001, W.BASE_SEED + 4, nblobs=50), lambda: W.plummer(200000, W.BASE_SEED + 2)):
+        x, y, z = gen()
+        ref = oracle.full_build(x, y, z, 64)
+        check(cs, ctx, ref["keys"])
+
+
+def test_unaligned_arrays(cs, ctx):
+    """keys only 8-byte aligned / perm only 4-byte aligned."""
+    rng = np.random.default_rng(13)
+    k = rng.integers(0, 1 << 63, 40001, dtype=np.uint64)
+    k[::7] = k[1::7][: k[::7].size]
+    P, perm = oracle.sort(k[1:])
+    dk = cs.from_u64(k, ctx.device)[1:]
+    dperm = torch.empty(k.size + 1, dtype=torch.int32, device=ctx.device)[1:k.size]
+    cs.sortKeys(ctx, dk, dperm)
+    assert np.array_equal(cs.u64(dk), P) and np.array_equal(cs.u32(dperm), perm)
