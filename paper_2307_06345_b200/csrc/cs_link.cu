@@ -312,9 +312,11 @@ cs_status enqueueLink(cs_context* ctx, const u64* leaves, const u32* dNumLeaves,
     StageTimer t(ctx, CS_STAGE_LINK, s);
     DeviceCtrl* ctrl = ctx->ctrl;
     u32* tileHist = ctx->linkTileHist;                              // [tiles][kLinkBins]
-    const u32 persistentGrid = (u32)ctx->numSMs * 8;
+    // one tile per CTA where possible: the tiles differ in cost (subtree-end searches), so many small CTAs
+    // balance better than few persistent ones
+    const u32 gridCap = (u32)ctx->numSMs * 64;
     u32 grid = divUp((u64)leafBound, kLinkTile);
-    if (grid > persistentGrid) grid = persistentGrid;
+    if (grid > gridCap) grid = gridCap;
     if (grid == 0) grid = 1;
     linkCountKernel<<<grid, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkCountKernel");

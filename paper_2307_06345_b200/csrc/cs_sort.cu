@@ -343,41 +343,47 @@ __global__ void __launch_bounds__(kFixupBlock)
         const bool runL = i > 0 && ((kl ^ key) >> LOW) == 0, runR = i + 1 < n && ((kr ^ key) >> LOW) == 0;
         u32 dst = i;
         if (runL || runR) {                                 // not alone in its run: count what precedes it
-            // the input is ordered by the leading bits, so the run is where runLo <= k < runHi
+            // The input is ordered by the leading bits, so the run [a, e) is where runLo <= k < runHi.  Its
+            // ends are found by doubling steps + bisection (all lanes of a run walk the same addresses).
             const u64 runLo = key & ~((1ull << LOW) - 1), runHi = runLo + (1ull << LOW);
+            u32 a = i, e = i + 1;
+            if (runL) {
+                u32 d = 2;                                  // keysIn[i - 1] is inside
+                while (d <= i && d <= 2 * kFixupMaxRun && keysIn[i - d] >= runLo) d *= 2;
+                u32 lo = d <= i ? i - d + 1 : 0, hi = i - d / 2;   // keysIn[hi] inside; first inside index in [lo, hi]
+                if (d <= i && d > 2 * kFixupMaxRun) lo = hi;      // beyond the limit anyway
+                while (lo < hi) {
+                    const u32 mid = lo + ((hi - lo) >> 1);
+                    if (keysIn[mid] >= runLo) hi = mid;
+                    else lo = mid + 1;
+                }
+                a = lo;
+            }
+            if (runR) {
+                u32 d = 2;                                  // keysIn[i + 1] is inside
+                while (d < n - i && d <= 2 * kFixupMaxRun && keysIn[i + d] < runHi) d *= 2;
+                u32 lo = i + d / 2 + 1, hi = d < n - i ? i + d : n;   // keysIn[lo - 1] inside; first outside index in [lo, hi]
+                if (d < n - i && d > 2 * kFixupMaxRun) hi = lo;
+                while (lo < hi) {
+                    const u32 mid = lo + ((hi - lo) >> 1);
+                    if (keysIn[mid] < runHi) lo = mid + 1;
+                    else hi = mid;
+                }
+                e = lo;
+            }
+            if (i - a > kFixupMaxRun || e - i - 1 > kFixupMaxRun) {   // longer than the limit: the gated passes redo the sort
+                *reinterpret_cast<volatile u32*>(redo) = 1u;
+                return;
+            }
+            // inside the run the leading bits agree, so the low words order it; ties keep their input order
+            const u32* lowWord = reinterpret_cast<const u32*>(keysIn);
+            const u32 mine = (u32)key;
             u32 before = 0;
-            const u64* p = keysIn + i;                      // walks to the start of the run
-            if (runL) {                                     // to the left: smaller or equal low bits precede
-                const u64* stop = keysIn + (i > kFixupMaxRun ? i - kFixupMaxRun : 0);   // at most kFixupMaxRun to the left
-                before += kl <= key;
-                --p;
-                while (p > stop) {
-                    const u64 k = p[-1];
-                    if (k < runLo) break;
-                    before += k <= key;
-                    --p;
-                }
-                if (p == stop && p > keysIn && p[-1] >= runLo) {   // longer than the limit: the gated passes redo the sort
-                    *reinterpret_cast<volatile u32*>(redo) = 1u;
-                    return;
-                }
+            for (u32 m = a; m < e; ++m) {
+                const u32 w = lowWord[2 * (size_t)m];
+                before += (w < mine) || (w == mine && m < i);
             }
-            if (runR) {                                     // to the right: strictly smaller low bits precede
-                const u64* q = keysIn + i + 2;
-                const u64* stop = keysIn + (n - i > kFixupMaxRun + 1 ? i + kFixupMaxRun + 1 : n);   // and to the right
-                before += kr < key;
-                while (q < stop) {
-                    const u64 k = *q;
-                    if (k >= runHi) break;
-                    before += k < key;
-                    ++q;
-                }
-                if (q == stop && q < keysIn + n && *q < runHi) {
-                    *reinterpret_cast<volatile u32*>(redo) = 1u;
-                    return;
-                }
-            }
-            dst = (u32)(p - keysIn) + before;
+            dst = a + before;
         }
         keysOut[dst] = key;
         valsOut[dst] = val;
