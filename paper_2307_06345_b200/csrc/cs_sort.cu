@@ -161,21 +161,26 @@ __device__ __forceinline__ u32 matchDigit(u32 d)
     return a & ~o;
 }
 
+// keys of one tile: warp-striped, so that (warp, item, lane) order == memory order (stability); pads sort last
+template <bool FULL>
+__device__ __forceinline__ void tileLoadKeys(u64 (&key)[kSortItems], const u64* __restrict__ keysIn, u32 tile, u32 valid)
+{
+    const u32 warpOff = (threadIdx.x >> 5) * (32 * kSortItems) + laneId();
+    const u64* src = keysIn + (u64)tile * kSortTile + warpOff;
+#pragma unroll
+    for (int j = 0; j < kSortItems; ++j)
+        key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU64(src + j * 32) : ~0ull;
+}
+
+// From the loaded keys to the tile staged in digit order in shared memory, with globalBase[] set
+// (ranking, per-digit prefixes, scatter of keys and values, look-back).  Ends with a barrier.
 template <int SHIFT, bool FIRST, bool FULL>
-__device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict__ keysIn, const u32* __restrict__ valsIn,
-                                             u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
-                                             const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
+__device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], const u32* __restrict__ valsIn, u32 tile,
+                                          u32 valid, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
     const u64 base = (u64)tile * kSortTile;
-
-    // ---- load: warp-striped, so that (warp, item, lane) order == memory order (stability) ----
-    u64 key[kSortItems];
     const u32 warpOff = warp * (32 * kSortItems) + lane;
-    const u64* src = keysIn + base + warpOff;
-#pragma unroll
-    for (int j = 0; j < kSortItems; ++j)
-        key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU64(src + j * 32) : ~0ull;   // pads sort last
 
     // ---- rank inside the warp: every peer reads the warp's running count of its digit (a
     // shared-memory broadcast) and the lowest peer bumps it once ------------------------------------
@@ -254,7 +259,13 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
     }
     __syncthreads();
 
-    // ---- write out: consecutive threads -> consecutive slots of a digit's run ----------------------
+}
+
+// write out: consecutive threads -> consecutive slots of a digit's run
+template <int SHIFT, bool FULL>
+__device__ __forceinline__ void tileWriteOut(const SortSmem& sm, u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 valid)
+{
+    const u32 tid = threadIdx.x;
 #pragma unroll
     for (int k = 0; k < kSortItems; ++k) {
         const u32 i = tid + k * kSortBlock;
@@ -265,6 +276,17 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
             valsOut[dst] = sm.vals[i];
         }
     }
+}
+
+template <int SHIFT, bool FIRST, bool FULL>
+__device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict__ keysIn, const u32* __restrict__ valsIn,
+                                             u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
+                                             const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
+{
+    u64 key[kSortItems];
+    tileLoadKeys<FULL>(key, keysIn, tile, valid);
+    tileStage<SHIFT, FIRST, FULL>(sm, key, valsIn, tile, valid, digitBase, lookback, epoch);
+    tileWriteOut<SHIFT, FULL>(sm, keysOut, valsOut, valid);
 }
 
 // One tile per CTA (grid = tiles): the passes of the default path and of cs_setSortMode(PLAIN).
