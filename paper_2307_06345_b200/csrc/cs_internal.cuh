@@ -30,7 +30,7 @@ constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits
 #define CS_SORT_BLOCK 512
 #endif
 #ifndef CS_SORT_ITEMS
-#define CS_SORT_ITEMS 15
+#define CS_SORT_ITEMS 13
 #endif
 #ifndef CS_SORT_MINBLOCKS
 #define CS_SORT_MINBLOCKS 2
@@ -38,7 +38,7 @@ constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits
 constexpr int kSortBlock = CS_SORT_BLOCK;
 constexpr int kSortMinBlocks = CS_SORT_MINBLOCKS;   // resident CTAs per SM the radix pass is compiled for
 constexpr int kSortItems = CS_SORT_ITEMS;
-constexpr int kSortTile = kSortBlock * kSortItems;   // 7680 keys per tile
+constexpr int kSortTile = kSortBlock * kSortItems;   // 6656 keys per tile
 
 // ---- leaf refinement / link geometry -------------------------------------------------
 constexpr int kLeafBlock = 256;

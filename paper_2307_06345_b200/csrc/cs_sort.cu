@@ -108,7 +108,7 @@ struct SortSmem {
 };
 
 #ifndef CS_SORT_LOOKBATCH
-#define CS_SORT_LOOKBATCH 8
+#define CS_SORT_LOOKBATCH 4
 #endif
 constexpr int kLookBatch = CS_SORT_LOOKBATCH;   // predecessors fetched per look-back round trip
 

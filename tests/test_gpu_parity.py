@@ -88,10 +88,10 @@ def fused(cs, ctx, x, y, z, bucket, ref):
 
 
 # ------------------------------------------------------------------------------------------------
-# small cases spanning several tiles and ragged tails (sort tile = 7680, leaf tile = 1024)
+# small cases spanning several tiles and ragged tails (sort tile = 6656, leaf tile = 1024)
 CASES = [
-    ("uniform", 1, 64), ("uniform", 2, 1), ("uniform", 7679, 16), ("uniform", 7680, 16), ("uniform", 7681, 16),
-    ("uniform", 3 * 7680 + 17, 8), ("uniform", 65536, 64), ("plummer", 100003, 64), ("plummer", 250000, 16),
+    ("uniform", 1, 64), ("uniform", 2, 1), ("uniform", 6655, 16), ("uniform", 6656, 16), ("uniform", 6657, 16),
+    ("uniform", 3 * 6656 + 17, 8), ("uniform", 65536, 64), ("plummer", 100003, 64), ("plummer", 250000, 16),
     ("blobs", 300001, 64), ("blobs", 131072, 1), ("gaussian", 200000, 32),
 ]
 
@@ -136,7 +136,7 @@ def test_unaligned_and_odd_inputs_take_the_scalar_path(cs, ctx):
 
 def test_sort_random_64bit_patterns_and_duplicates(cs, ctx):
     rng = np.random.default_rng(5)
-    for n in (1, 31, 33, 5000, 7680 * 2, 100001):
+    for n in (1, 31, 33, 5000, 6656 * 2, 100001):
         k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
         if n > 100:
             k[rng.integers(0, n, n // 3)] = k[rng.integers(0, n, n // 3)]     # many duplicates
