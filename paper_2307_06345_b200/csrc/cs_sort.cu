@@ -200,6 +200,17 @@ __device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], 
         __syncwarp();
         rankPk[j >> 1] |= (prev + lower) << ((j & 1) * 16);
     }
+    // values: requested now, used after the key scatter (their latency hides behind the per-digit phase);
+    // the first pass synthesises the identity permutation instead of reading it
+    u32 val[kSortItems];
+    {
+        const u32* vsrc = valsIn + base + warpOff;
+#pragma unroll
+        for (int j = 0; j < kSortItems; ++j) {
+            if (FIRST) val[j] = (u32)base + warpOff + j * 32;
+            else val[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU32(vsrc + j * 32) : 0u;
+        }
+    }
     __syncthreads();
 
     // ---- per digit (one thread each): tile count, tile-local start, first slot of every warp ------
@@ -233,15 +244,6 @@ __device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], 
         sm.keys[pos] = key[j];
         if (j & 1) rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFFu) | (pos << 16);
         else rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFF0000u) | pos;
-    }
-    // values: pass 0 synthesises the identity permutation instead of reading it
-    asm volatile("" ::: "memory");        // keep the value loads behind the key scatter (register pressure)
-    u32 val[kSortItems];
-    const u32* vsrc = valsIn + base + warpOff;
-#pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
-        if (FIRST) val[j] = (u32)base + warpOff + j * 32;
-        else val[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU32(vsrc + j * 32) : 0u;
     }
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) sm.vals[(rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu] = val[j];
