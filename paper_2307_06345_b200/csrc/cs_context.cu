@@ -40,7 +40,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     Layout L{};
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = alignUp(o + bytes); return at; };
-    const size_t sortTiles = (maxParticles + kSortTile - 1) / kSortTile + 1;
+    const size_t sortTiles = (maxParticles + kSortLastTile - 1) / kSortLastTile + 1;   // the smaller of the two tile sizes
     const size_t dirTiles = (maxParticles >> kDirectTileLog2) + 2;          // one-pass leaf build: positions 0 .. n
     size_t leafTiles = ((size_t)maxLeaves + 1 + 1023) / 1024 + 1;          // covers kLeafTile, kScanTile >= 1024
     if (leafTiles < dirTiles / 1024 + 2) leafTiles = dirTiles / 1024 + 2;  // the scan of the one-pass build's tile totals

@@ -39,6 +39,7 @@ constexpr int kSortBlock = CS_SORT_BLOCK;
 constexpr int kSortMinBlocks = CS_SORT_MINBLOCKS;   // resident CTAs per SM the radix pass is compiled for
 constexpr int kSortItems = CS_SORT_ITEMS;
 constexpr int kSortTile = kSortBlock * kSortItems;   // 6656 keys per tile
+constexpr int kSortLastTile = kSortTile - 320;       // nominal tile of the pass that also orders the low bits (cs_sort.cu)
 
 // ---- leaf refinement / link geometry -------------------------------------------------
 constexpr int kLeafBlock = 256;

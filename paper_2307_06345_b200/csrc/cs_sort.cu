@@ -11,14 +11,15 @@
 //
 // Short cut: SFC keys of N particles are all but decided by their leading
 // digits.  The default path sorts by the 5 leading digits (bits 18..62) with 5 passes and then
-// orders the low 18 bits inside every run of equal leading digits directly (sortFixupKernel:
-// rank = elements of the run that must precede, counted by scanning the run, O(run length) per
-// element).  A run longer than kFixupMaxRun + 1 raises a device flag instead; the 7 plain passes
-// that follow in the stream are gated on that flag and redo the sort from the (still complete)
-// output of pass 5.  Either way the result is the stable sort: parity does not depend on the path.
+// orders the low 18 bits inside every run of equal leading digits directly, in the shared-memory
+// stage of the fifth pass (onesweepLastKernel: rank = elements of the run that must precede,
+// counted by scanning the run, O(run length) per element).  A run longer than kFixupMaxRun + 1
+// raises a device flag instead; the 7 plain passes that follow in the stream are gated on that
+// flag and redo the sort from the (still complete) input of the fifth pass.  Either way the
+// result is the stable sort: parity does not depend on the path.
 //
 // Model bytes per particle (SURVEY 8d, 8 passes of 8 bits): 196; moved by the default path:
-// pass 0 (8 read, 12 written) + 4 x 24 + fix-up 24 = 140 (histograms come from the key kernel).
+// pass 0 (8 read, 12 written) + 4 x 24 = 116 (histograms come from the key kernel).
 #include "cs_device.cuh"
 
 namespace cs {
@@ -163,10 +164,10 @@ __device__ __forceinline__ u32 matchDigit(u32 d)
 
 // keys of one tile: warp-striped, so that (warp, item, lane) order == memory order (stability); pads sort last
 template <bool FULL>
-__device__ __forceinline__ void tileLoadKeys(u64 (&key)[kSortItems], const u64* __restrict__ keysIn, u32 tile, u32 valid)
+__device__ __forceinline__ void tileLoadKeys(u64 (&key)[kSortItems], const u64* __restrict__ keysIn, u64 base, u32 valid)
 {
     const u32 warpOff = (threadIdx.x >> 5) * (32 * kSortItems) + laneId();
-    const u64* src = keysIn + (u64)tile * kSortTile + warpOff;
+    const u64* src = keysIn + base + warpOff;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j)
         key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU64(src + j * 32) : ~0ull;
@@ -176,10 +177,9 @@ __device__ __forceinline__ void tileLoadKeys(u64 (&key)[kSortItems], const u64* 
 // (ranking, per-digit prefixes, scatter of keys and values, look-back).  Ends with a barrier.
 template <int SHIFT, bool FIRST, bool FULL>
 __device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], const u32* __restrict__ valsIn, u32 tile,
-                                          u32 valid, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
+                                          u64 base, u32 valid, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
-    const u64 base = (u64)tile * kSortTile;
     const u32 warpOff = warp * (32 * kSortItems) + lane;
 
     // ---- rank inside the warp: every peer reads the warp's running count of its digit (a
@@ -286,8 +286,9 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
                                              const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
     u64 key[kSortItems];
-    tileLoadKeys<FULL>(key, keysIn, tile, valid);
-    tileStage<SHIFT, FIRST, FULL>(sm, key, valsIn, tile, valid, digitBase, lookback, epoch);
+    const u64 base = (u64)tile * kSortTile;
+    tileLoadKeys<FULL>(key, keysIn, base, valid);
+    tileStage<SHIFT, FIRST, FULL>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
     tileWriteOut<SHIFT, FULL>(sm, keysOut, valsOut, valid);
 }
 
@@ -312,6 +313,171 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
         onesweepTile<SHIFT, FIRST, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
     else
         onesweepTile<SHIFT, FIRST, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
+}
+
+// ---- last pass of the default path: radix pass over the top digit + fix-up of the low bits ---------------
+// Input: stably sorted by bits LOW..53.  After this pass's stable split by the top digit the elements
+// are sorted by all bits >= LOW; what is left is the order of the low bits inside every run of equal
+// leading bits.  The elements of such a run are adjacent in the input's order within one top digit, so if
+// no run straddles a tile, every run lies contiguous in the tile staged in shared memory and can be
+// ordered there, on the way out.  Hence the tiles are cut at run boundaries: nominal boundaries every
+// kLastTile elements, each moved back to the start of the run it falls into (at most kFixupMaxRun
+// elements).  An element of a run goes to runStart + (run elements with smaller low bits) + (earlier run
+// elements with equal low bits).  A run longer than kFixupMaxRun + 1 raises *redo instead (the gated passes
+// that follow redo the sort from this pass's input).
+constexpr u32 kFixupMaxRun = 256;
+constexpr u32 kLastTile = kSortLastTile;                  // nominal tile: room for a boundary run, multiple of 64
+static_assert(kLastTile % 64 == 0 && kLastTile > 2 * kFixupMaxRun, "nominal tile of the last pass");
+
+// start of the run (equal bits >= LOW) that element `b` falls into, found by one warp; 0 < b < n.
+// *tooLong is set if the run starts more than kFixupMaxRun elements before b (then b itself is returned).
+template <int LOW>
+__device__ __forceinline__ u32 runStartBefore(const u64* __restrict__ keysIn, u32 b, bool* tooLong)
+{
+    const u32 lane = laneId();
+    const u64 kb = keysIn[b];
+    u32 back = 0;
+    for (;;) {
+        const u32 off = back + lane + 1;                    // element b - off
+        const bool same = off <= b && ((keysIn[b - (off <= b ? off : 0)] ^ kb) >> LOW) == 0;
+        const u32 m = __ballot_sync(kFull, same);
+        const u32 c = m == kFull ? 32u : (u32)__ffs((int)~m) - 1u;   // lanes 0..c-1 are in the run
+        back += c;
+        if (c < 32) break;
+        if (back > kFixupMaxRun) break;
+    }
+    if (back > kFixupMaxRun) {
+        *tooLong = true;
+        return b;
+    }
+    return b - back;
+}
+
+// Write out with the fix-up, warp-cooperative and free of divergence.  The staged tile is ordered by the
+// bits >= LOW, so a run (equal bits >= LOW) is a contiguous range of slots; "head" = first slot of a run.
+// Every warp takes a range of slots that starts and ends at heads and walks it in windows of up to 32
+// slots that again start at a head and hold whole runs only (the last, unfinished run of a window opens
+// the next one).  Inside a window a lane learns its run [rs, re) from the ballot of the head flags and
+// counts the run members that must precede it from shuffled low words: d = 1 .. longest run - 1 steps for
+// the whole window.  A run of more than 32 slots is ranked against all of its members read from shared
+// memory.  Slot of an element = run start + (members with smaller low bits) + (earlier members with
+// equal low bits); it is stored straight to its place in the output.
+template <int SHIFT, int LOW>
+__device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u64* __restrict__ keysOut, u32* __restrict__ valsOut,
+                                                  u32 valid, u32* redo)
+{
+    const u32 lane = laneId(), warp = threadIdx.x >> 5;
+    const u64* keys = sm.keys;
+    const u32* low = reinterpret_cast<const u32*>(sm.keys);
+    auto same = [](u64 a, u64 b) { return ((a ^ b) >> LOW) == 0; };
+    auto emit = [&](u32 q, u64 kk, u32 slot) {
+        const u32 dst = sm.globalBase[digitOf(kk, SHIFT)] + slot;
+        keysOut[dst] = kk;
+        valsOut[dst] = sm.vals[q];
+    };
+    // first head at or after slot x; `valid` counts as one
+    auto firstHeadFrom = [&](u32 x) -> u32 {
+        if (x == 0) return 0u;
+        for (u32 p = x;; p += 32) {
+            if (p >= valid) return valid;
+            const u32 q = p + lane;
+            const bool head = q >= valid || !same(keys[q - 1], keys[q]);
+            const u32 H = __ballot_sync(kFull, head);
+            if (H) return p + (u32)__ffs((int)H) - 1u;
+        }
+    };
+    const u32 share = ((valid + kSortWarps - 1) / kSortWarps + 31u) & ~31u;
+    u32 p = firstHeadFrom(warp * share);
+    const u32 end = firstHeadFrom((warp + 1) * share);     // the last warp's share ends at or beyond `valid`
+    bool tooLong = false;
+    while (p < end) {
+        const u32 q = p + lane;
+        const bool in = q < end;
+        const u64 kk = keys[in ? q : p];
+        const bool head = !in || lane == 0 || !same(keys[(in && lane != 0) ? q - 1 : p], kk);
+        const u32 H = __ballot_sync(kFull, head);
+        const bool nextHead = p + 32 >= end || !same(keys[p + 31], keys[p + 32]);   // warp-uniform
+        const u32 mine = (u32)kk;
+        if (H == 1u && !nextHead) {
+            // ---- one run of more than 32 slots: find its end, rank every member against all of them ----
+            u32 e = p + 32;
+            for (;;) {
+                const u32 q2 = e + lane;
+                const u32 m = __ballot_sync(kFull, q2 < end && same(keys[q2 < end ? q2 : p], kk));
+                const u32 c = m == kFull ? 32u : (u32)__ffs((int)~m) - 1u;
+                e += c;
+                if (c < 32 || e - p > kFixupMaxRun + 1) break;
+            }
+            if (e - p > kFixupMaxRun + 1) tooLong = true;   // beyond the limit: the gated passes redo the sort
+            else {
+                for (u32 c0 = p; c0 < e; c0 += 32) {
+                    const u32 qc = c0 + lane;
+                    const bool act = qc < e;
+                    const u64 kc = keys[act ? qc : p];
+                    const u32 mc = (u32)kc;
+                    u32 before = 0;
+                    for (u32 m = p; m < e; ++m) {
+                        const u32 w = low[2 * m];
+                        before += ((w < mc) || (w == mc && m < qc)) ? 1u : 0u;
+                    }
+                    if (act) emit(qc, kc, p + before);
+                }
+            }
+            p = e;
+            continue;
+        }
+        // ---- whole runs inside the window [p, p + wend) -------------------------------------------------------
+        const u32 wend = nextHead ? 32u : 31u - (u32)__clz((int)H);   // the unfinished last run opens the next window
+        const bool act = in && lane < wend;
+        const u32 rs = 31u - (u32)__clz((int)(H & (0xFFFFFFFFu >> (31u - lane))));   // head at or below this lane
+        const u32 above = (H >> 1) >> lane;                                            // heads above it, bit 0 <-> lane + 1
+        u32 re = above ? lane + (u32)__ffs((int)above) : 32u;
+        re = re < wend ? re : wend;
+        const u32 longest = __reduce_max_sync(kFull, act ? re - rs : 1u);
+        u32 before = 0;
+        for (u32 d = 1; d < longest; ++d) {
+            const u32 up = __shfl_up_sync(kFull, mine, d), dn = __shfl_down_sync(kFull, mine, d);
+            before += (lane >= rs + d && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
+            before += (lane + d < re && dn < mine) ? 1u : 0u;       // strictly smaller ones to the right
+        }
+        if (act) emit(q, kk, p + rs + before);
+        p += wend;
+    }
+    if (tooLong) *reinterpret_cast<volatile u32*>(redo) = 1u;
+}
+
+template <int SHIFT, int LOW>
+__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
+    onesweepLastKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
+                       u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase, u32* ticket, u64* lookback,
+                       u32 epoch, u32* redo)
+{
+    extern __shared__ __align__(16) unsigned char smemRaw[];
+    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    __shared__ u32 sCut[2];
+    const u32 tid = threadIdx.x;
+    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
+    for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
+    __syncthreads();
+    const u32 tile = sm.tile;
+    if (tid < 64) {                                         // warps 0 and 1: where this tile starts and ends
+        const u32 w = tid >> 5;
+        const u64 nominal = (u64)(tile + w) * kLastTile;
+        u32 cut = nominal < n ? (u32)nominal : n;
+        bool tooLong = false;
+        if (cut > 0 && cut < n) cut = runStartBefore<LOW>(keysIn, cut, &tooLong);
+        if ((tid & 31u) == 0) {
+            sCut[w] = cut;
+            if (tooLong) *reinterpret_cast<volatile u32*>(redo) = 1u;
+        }
+    }
+    __syncthreads();
+    const u32 base = sCut[0], valid = sCut[1] - sCut[0];
+    u64 key[kSortItems];
+    tileLoadKeys<false>(key, keysIn, base, valid);
+    tileStage<SHIFT, false, false>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
+    tileWriteOutFixup<SHIFT, LOW>(sm, keysOut, valsOut, valid, redo);
 }
 
 // The redo passes behind the fix-up: persistent CTAs that leave at once unless *gate != 0, so that
@@ -344,85 +510,13 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     }
 }
 
-// ---- fix-up of the low bits inside runs of equal leading digits ----------------------------------------
-// In: elements stably sorted by key >> LOW.  Out: stably sorted by the whole key.  An element moves
-// inside its run only: to runStart + (elements of the run with smaller low bits) + (elements of the run
-// before it with equal low bits).  Neighbours are read through L1 (the lines were just loaded by the
-// adjacent threads).  Runs longer than kFixupMaxRun + 1: *redo = 1 and the kernel gives up.
-constexpr int kFixupBlock = 256;
-constexpr u32 kFixupMaxRun = 256;
-
-template <int LOW>
-__global__ void __launch_bounds__(kFixupBlock)
-    sortFixupKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
-                    u32* __restrict__ valsOut, u32 n, u32* redo)
-{
-    const u32 stride = gridDim.x * kFixupBlock;
-    u32 it = 0;
-    for (u32 i = blockIdx.x * kFixupBlock + threadIdx.x; i < n; i += stride, ++it) {
-        const u64 key = keysIn[i];
-        const u32 val = ldStreamU32(valsIn + i);
-        // same run <=> the keys agree above bit LOW; inside a run the key order is the order of the low bits
-        const u64 kl = keysIn[i > 0 ? i - 1 : 0], kr = keysIn[i + 1 < n ? i + 1 : i];
-        const bool runL = i > 0 && ((kl ^ key) >> LOW) == 0, runR = i + 1 < n && ((kr ^ key) >> LOW) == 0;
-        u32 dst = i;
-        if (runL || runR) {                                 // not alone in its run: count what precedes it
-            // The input is ordered by the leading bits, so the run [a, e) is where runLo <= k < runHi.  Its
-            // ends are found by doubling steps + bisection (all lanes of a run walk the same addresses).
-            const u64 runLo = key & ~((1ull << LOW) - 1), runHi = runLo + (1ull << LOW);
-            u32 a = i, e = i + 1;
-            if (runL) {
-                u32 d = 2;                                  // keysIn[i - 1] is inside
-                while (d <= i && d <= 2 * kFixupMaxRun && keysIn[i - d] >= runLo) d *= 2;
-                u32 lo = d <= i ? i - d + 1 : 0, hi = i - d / 2;   // keysIn[hi] inside; first inside index in [lo, hi]
-                if (d <= i && d > 2 * kFixupMaxRun) lo = hi;      // beyond the limit anyway
-                while (lo < hi) {
-                    const u32 mid = lo + ((hi - lo) >> 1);
-                    if (keysIn[mid] >= runLo) hi = mid;
-                    else lo = mid + 1;
-                }
-                a = lo;
-            }
-            if (runR) {
-                u32 d = 2;                                  // keysIn[i + 1] is inside
-                while (d < n - i && d <= 2 * kFixupMaxRun && keysIn[i + d] < runHi) d *= 2;
-                u32 lo = i + d / 2 + 1, hi = d < n - i ? i + d : n;   // keysIn[lo - 1] inside; first outside index in [lo, hi]
-                if (d < n - i && d > 2 * kFixupMaxRun) hi = lo;
-                while (lo < hi) {
-                    const u32 mid = lo + ((hi - lo) >> 1);
-                    if (keysIn[mid] < runHi) lo = mid + 1;
-                    else hi = mid;
-                }
-                e = lo;
-            }
-            if (i - a > kFixupMaxRun || e - i - 1 > kFixupMaxRun) {   // longer than the limit: the gated passes redo the sort
-                *reinterpret_cast<volatile u32*>(redo) = 1u;
-                return;
-            }
-            // inside the run the leading bits agree, so the low words order it; ties keep their input order
-            const u32* lowWord = reinterpret_cast<const u32*>(keysIn);
-            const u32 mine = (u32)key;
-            u32 before = 0;
-            for (u32 m = a; m < e; ++m) {
-                const u32 w = lowWord[2 * (size_t)m];
-                before += (w < mine) || (w == mine && m < i);
-            }
-            dst = a + before;
-        }
-        keysOut[dst] = key;
-        valsOut[dst] = val;
-        // now and then: no point in finishing once another thread has given up
-        if ((it & 15u) == 15u && *reinterpret_cast<const volatile u32*>(redo)) return;
-    }
-}
-
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
 {
     CS_CUDA(ctx, cudaMemsetAsync(ctx->sortHist, 0, (kSortPasses * kRadix + 64) * sizeof(u32), s));
     return CS_OK;
 }
 
-constexpr int kTopPasses = 5;                               // digits 2..6 (bits 18..62) before the fix-up
+constexpr int kTopPasses = 5;                               // digits 2..6 (bits 18..62); the fifth also orders the low bits
 constexpr int kFixupLow = (kSortPasses - kTopPasses) * kRadixBits;
 static_assert(kSortPasses == 7 && kRadixBits == 9, "the pass plan below is written for 7 digits of 9 bits");
 
@@ -473,10 +567,10 @@ static cs_status launchGatedPass(cs_context* ctx, PassPlan& pl, const u32* gate,
     return CS_OK;
 }
 
-// Where the first radix pass reads the unsorted keys.  The passes alternate between the caller's
-// arrays and the workspace's: the default path (5 passes + fix-up, and 7 more if redone) ends where
-// it started; the plain 7 passes end in the other pair.
-u64* sortSource(cs_context* ctx, u64* keys) { return ctx->sortPlain ? ctx->keysAlt : keys; }
+// Where the first radix pass reads the unsorted keys.  The passes alternate between the workspace's
+// arrays and the caller's; both plans (5 passes, and 7 more if redone; 7 plain passes) run an odd number
+// of passes over the data, so they start in the workspace and end in the caller's arrays.
+u64* sortSource(cs_context* ctx, u64*) { return ctx->keysAlt; }
 
 // fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
 // (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
@@ -517,27 +611,29 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         CS_TRY((launchPass<45, false>(ctx, pl, s)));
         return launchPass<54, false>(ctx, pl, s);
     }
-    {   // leading digits, most of the order
+    u32* redo = ctx->sortTickets + kSortRedoSlot;
+    {   // leading digits; the last of these passes also orders the low bits inside the runs
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
         CS_TRY((launchPass<18, true>(ctx, pl, s)));
         CS_TRY((launchPass<27, false>(ctx, pl, s)));
         CS_TRY((launchPass<36, false>(ctx, pl, s)));
         CS_TRY((launchPass<45, false>(ctx, pl, s)));
-        CS_TRY((launchPass<54, false>(ctx, pl, s)));
-    }
-    StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
-    // low bits inside the runs; out of place, so the input stays intact for a redo
-    u32* redo = ctx->sortTickets + kSortRedoSlot;
-    {
-        u32 grid = divUp(n, kFixupBlock);
-        const u32 cap = (u32)ctx->numSMs * 32;
-        if (grid > cap) grid = cap;
+        static bool attrSet = false;
+        if (!attrSet) {
+            CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)sizeof(SortSmem)));
+            attrSet = true;
+        }
+        const u32 epoch = nextEpoch(ctx, s);
         const int in = pl.cur, out = in ^ 1;
-        sortFixupKernel<kFixupLow><<<grid, kFixupBlock, 0, s>>>(pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, redo);
-        CS_LAUNCH_CHECK(ctx, "sortFixupKernel");
+        onesweepLastKernel<54, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
+            pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + 6 * kRadix, ctx->sortTickets + pl.ticketSlot++,
+            ctx->sortLookback, epoch, redo);
+        CS_LAUNCH_CHECK(ctx, "onesweepLastKernel");
     }
-    // gated redo from the output of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
-    // which is where the fix-up wrote
+    // gated redo from the input of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
+    // which is where the fifth pass wrote
+    StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     CS_TRY((launchGatedPass<0>(ctx, pl, redo, s)));
     CS_TRY((launchGatedPass<9>(ctx, pl, redo, s)));
     CS_TRY((launchGatedPass<18>(ctx, pl, redo, s)));
