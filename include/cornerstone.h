@@ -53,8 +53,8 @@ typedef enum cs_status {
 enum {
     CS_STAGE_BOX = 0, CS_STAGE_KEYS = 1, CS_STAGE_SORT = 2, CS_STAGE_LEAVES = 3, CS_STAGE_LINK = 4,
     CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6,
-    CS_STAGE_SORT_PASSES = 7,    /* the radix passes that always run: 5 (CS_SORT_AUTO) or 7 (CS_SORT_PLAIN) */
-    CS_STAGE_SORT_FIXUP = 8,     /* CS_SORT_AUTO: fix-up of the low 18 bits + the gated redo passes behind it */
+    CS_STAGE_SORT_PASSES = 7,    /* the plain radix passes: 4 (CS_SORT_AUTO) or 7 (CS_SORT_PLAIN) */
+    CS_STAGE_SORT_FIXUP = 8,     /* CS_SORT_AUTO: fifth pass, which also orders the low 18 bits, + the gated redo passes */
     CS_NUM_STAGES = 9
 };
 
@@ -110,8 +110,8 @@ cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, cons
 cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream);
 
 /* cs_setSortMode -- how cs_sortKeys / cs_buildOctree reach the (unique) stable order.
- *   CS_SORT_AUTO (default): 5 radix passes over the 5 leading 9-bit digits, then the low 18
- *   bits are ordered inside every run of equal leading digits; if some run is longer than
+ *   CS_SORT_AUTO (default): 5 radix passes over the 5 leading 9-bit digits; the fifth also
+ *   orders the low 18 bits inside every run of equal leading digits; if some run is longer than
  *   257 elements (particles deeper than octree level 15 in bulk) the 7 plain passes are run
  *   behind it instead, decided on the device with no host round trip.  cs_buildOctree
  *   remembers that outcome and uses the plain passes directly from then on.
@@ -119,7 +119,8 @@ cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t 
  *   The sorted keys and perm are identical in both modes.  Errors: INVALID_ARG. */
 enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1 };
 cs_status cs_setSortMode(cs_context* ctx, int mode);
-/* Radix passes the next sort on this context launches unconditionally: 5 or 7 (0 if ctx is NULL). */
+/* Plain radix passes of the next sort on this context (the ones CS_STAGE_SORT_PASSES times): 4 or 7
+ * (0 if ctx is NULL). */
 int cs_sortPasses(const cs_context* ctx);
 
 /* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1

@@ -180,7 +180,7 @@ class Context:
         self.check(lib().cs_setSortMode(self.handle, int(mode)))
 
     def sortPasses(self) -> int:
-        """Radix passes the next sort launches unconditionally (5 with the fix-up, 7 plain)."""
+        """Plain radix passes of the next sort (what the stage "sort_passes" times): 4, or 7 in SORT_PLAIN."""
         return int(lib().cs_sortPasses(self.handle))
 
     def stageTimes(self):

@@ -116,7 +116,7 @@ cs_status cs_setSortMode(cs_context* ctx, int mode)
     return CS_OK;
 }
 
-int cs_sortPasses(const cs_context* ctx) { return ctx ? (ctx->sortPlain ? 7 : 5) : 0; }
+int cs_sortPasses(const cs_context* ctx) { return ctx ? (ctx->sortPlain ? 7 : 4) : 0; }
 
 cs_status cs_setLeafMode(cs_context* ctx, int mode)
 {

@@ -355,72 +355,76 @@ __device__ __forceinline__ u32 runStartBefore(const u64* __restrict__ keysIn, u3
 
 // Write out with the fix-up, warp-cooperative and free of divergence.  The staged tile is ordered by the
 // bits >= LOW, so a run (equal bits >= LOW) is a contiguous range of slots; "head" = first slot of a run.
-// Every warp takes a range of slots that starts and ends at heads and walks it in windows of up to 32
-// slots that again start at a head and hold whole runs only (the last, unfinished run of a window opens
-// the next one).  Inside a window a lane learns its run [rs, re) from the ballot of the head flags and
-// counts the run members that must precede it from shuffled low words: d = 1 .. longest run - 1 steps for
-// the whole window.  A run of more than 32 slots is ranked against all of its members read from shared
-// memory.  Slot of an element = run start + (members with smaller low bits) + (earlier members with
-// equal low bits); it is stored straight to its place in the output.
+// First every thread marks the heads among its slots into a bit mask in shared memory (headMask, bit i of
+// the mask <-> slot i; slot `valid` counts as a head).  Then every warp takes a range of slots that starts
+// and ends at heads and walks it in windows of up to 32 slots that again start at a head and hold whole
+// runs only (the last, unfinished run of a window opens the next one).  Inside a window a lane learns its
+// run [rs, re) from the window's head bits and counts the run members that must precede it from shuffled
+// low words: d = 1 .. longest run - 1 steps for the whole window; a window of heads only goes straight
+// out.  A run of more than 32 slots is ranked against all of its members read from shared memory.  Slot of
+// an element = run start + (members with smaller low bits) + (earlier members with equal low bits); it is
+// stored straight to its place in the output.
+constexpr int kHeadWords = kSortTile / 32 + 2;
+
 template <int SHIFT, int LOW>
-__device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u64* __restrict__ keysOut, u32* __restrict__ valsOut,
-                                                  u32 valid, u32* redo)
+__device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headMask, u64* __restrict__ keysOut,
+                                                  u32* __restrict__ valsOut, u32 valid, u32* redo)
 {
-    const u32 lane = laneId(), warp = threadIdx.x >> 5;
+    const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
     const u64* keys = sm.keys;
     const u32* low = reinterpret_cast<const u32*>(sm.keys);
-    auto same = [](u64 a, u64 b) { return ((a ^ b) >> LOW) == 0; };
-    auto emit = [&](u32 q, u64 kk, u32 slot) {
+    // ---- head bits: consecutive threads <-> consecutive slots, one ballot per 32 slots -----------------
+#pragma unroll
+    for (int k = 0; k < kSortItems; ++k) {
+        const u32 i = tid + k * kSortBlock;
+        const bool head = i == 0 || i >= valid || ((keys[i - (i ? 1 : 0)] ^ keys[i]) >> LOW) != 0;
+        const u32 H = __ballot_sync(kFull, head);
+        if (lane == 0) headMask[i >> 5] = H;
+    }
+    if (tid < 2) headMask[kSortTile / 32 + tid] = kFull;
+    __syncthreads();
+    // the 32 head bits of slots x .. x + 31, and the position of the first head at or after x (x <= valid)
+    auto headBits = [&](u32 x) { return __funnelshift_r(headMask[x >> 5], headMask[(x >> 5) + 1], x & 31u); };
+    auto firstHeadFrom = [&](u32 x) -> u32 {
+        for (;; x += 32) {
+            const u32 H = headBits(x);
+            if (H) return x + (u32)__ffs((int)H) - 1u;
+        }
+    };
+    auto emit = [&](u32 q, u32 slot) {
+        const u64 kk = keys[q];
         const u32 dst = sm.globalBase[digitOf(kk, SHIFT)] + slot;
         keysOut[dst] = kk;
         valsOut[dst] = sm.vals[q];
     };
-    // first head at or after slot x; `valid` counts as one
-    auto firstHeadFrom = [&](u32 x) -> u32 {
-        if (x == 0) return 0u;
-        for (u32 p = x;; p += 32) {
-            if (p >= valid) return valid;
-            const u32 q = p + lane;
-            const bool head = q >= valid || !same(keys[q - 1], keys[q]);
-            const u32 H = __ballot_sync(kFull, head);
-            if (H) return p + (u32)__ffs((int)H) - 1u;
-        }
-    };
     const u32 share = ((valid + kSortWarps - 1) / kSortWarps + 31u) & ~31u;
-    u32 p = firstHeadFrom(warp * share);
-    const u32 end = firstHeadFrom((warp + 1) * share);     // the last warp's share ends at or beyond `valid`
+    const u32 start = warp * share < valid ? warp * share : valid, stop = (warp + 1) * share < valid ? (warp + 1) * share : valid;
+    u32 p = firstHeadFrom(start);
+    const u32 end = firstHeadFrom(stop);                    // slot `valid` is a head: both are <= valid
     bool tooLong = false;
     while (p < end) {
+        const u32 H = headBits(p);                          // bit 0 is set: p is a head
+        const bool nextHead = (headMask[(p + 32) >> 5] >> ((p + 32) & 31u)) & 1u;
         const u32 q = p + lane;
-        const bool in = q < end;
-        const u64 kk = keys[in ? q : p];
-        const bool head = !in || lane == 0 || !same(keys[(in && lane != 0) ? q - 1 : p], kk);
-        const u32 H = __ballot_sync(kFull, head);
-        const bool nextHead = p + 32 >= end || !same(keys[p + 31], keys[p + 32]);   // warp-uniform
-        const u32 mine = (u32)kk;
+        if (H == kFull && nextHead) {                       // no two slots share a run (slots from `end` on are heads too)
+            if (q < end) emit(q, q);
+            p += 32;
+            continue;
+        }
         if (H == 1u && !nextHead) {
             // ---- one run of more than 32 slots: find its end, rank every member against all of them ----
-            u32 e = p + 32;
-            for (;;) {
-                const u32 q2 = e + lane;
-                const u32 m = __ballot_sync(kFull, q2 < end && same(keys[q2 < end ? q2 : p], kk));
-                const u32 c = m == kFull ? 32u : (u32)__ffs((int)~m) - 1u;
-                e += c;
-                if (c < 32 || e - p > kFixupMaxRun + 1) break;
-            }
+            const u32 e = firstHeadFrom(p + 32);
             if (e - p > kFixupMaxRun + 1) tooLong = true;   // beyond the limit: the gated passes redo the sort
             else {
                 for (u32 c0 = p; c0 < e; c0 += 32) {
                     const u32 qc = c0 + lane;
-                    const bool act = qc < e;
-                    const u64 kc = keys[act ? qc : p];
-                    const u32 mc = (u32)kc;
+                    const u32 mc = low[2 * (qc < e ? qc : p)];
                     u32 before = 0;
                     for (u32 m = p; m < e; ++m) {
                         const u32 w = low[2 * m];
                         before += ((w < mc) || (w == mc && m < qc)) ? 1u : 0u;
                     }
-                    if (act) emit(qc, kc, p + before);
+                    if (qc < e) emit(qc, p + before);
                 }
             }
             p = e;
@@ -428,19 +432,21 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u64* __res
         }
         // ---- whole runs inside the window [p, p + wend) -------------------------------------------------------
         const u32 wend = nextHead ? 32u : 31u - (u32)__clz((int)H);   // the unfinished last run opens the next window
-        const bool act = in && lane < wend;
+        const bool act = q < end && lane < wend;
+        const u32 mine = low[2 * (q < end ? q : p)];
         const u32 rs = 31u - (u32)__clz((int)(H & (0xFFFFFFFFu >> (31u - lane))));   // head at or below this lane
         const u32 above = (H >> 1) >> lane;                                            // heads above it, bit 0 <-> lane + 1
         u32 re = above ? lane + (u32)__ffs((int)above) : 32u;
         re = re < wend ? re : wend;
+        const u32 roomL = lane - rs, roomR = re - 1u - lane;                           // run members to the left / right
         const u32 longest = __reduce_max_sync(kFull, act ? re - rs : 1u);
         u32 before = 0;
         for (u32 d = 1; d < longest; ++d) {
             const u32 up = __shfl_up_sync(kFull, mine, d), dn = __shfl_down_sync(kFull, mine, d);
-            before += (lane >= rs + d && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
-            before += (lane + d < re && dn < mine) ? 1u : 0u;       // strictly smaller ones to the right
+            before += (d <= roomL && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
+            before += (d <= roomR && dn < mine) ? 1u : 0u;      // strictly smaller ones to the right
         }
-        if (act) emit(q, kk, p + rs + before);
+        if (act) emit(q, p + rs + before);
         p += wend;
     }
     if (tooLong) *reinterpret_cast<volatile u32*>(redo) = 1u;
@@ -455,6 +461,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
     __shared__ u32 sCut[2];
+    __shared__ u32 sHeadMask[kHeadWords];
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
     u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
@@ -477,7 +484,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     u64 key[kSortItems];
     tileLoadKeys<false>(key, keysIn, base, valid);
     tileStage<SHIFT, false, false>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
-    tileWriteOutFixup<SHIFT, LOW>(sm, keysOut, valsOut, valid, redo);
+    tileWriteOutFixup<SHIFT, LOW>(sm, sHeadMask, keysOut, valsOut, valid, redo);
 }
 
 // The redo passes behind the fix-up: persistent CTAs that leave at once unless *gate != 0, so that
@@ -612,12 +619,15 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         return launchPass<54, false>(ctx, pl, s);
     }
     u32* redo = ctx->sortTickets + kSortRedoSlot;
-    {   // leading digits; the last of these passes also orders the low bits inside the runs
+    {   // leading digits
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
         CS_TRY((launchPass<18, true>(ctx, pl, s)));
         CS_TRY((launchPass<27, false>(ctx, pl, s)));
         CS_TRY((launchPass<36, false>(ctx, pl, s)));
         CS_TRY((launchPass<45, false>(ctx, pl, s)));
+    }
+    StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
+    {   // top digit; this pass also orders the low bits inside the runs
         static bool attrSet = false;
         if (!attrSet) {
             CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -633,7 +643,6 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     }
     // gated redo from the input of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
     // which is where the fifth pass wrote
-    StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     CS_TRY((launchGatedPass<0>(ctx, pl, redo, s)));
     CS_TRY((launchGatedPass<9>(ctx, pl, redo, s)));
     CS_TRY((launchGatedPass<18>(ctx, pl, redo, s)));
