@@ -151,6 +151,31 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def rank_workload(cfg, rank: int):
+    """Replicas only: every rank builds its own tree on its own particle set, so rank r
+    draws the same recipe from another seed."""
+    if rank == 0:
+        return cfg
+    import dataclasses
+    return dataclasses.replace(cfg, seed=cfg.seed + 7919 * rank)
+
+
+def max_over_ranks(value: float, world: int, device) -> float:
+    """Device (or host, for the gloo tests) time of the slowest rank."""
+    if world == 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_per_rank: int, world: int, ms_per_step: float) -> float:
+    """Mparticles/s of the whole job: the particles all ranks processed per step / the slowest rank's time."""
+    return n_per_rank * world / (ms_per_step * 1e-3) / 1e6
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -168,10 +193,7 @@ def run_ours(args):
     n = cfg.n if args.n is None else args.n
     bucket = cfg.bucket_sizes[-1]
     # replicas only: every rank builds its own tree on its own particle set
-    cfg_rank = cfg
-    if rank:
-        import dataclasses
-        cfg_rank = dataclasses.replace(cfg, seed=cfg.seed + 7919 * rank)
+    cfg_rank = rank_workload(cfg, rank)
     x, y, z = cfg_rank.generate(n)
     in_sum = None
     if rank == 0:
@@ -211,12 +233,9 @@ def run_ours(args):
         barrier()
     ms = ev0.elapsed_time(ev1)
     launches = ctx.stageTimes()["launches"] - launches0
-    if world > 1:
-        tmax = torch.tensor([ms], device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
+    ms = max_over_ranks(ms, world, "cuda")
     ms_per_step = ms / args.steps
-    value = n * world / (ms_per_step * 1e-3) / 1e6
+    value = whole_job_value(n, world, ms_per_step)
     stages = {k: v / args.steps for k, v in stages.items()}
 
     # ---- end to end: HOST buffers through cs_buildOctreeHost, copies inside the timed region ---
@@ -231,11 +250,8 @@ def run_ours(args):
             sz = cs.buildOctreeHost(ctx, hx, hy, hz, bucket, hb)
         torch.cuda.synchronize()
         dt = (time.perf_counter() - t0) / e2e_steps
-        if world > 1:
-            tmax = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-            dt = float(tmax.item())
-        e2e = {"value": n * world / dt / 1e6, "unit": UNIT, "h2d_bytes_per_step": 24 * n,
+        dt = max_over_ranks(dt, world, "cuda")
+        e2e = {"value": whole_job_value(n, world, dt * 1e3), "unit": UNIT, "h2d_bytes_per_step": 24 * n,
                "d2h_bytes_per_step": hb.bytes_back(n, sz["numLeaves"], sz["numNodes"]),
                "ms_per_step": dt * 1e3, "steps": e2e_steps}
 
