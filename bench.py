@@ -106,6 +106,18 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def _host_cpu():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"model": model, "nproc": os.cpu_count()}
+
+
 def _workload(name: str):
     from paper_2307_06345_b200 import workloads as W
     table = {"c1": W.CONFIGS[0], "c2": W.CONFIGS[1], "c3": W.CONFIGS[2], "c4": W.CONFIGS[3], "c5": W.CONFIGS[4]}
@@ -143,7 +155,7 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": cfg.name, "n_particles": cfg.n, "bucketSize": bucket,
                    "sample": f"first {sample_n} particles of the same recipe per step"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "host": _host_cpu(),
                          "sample": f"{sample_n} particles of {cfg.name}, full path, per step"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -278,12 +290,47 @@ def run_ours(args):
                   "frac_of_nominal_8TBs": model_bytes / (ms_per_step * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
                   "frac_of_measured_peak": model_bytes / (ms_per_step * 1e-3) / 1e9 / peak}
 
+    # per stage: fixed model bytes and compulsory bytes against the nominal and the measured peak
+    stage_bytes = {"box": (24, 24), "keys": (32, 32), "sort": (196, 20)}     # (model, compulsory) per particle
+    stages_roofline = {}
+    for k, (bm, bc) in stage_bytes.items():
+        t = stages[k] * 1e-3
+        if t > 0:
+            stages_roofline[k] = {"ms": stages[k], "mparticles_per_s": n / t / 1e6,
+                                  "model_frac_of_nominal_8TBs": bm * n / t / 1e9 / NOMINAL_HBM_GBS,
+                                  "compulsory_frac_of_nominal_8TBs": bc * n / t / 1e9 / NOMINAL_HBM_GBS,
+                                  "model_frac_of_measured_peak": bm * n / t / 1e9 / peak}
+    for k in ("leaves", "link"):                                                  # latency-bound: budgeted in time
+        stages_roofline[k] = {"ms": stages[k], "mparticles_per_s": n / (stages[k] * 1e-3) / 1e6 if stages[k] > 0 else None,
+                              "share_of_step": stages[k] / ms_per_step}
+
+    # ---- incremental rebuilds (config 5's recipe: displace every particle, rebuild from the previous leaves) ---
+    incremental = None
+    if args.rebuilds and cfg.incremental_steps:
+        prev = tree["leaves"].clone()
+        times, rounds = [], []
+        for k in range(1, min(args.rebuilds, cfg.incremental_steps) + 1):
+            x, y, z = cfg_rank.step(x, y, z, k)
+            dx, dy, dz = (torch.from_numpy(a).cuda() for a in (x, y, z))
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            tree = cs.buildOctree(ctx, dx, dy, dz, bucket, buffers=bufs, prevLeaves=prev)
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1))
+            rounds.append(tree["rounds"])
+            prev = tree["leaves"].clone()
+        incremental = {"rebuilds": len(times), "ms_per_rebuild": float(np.mean(times)), "ms_each": times,
+                       "rounds": rounds, "mparticles_per_s": n / (float(np.mean(times)) * 1e-3) / 1e6,
+                       "what": "box + keys + full re-sort + buildLeaves(previous leaves) + link + counts"}
+
     # ---- CPU baseline: the oracle as it stands, one core, bounded sample ---------------------
     cpu = None
     if not args.no_cpu:
         sample_n = min(n, args.cpu_sample)
         dt, _ = _oracle_sample(cfg, sample_n, bucket)
-        cpu = {"value": sample_n / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+        cpu = {"value": sample_n / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle", "host": _host_cpu(),
                "sample": f"first {sample_n} particles of {cfg.name} (same recipe), full path once, {dt:.1f} s"}
 
     line = {
@@ -295,6 +342,7 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (1.5 GiB of coordinates per step at N=2^26)",
                    "input_checksum_first_1Mi": in_sum},
         "roofline": roofline, "full_build": full_build, "cpu_baseline": cpu, "e2e": e2e,
+        "stages_roofline": stages_roofline, "incremental": incremental,
         "gpu_launches": int(launches), "stages_ms": stages, "clocks": clocks.summary(),
     }
     print(json.dumps(line), flush=True)
@@ -312,6 +360,8 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the particle count (same recipe)")
     ap.add_argument("--cpu-sample", type=int, default=1 << 26)
     ap.add_argument("--ref-sample", type=int, default=1 << 22)
+    ap.add_argument("--rebuilds", type=int, default=0,
+                    help="after the timed builds, time this many incremental rebuilds (workloads with a step recipe: c5)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
