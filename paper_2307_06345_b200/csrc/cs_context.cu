@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, divLevel, tileLookback, dirFlags, dirTotals, dirBases, linkTileHist, ctrl, total;
+        leafOffFinal, leafTasks, divLevel, tileLookback, dirFlags, dirTotals, dirBases, dirListSize, dirListKeys, dirListMeta, linkTileHist, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -63,6 +63,9 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.dirFlags = take(dirTiles << (kDirectTileLog2 - 3));                  // one-pass leaf build: 1 bit per position
     L.dirTotals = take((dirTiles + 2) * sizeof(u32));                      // K entries per tile
     L.dirBases = take((dirTiles + 2) * sizeof(u32));                       // exclusive prefix of dirTotals
+    L.dirListSize = take(dirTiles * sizeof(u32));
+    L.dirListKeys = take(dirTiles * kDirectCompact * sizeof(ulonglong2));   // 2 B per particle
+    L.dirListMeta = take(dirTiles * kDirectCompact * sizeof(u32));          // 0.5 B per particle
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
@@ -221,6 +224,9 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->dirFlags = (unsigned char*)(ctx->slab + L.dirFlags);
     ctx->dirTotals = (u32*)(ctx->slab + L.dirTotals);
     ctx->dirBases = (u32*)(ctx->slab + L.dirBases);
+    ctx->dirListSize = (u32*)(ctx->slab + L.dirListSize);
+    ctx->dirListKeys = (ulonglong2*)(ctx->slab + L.dirListKeys);
+    ctx->dirListMeta = (u32*)(ctx->slab + L.dirListMeta);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
     *out = ctx;

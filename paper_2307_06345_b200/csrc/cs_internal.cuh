@@ -54,6 +54,7 @@ constexpr int kLinkBins = 2 * (kL + 1);              // per level: all nodes, in
 // one-pass leaf build (cs_leaves_direct.cu): particle boundaries per tile, largest bucketSize it takes
 constexpr int kDirectTileLog2 = 11;
 constexpr int kDirectMaxBucket = 1024;
+constexpr int kDirectCompact = 256;      // leaf starts per tile that the levels kernel hands over as a compact list
 
 constexpr int kScanBlock = 256;
 constexpr int kScanItems = 8;
@@ -125,6 +126,9 @@ struct cs_context {
     unsigned char* dirFlags = nullptr; // one-pass leaf build: bit j set <=> position j owns entries of K
     cs::u32* dirTotals = nullptr;      // [tiles] K entries owned by the positions of a tile
     cs::u32* dirBases = nullptr;       // [tiles + 1] exclusive prefix of dirTotals
+    cs::u32* dirListSize = nullptr;    // [tiles] leaf starts of the tile, or ~0u if they exceed kDirectCompact (then flags / levels serve)
+    ulonglong2* dirListKeys = nullptr; // [tiles][kDirectCompact] the two keys around each leaf start
+    cs::u32* dirListMeta = nullptr;    // [tiles][kDirectCompact] position | levels | entry count of each leaf start
     int leafMode = 0;                  // cs_setLeafMode
     cs::u32* linkTileHist = nullptr;   // [tiles][kLinkBins] node counts per tile, level and kind
     cs::DeviceCtrl* ctrl = nullptr;

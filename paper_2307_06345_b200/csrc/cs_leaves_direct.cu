@@ -232,7 +232,8 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
 // (flags, one bit per position) and how many entries the tile owns (totals).  No CTA waits for another.
 __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
     leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 b, unsigned char* __restrict__ dArr,
-                       unsigned char* __restrict__ flags, u32* __restrict__ totals)
+                       unsigned char* __restrict__ flags, u32* __restrict__ totals, u32* __restrict__ listSize,
+                       ulonglong2* __restrict__ listKeys, u32* __restrict__ listMeta)
 {
     extern __shared__ __align__(16) unsigned char dsm[];
     __shared__ u32 sTotal, sMaxLevel;
@@ -265,8 +266,6 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
     // one bit per position: bit k of the byte <-> position 8 tid + k
     const u32 bitsA = ((fA & 0x01010101u) * 0x10204080u) >> 28, bitsB = ((fB & 0x01010101u) * 0x10204080u) >> 28;
     const u32 fbyte = bitsA | (bitsB << 4);
-    flags[(size_t)tile * kDirBlock + tid] = (unsigned char)fbyte;
-    *reinterpret_cast<uint2*>(dArr + (size_t)T0 + 8 * tid) = make_uint2(dA, dB);
     const u32 mine = __popc(fbyte);
     u32 mx = __vmaxu4(dA, dB);
     mx = __vmaxu4(mx, mx >> 16);
@@ -279,17 +278,31 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
     if ((tid & 31u) == 0 && mx + 1 > sMaxLevel) atomicMax(&sMaxLevel, mx + 1);   // leaf level D = d + 1
     __syncthreads();
 
-    // ---- K entries owned by the tile --------------------------------------------------------------
+    // ---- K entries owned by the tile; the leaf starts go to the emission kernel as a compact list (the two
+    // keys, position, levels and entry count of each), or, if there are too many, as flags + level bytes -------
+    const bool compact = nb <= (u32)kDirectCompact;
+    if (!compact) flags[(size_t)tile * kDirBlock + tid] = (unsigned char)fbyte;
+    // level bytes: the whole tile for the gather path, and always its last particles (position T0 + 2048 of the
+    // next tile reads the level of particle T0 + 2047)
+    if (!compact || tid == kDirBlock - 1) *reinterpret_cast<uint2*>(dArr + (size_t)T0 + 8 * tid) = make_uint2(dA, dB);
     u32 cnt = 0;
     for (u32 m = tid; m < nb; m += kDirBlock) {
         const u32 p = sm.list[m];
-        cnt += dirCount(sm.K[p + b], sm.K[p + b + 1], dmax[p] + 1, dmax[p + 1] + 1, (u32)(T0 + p), n);
+        const u64 a = sm.K[p + b], c = sm.K[p + b + 1];
+        const u32 Da = dmax[p] + 1u, Dc = dmax[p + 1] + 1u;
+        const u32 e = dirCount(a, c, (int)Da, (int)Dc, (u32)(T0 + p), n);
+        cnt += e;
+        if (compact) {                                       // p < 2^11, levels <= 22, e <= 7 * 21 + 7 + 1
+            listKeys[(size_t)tile * kDirectCompact + m] = make_ulonglong2(a, c);
+            listMeta[(size_t)tile * kDirectCompact + m] = p | (Da << 11) | (Dc << 16) | (e << 21);
+        }
     }
     cnt = warpReduceSum(cnt);
     if ((tid & 31u) == 0 && cnt) atomicAdd(&sTotal, cnt);
     __syncthreads();
     if (tid == 0) {
         totals[tile] = sTotal;
+        listSize[tile] = compact ? nb : 0xFFFFFFFFu;
         atomicMax(&ctrl->changed[0], sMaxLevel);           // changed[0] doubles as the deepest leaf level
     }
 }
@@ -301,41 +314,64 @@ constexpr int kEmitBlock = kDirBlock / 2;                 // 16 positions per th
 __global__ void __launch_bounds__(kEmitBlock)
     leavesEmitDirectKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, const unsigned char* __restrict__ dArr,
                            const unsigned char* __restrict__ flags, const u32* __restrict__ bases, u32 tiles,
-                           u64* __restrict__ K, u32* __restrict__ off, u32 cap)
+                           const u32* __restrict__ listSize, const ulonglong2* __restrict__ listKeys,
+                           const u32* __restrict__ listMeta, u64* __restrict__ K, u32* __restrict__ off, u32 cap)
 {
     __shared__ unsigned short list[kDirTile];
     __shared__ u32 warpSums[kEmitBlock / 32 + 1];
     const u32 tid = threadIdx.x;
     const u32 tile = blockIdx.x;
     const u64 T0 = (u64)tile * kDirTile;
-    const u32 fbits = reinterpret_cast<const unsigned short*>(flags)[(size_t)tile * kEmitBlock + tid];
     u32 carry = bases[tile];
-    u32 nb;
-    u32 slot = blockExclusiveScan<kEmitBlock>(__popc(fbits), warpSums, &nb);
-    for (u32 f = fbits; f; f &= f - 1) list[slot++] = (unsigned short)(16 * tid + __ffs((int)f) - 1);
-    __syncthreads();
-    for (u32 base = 0; base < nb; base += kEmitBlock) {
-        const u32 m = base + tid;
-        u64 a = 0, c = 0;
-        int Da = 0, Dc = 0;
-        u32 j = 0, cnt = 0;
-        if (m < nb) {
-            j = (u32)(T0 + list[m]);
-            if (j > 0) {
-                a = __ldg(P + j - 1);
-                Da = dArr[j - 1] + 1;
+    const u32 listed = listSize[tile];
+    if (listed != 0xFFFFFFFFu) {
+        // ---- compact list from the levels kernel: nothing to gather, nothing to recount ------------------------
+        for (u32 base = 0; base < listed; base += kEmitBlock) {
+            const u32 m = base + tid;
+            ulonglong2 ac = make_ulonglong2(0, 0);
+            u32 meta = 0;
+            if (m < listed) {
+                ac = listKeys[(size_t)tile * kDirectCompact + m];
+                meta = listMeta[(size_t)tile * kDirectCompact + m];
             }
-            if (j < n) {
-                c = __ldg(P + j);
-                Dc = dArr[j] + 1;
-            }
-            cnt = dirCount(a, c, Da, Dc, j, n);
+            const u32 cnt = meta >> 21;
+            u32 t;
+            const u32 e = blockExclusiveScan<kEmitBlock>(cnt, warpSums, &t);
+            if (cnt)
+                dirEmit(ac.x, ac.y, (int)((meta >> 11) & 31u), (int)((meta >> 16) & 31u), (u32)(T0 + (meta & 2047u)), n,
+                        carry + e, K, off, cap);
+            carry += t;
+            __syncthreads();                                // warpSums is reused by the next chunk
         }
-        u32 t;
-        const u32 e = blockExclusiveScan<kEmitBlock>(cnt, warpSums, &t);
-        if (cnt) dirEmit(a, c, Da, Dc, j, n, carry + e, K, off, cap);
-        carry += t;
-        __syncthreads();                                    // warpSums is reused by the next chunk
+    } else {
+        const u32 fbits = reinterpret_cast<const unsigned short*>(flags)[(size_t)tile * kEmitBlock + tid];
+        u32 nb;
+        u32 slot = blockExclusiveScan<kEmitBlock>(__popc(fbits), warpSums, &nb);
+        for (u32 f = fbits; f; f &= f - 1) list[slot++] = (unsigned short)(16 * tid + __ffs((int)f) - 1);
+        __syncthreads();
+        for (u32 base = 0; base < nb; base += kEmitBlock) {
+            const u32 m = base + tid;
+            u64 a = 0, c = 0;
+            int Da = 0, Dc = 0;
+            u32 j = 0, cnt = 0;
+            if (m < nb) {
+                j = (u32)(T0 + list[m]);
+                if (j > 0) {
+                    a = __ldg(P + j - 1);
+                    Da = dArr[j - 1] + 1;
+                }
+                if (j < n) {
+                    c = __ldg(P + j);
+                    Dc = dArr[j] + 1;
+                }
+                cnt = dirCount(a, c, Da, Dc, j, n);
+            }
+            u32 t;
+            const u32 e = blockExclusiveScan<kEmitBlock>(cnt, warpSums, &t);
+            if (cnt) dirEmit(a, c, Da, Dc, j, n, carry + e, K, off, cap);
+            carry += t;
+            __syncthreads();                                // warpSums is reused by the next chunk
+        }
     }
     if (tile == 0 && tid == 0) {                            // close the build
         const u32 nl = bases[tiles] - 1;                    // K entries minus the terminal 8^21
@@ -393,10 +429,12 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
     }
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
     leavesLevelsKernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags,
-                                                         ctx->dirTotals);
+                                                         ctx->dirTotals, ctx->dirListSize, ctx->dirListKeys,
+                                                         ctx->dirListMeta);
     CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
     CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));
     leavesEmitDirectKernel<<<tiles, kEmitBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
+                                                       ctx->dirListSize, ctx->dirListKeys, ctx->dirListMeta,
                                                        ctx->leafK[0], ctx->leafOff[0], cap);
     CS_LAUNCH_CHECK(ctx, "leavesEmitDirectKernel");
     return CS_OK;
