@@ -125,13 +125,27 @@ def _workload(name: str):
 
 
 def _oracle_sample(cfg, sample_n: int, bucket: int, seed_shift: int = 0):
-    """Time the oracle, as it stands, on a bounded sample of the workload (single core)."""
+    """Time the oracle, as it stands, on a bounded sample of the workload (single core): the stage calls that
+    oracle.full_build makes, one after the other, each on the clock."""
     import oracle
     x, y, z = cfg.generate(sample_n)
-    t0 = time.perf_counter()
-    ref = oracle.full_build(x, y, z, bucket)
-    dt = time.perf_counter() - t0
-    return dt, ref["leaves"].size - 1
+    stages = {}
+    t00 = t0 = time.perf_counter()
+
+    def lap(name):
+        nonlocal t0
+        t1 = time.perf_counter()
+        stages[name] = t1 - t0
+        t0 = t1
+
+    b = oracle.box(x, y, z); lap("box")
+    k = oracle.keys(x, y, z, b); lap("keys")
+    P, perm = oracle.sort(k); lap("sort")
+    K, counts = oracle.leaves_topdown(P, bucket); lap("leaves")
+    tree = oracle.link(K); lap("link")
+    oracle.node_counts(counts, tree); lap("counts")
+    _oracle_sample.stages = stages
+    return time.perf_counter() - t00, K.size - 1
 
 
 def run_reference(args):
@@ -343,7 +357,8 @@ def run_ours(args):
         sample_n = min(n, args.cpu_sample)
         dt, _ = _oracle_sample(cfg, sample_n, bucket)
         cpu = {"value": sample_n / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle", "host": _host_cpu(),
-               "sample": f"first {sample_n} particles of {cfg.name} (same recipe), full path once, {dt:.1f} s"}
+               "sample": f"first {sample_n} particles of {cfg.name} (same recipe), full path once, {dt:.1f} s",
+               "stages_s": {k: round(v, 3) for k, v in _oracle_sample.stages.items()}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
