@@ -29,7 +29,7 @@
 namespace cs {
 
 #ifndef CS_DIR_MINBLOCKS
-#define CS_DIR_MINBLOCKS 4
+#define CS_DIR_MINBLOCKS 6
 #endif
 constexpr int kDirBlock = 256;
 constexpr int kDirItems = 8;

@@ -198,7 +198,10 @@ __device__ __forceinline__ u32 subtreeEnd(const u64* __restrict__ K, u32 j, u32 
     return lo;
 }
 
-__global__ void __launch_bounds__(kLinkBlock)
+#ifndef CS_LINK_MINBLOCKS
+#define CS_LINK_MINBLOCKS 4
+#endif
+__global__ void __launch_bounds__(kLinkBlock, CS_LINK_MINBLOCKS)
     linkEmitKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves, LinkOut out,
                    const u32* __restrict__ tilePrefix)
 {

@@ -7,8 +7,11 @@ namespace cs {
 
 constexpr int kBoxBlock = 512;
 constexpr int kBoxBlocksPerSM = 4;
+#ifndef CS_KEYS_MINBLOCKS
+#define CS_KEYS_MINBLOCKS 4
+#endif
 constexpr int kKeysBlock = 256;
-constexpr int kKeysBlocksPerSM = 4;
+constexpr int kKeysBlocksPerSM = CS_KEYS_MINBLOCKS;
 
 // ---------------------------------------------------------------------------------------------
 // H1: per-dimension min / max.  Each CTA reduces a grid-strided slice, writes 6 partials, and
@@ -242,7 +245,7 @@ __device__ __forceinline__ void histAdd(u32* sh, u64 key)
 }
 
 template <bool VEC, bool HIST>
-__global__ void __launch_bounds__(kKeysBlock, 4) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
+__global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
                                                          const double* __restrict__ z, u64 n,
                                                          const double* __restrict__ box6, u64* __restrict__ keys,
                                                          u32* gHist)
