@@ -320,28 +320,32 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
 // are sorted by all bits >= LOW; what is left is the order of the low bits inside every run of equal
 // leading bits.  The elements of such a run are adjacent in the input's order within one top digit, so if
 // no run straddles a tile, every run lies contiguous in the tile staged in shared memory and can be
-// ordered there, on the way out.  Hence the tiles are cut at run boundaries: nominal boundaries every
-// kLastTile elements, each moved back to the start of the run it falls into (at most kFixupMaxRun
-// elements).  An element of a run goes to runStart + (run elements with smaller low bits) + (earlier run
+// ordered there, on the way out.  Hence the tiles are cut between groups of elements that agree in the
+// bits LOW..53 (the input's order; a run is part of one group): nominal boundaries every kLastTile
+// elements, each moved back to the start of the group it falls into (at most kFixupMaxRun elements).  An element of a run goes to runStart + (run elements with smaller low bits) + (earlier run
 // elements with equal low bits).  A run longer than kFixupMaxRun + 1 raises *redo instead (the gated passes
 // that follow redo the sort from this pass's input).
 constexpr u32 kFixupMaxRun = 256;
 constexpr u32 kLastTile = kSortLastTile;                  // nominal tile: room for a boundary run, multiple of 64
 static_assert(kLastTile % 64 == 0 && kLastTile > 2 * kFixupMaxRun, "nominal tile of the last pass");
 
-// start of the run (equal bits >= LOW) that element `b` falls into, found by one warp; 0 < b < n.
-// *tooLong is set if the run starts more than kFixupMaxRun elements before b (then b itself is returned).
-template <int LOW>
-__device__ __forceinline__ u32 runStartBefore(const u64* __restrict__ keysIn, u32 b, bool* tooLong)
+// Where to cut the input at or before element `b` (0 < b < n) so that no run is split: the input is ordered
+// by the bits LOW .. TOP-1 only, so the members of a run (equal bits >= LOW) need not be neighbours there; the
+// elements that agree in the bits LOW .. TOP-1 are (a "group": every run lies inside one).  Returns the start
+// of the group of element b, found by one warp.  *tooLong is set if it starts more than kFixupMaxRun elements
+// before b (then b itself is returned).
+template <int LOW, int TOP>
+__device__ __forceinline__ u32 groupStartBefore(const u64* __restrict__ keysIn, u32 b, bool* tooLong)
 {
+    constexpr u64 kGroupBits = ((1ull << TOP) - 1) & ~((1ull << LOW) - 1);
     const u32 lane = laneId();
     const u64 kb = keysIn[b];
     u32 back = 0;
     for (;;) {
         const u32 off = back + lane + 1;                    // element b - off
-        const bool same = off <= b && ((keysIn[b - (off <= b ? off : 0)] ^ kb) >> LOW) == 0;
+        const bool same = off <= b && ((keysIn[b - (off <= b ? off : 0)] ^ kb) & kGroupBits) == 0;
         const u32 m = __ballot_sync(kFull, same);
-        const u32 c = m == kFull ? 32u : (u32)__ffs((int)~m) - 1u;   // lanes 0..c-1 are in the run
+        const u32 c = m == kFull ? 32u : (u32)__ffs((int)~m) - 1u;   // lanes 0..c-1 are in the group
         back += c;
         if (c < 32) break;
         if (back > kFixupMaxRun) break;
@@ -473,7 +477,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
         const u64 nominal = (u64)(tile + w) * kLastTile;
         u32 cut = nominal < n ? (u32)nominal : n;
         bool tooLong = false;
-        if (cut > 0 && cut < n) cut = runStartBefore<LOW>(keysIn, cut, &tooLong);
+        if (cut > 0 && cut < n) cut = groupStartBefore<LOW, SHIFT>(keysIn, cut, &tooLong);
         if ((tid & 31u) == 0) {
             sCut[w] = cut;
             if (tooLong) *reinterpret_cast<volatile u32*>(redo) = 1u;

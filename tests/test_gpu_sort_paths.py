@@ -143,3 +143,20 @@ def test_unaligned_arrays(cs, ctx):
     dperm = torch.empty(k.size + 1, dtype=torch.int32, device=ctx.device)[1:k.size]
     cs.sortKeys(ctx, dk, dperm)
     assert np.array_equal(cs.u64(dk), P) and np.array_equal(cs.u32(dperm), perm)
+
+
+@pytest.mark.parametrize("group", [3, 40, 200])
+def test_runs_that_are_not_neighbours_before_the_last_pass(cs, ctx, group):
+    """Keys that agree in bits 18..53 but differ in the top digit are interleaved in the order the fifth pass
+    reads (it is sorted by bits 18..53 only), so the members of a run (equal bits 18..62) are not neighbours
+    there.  The tile cuts of that pass must not separate them: with groups this long every cut falls into one."""
+    rng = np.random.default_rng(100 + group)
+    n_groups = 300000 // group
+    mid = rng.choice(1 << 36, size=n_groups, replace=False).astype(np.uint64)            # bits 18..53
+    mid = np.repeat(mid, group)
+    top = rng.integers(0, 4, mid.size, dtype=np.uint64) * np.uint64(127)                 # 4 different top digits
+    low = rng.integers(0, 1 << LOW, mid.size, dtype=np.uint64)
+    k = (top << np.uint64(54)) | (mid << np.uint64(LOW)) | low
+    k[::11] = k[1::11][: k[::11].size]                                                   # and some equal whole keys
+    rng.shuffle(k)
+    check(cs, ctx, k)
