@@ -1,6 +1,6 @@
 """GPU parity on randomly drawn small cases: sizes around the tile sizes of every kernel, bucket sizes from 1 to
 1024, and particle sets with the structures that steer the data-dependent paths (uniform, tight clusters deeper
-than level 15, exact duplicates, points on a coarse lattice, a flat dimension).  Every output of cs_buildOctree
+than level 15, exact duplicates, points on a coarse lattice, a flat dimension, cells repeated across octants).  Every output of cs_buildOctree
 must equal the oracle's, bit for bit.  Seeds are fixed: the cases are the same in every run.
 """
 import numpy as np
@@ -48,6 +48,15 @@ def draw(rng, n, kind):
     elif kind == "flat":                           # one dimension without extent
         p = rng.random((3, n))
         p[1, :] = 0.25
+    elif kind == "twins":                          # same cell path on levels 4..15, other octants on levels 1..3:
+        m = max(1, n // 6)                         # keys equal in bits 18..53 that differ in the top digit
+        mid = rng.integers(0, 1 << 12, (3, m))     # grid bits 6..17 of each dimension
+        pick = rng.integers(0, m, n)
+        g = (rng.integers(0, 8, (3, n)) << 18) | (mid[:, pick] << 6) | rng.integers(0, 64, (3, n))
+        p = (g + 0.5) / float(1 << 21)
+        if n >= 2:                                 # pin the box to [0, 1]: the grid above is then the key grid
+            p[:, 0] = 0.0
+            p[:, 1] = 1.0
     else:
         raise ValueError(kind)
     return tuple(np.ascontiguousarray(p[d], dtype=np.float64) for d in range(3))
@@ -55,7 +64,7 @@ def draw(rng, n, kind):
 
 SIZES = (1, 2, 63, 64, 65, 257, 2047, 2048, 2049, 6335, 6336, 6337, 6655, 6656, 6657, 13313, 40000, 100003, 262144,
          400001)
-KINDS = ("uniform", "clusters", "duplicates", "lattice", "flat")
+KINDS = ("uniform", "clusters", "duplicates", "lattice", "flat", "twins")
 BUCKETS = (1, 2, 8, 64, 300, 1024)
 
 
