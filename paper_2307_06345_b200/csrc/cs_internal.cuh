@@ -54,7 +54,10 @@ constexpr int kLinkBins = 2 * (kL + 1);              // per level: all nodes, in
 // one-pass leaf build (cs_leaves_direct.cu): particle boundaries per tile, largest bucketSize it takes
 constexpr int kDirectTileLog2 = 11;
 constexpr int kDirectMaxBucket = 1024;
-constexpr int kDirectCompact = 256;      // leaf starts per tile that the levels kernel hands over as a compact list
+#ifndef CS_DIR_COMPACT
+#define CS_DIR_COMPACT 256
+#endif
+constexpr int kDirectCompact = CS_DIR_COMPACT;   // leaf starts per tile that the levels kernel hands over as a compact list
 
 constexpr int kScanBlock = 256;
 constexpr int kScanItems = 8;
