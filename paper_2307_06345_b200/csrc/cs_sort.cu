@@ -85,17 +85,13 @@ __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restri
     }
 }
 
-// exclusive scan of each pass's digit counts, in place (one CTA)
+// exclusive scan of each pass's digit counts, in place (one CTA per pass)
 __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 {
     __shared__ u32 warpSums[kRadix / 32 + 1];
-    for (int p = 0; p < kSortPasses; ++p) {
-        u32 v = gHist[p * kRadix + threadIdx.x];
-        u32 total;
-        u32 excl = blockExclusiveScan<kRadix>(v, warpSums, &total);
-        gHist[p * kRadix + threadIdx.x] = excl;
-        __syncthreads();
-    }
+    const u32 i = blockIdx.x * kRadix + threadIdx.x;
+    u32 total;
+    gHist[i] = blockExclusiveScan<kRadix>(gHist[i], warpSums, &total);
 }
 
 // ---- one radix pass ------------------------------------------------------------------------------
@@ -600,7 +596,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
             sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first);
             CS_LAUNCH_CHECK(ctx, "sortHistKernel");
         }
-        sortScanHistKernel<<<1, kRadix, 0, s>>>(ctx->sortHist);
+        sortScanHistKernel<<<kSortPasses, kRadix, 0, s>>>(ctx->sortHist);
         CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
     }
     ctx->evUsed[CS_STAGE_SORT_FIXUP] = false;
