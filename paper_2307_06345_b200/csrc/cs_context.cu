@@ -229,6 +229,12 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->dirListMeta = (u32*)(ctx->slab + L.dirListMeta);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
+    cs_status st = sortInit(ctx);
+    if (st == CS_OK) st = leavesDirectInit(ctx);
+    if (st != CS_OK) {
+        cs_destroy(ctx);
+        return st;
+    }
     *out = ctx;
     return CS_OK;
 }

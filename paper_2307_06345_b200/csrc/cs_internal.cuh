@@ -194,6 +194,8 @@ cs_status enqueueBox(cs_context*, const double* x, const double* y, const double
 // withHist: also accumulate the 8 digit histograms of the radix sort into ctx->sortHist
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
                       u64* keys, bool withHist, cudaStream_t);
+cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
+cs_status leavesDirectInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
 u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
 cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t);

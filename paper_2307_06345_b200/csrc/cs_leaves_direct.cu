@@ -407,6 +407,14 @@ __global__ void leavesDirectRootKernel(DeviceCtrl* ctrl, u64* K, u32* off, u32 n
     }
 }
 
+// dynamic shared memory of the levels kernel up to the largest bucket size it takes (per device: once per cs_create)
+cs_status leavesDirectInit(cs_context* ctx)
+{
+    CS_CUDA(ctx, cudaFuncSetAttribute(leavesLevelsKernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)dirLayout(kDirectMaxBucket).total));
+    return CS_OK;
+}
+
 bool leavesDirectSupported(const cs_context* ctx, u32 bucket)
 {
     return bucket <= (u32)kDirectMaxBucket && dirLayout(bucket).total <= 200u * 1024u && ctx->dirFlags != nullptr;
@@ -422,11 +430,6 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
         return CS_OK;
     }
     const DirLayout L = dirLayout(bucket);
-    static u32 attrBytes = 0;
-    if (L.total > 48u * 1024u && L.total > attrBytes) {
-        CS_CUDA(ctx, cudaFuncSetAttribute(leavesLevelsKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
-        attrBytes = L.total;
-    }
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
     leavesLevelsKernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags,
                                                          ctx->dirTotals, ctx->dirListSize, ctx->dirListKeys,

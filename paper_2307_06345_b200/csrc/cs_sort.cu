@@ -538,12 +538,6 @@ struct PassPlan {
 template <int SHIFT, bool FIRST>
 static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 {
-    static bool attrSet = false;
-    if (!attrSet) {
-        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<SHIFT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)sizeof(SortSmem)));
-        attrSet = true;
-    }
     const u32 epoch = nextEpoch(ctx, s);
     const int in = pl.cur, out = in ^ 1;
     onesweepKernel<SHIFT, FIRST><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
@@ -557,12 +551,6 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 template <int SHIFT>
 static cs_status launchGatedPass(cs_context* ctx, PassPlan& pl, const u32* gate, cudaStream_t s)
 {
-    static bool attrSet = false;
-    if (!attrSet) {
-        CS_CUDA(ctx, cudaFuncSetAttribute(onesweepGatedKernel<SHIFT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)sizeof(SortSmem)));
-        attrSet = true;
-    }
     const u32 epoch = nextEpoch(ctx, s);
     const int in = pl.cur, out = in ^ 1;
     const u32 resident = (u32)ctx->numSMs * kSortMinBlocks;
@@ -571,6 +559,32 @@ static cs_status launchGatedPass(cs_context* ctx, PassPlan& pl, const u32* gate,
         ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, gate);
     CS_LAUNCH_CHECK(ctx, "onesweepGatedKernel");
     pl.cur = out;
+    return CS_OK;
+}
+
+// The radix kernels need more dynamic shared memory than the default limit: opt in on the context's device
+// (function attributes are per device, so this runs once per cs_create, not once per process).
+template <int SHIFT>
+static cudaError_t sortInitShift()
+{
+    const int bytes = (int)sizeof(SortSmem);
+    cudaError_t e = cudaFuncSetAttribute(onesweepKernel<SHIFT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweepGatedKernel<SHIFT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return e;
+}
+cs_status sortInit(cs_context* ctx)
+{
+    const int bytes = (int)sizeof(SortSmem);
+    CS_CUDA(ctx, sortInitShift<0>());
+    CS_CUDA(ctx, sortInitShift<9>());
+    CS_CUDA(ctx, sortInitShift<18>());
+    CS_CUDA(ctx, sortInitShift<27>());
+    CS_CUDA(ctx, sortInitShift<36>());
+    CS_CUDA(ctx, sortInitShift<45>());
+    CS_CUDA(ctx, sortInitShift<54>());
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     return CS_OK;
 }
 
@@ -628,12 +642,6 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     }
     StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     {   // top digit; this pass also orders the low bits inside the runs
-        static bool attrSet = false;
-        if (!attrSet) {
-            CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              (int)sizeof(SortSmem)));
-            attrSet = true;
-        }
         const u32 epoch = nextEpoch(ctx, s);
         const int in = pl.cur, out = in ^ 1;
         onesweepLastKernel<54, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
