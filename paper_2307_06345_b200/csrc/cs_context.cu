@@ -80,7 +80,7 @@ u32 nextEpoch(cs_context* ctx, cudaStream_t s)
     if (ctx->epoch >= (1u << 30)) {   // wrap: clear every look-back array once
         Layout L = makeLayout(ctx->maxParticles, ctx->maxLeaves, kBoxGridMax);
         cudaMemsetAsync(ctx->sortLookback, 0, L.boxPartials - L.sortLookback, s);
-        cudaMemsetAsync(ctx->tileLookback, 0, L.linkTileHist - L.tileLookback, s);
+        cudaMemsetAsync(ctx->tileLookback, 0, L.dirFlags - L.tileLookback, s);
         ctx->epoch = 1;
     }
     return ctx->epoch;
