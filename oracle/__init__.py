@@ -32,6 +32,9 @@ def lib():
         _lib.orc_leaves_topdown.restype = C.c_int64
         _lib.orc_link.restype = C.c_int64
         _lib.orc_node_counts.restype = None
+        _lib.orc_node_geometry.restype = None
+        _lib.orc_centers_of_mass.restype = None
+        _lib.orc_mac_min_distance.restype = None
     return _lib
 
 
@@ -183,4 +186,34 @@ def full_build(x, y, z, bucket_size):
     out = {"box": b, "keys": k, "sortedKeys": P, "perm": perm, "leaves": K, "counts": counts,
            "nodeFirst": first, "nodeCount": count}
     out.update(tree)
+    return out
+
+
+def node_geometry(prefixes, box6):
+    """O8: (centers[3, n], halfSizes[3, n]) of the nodes' cells in the bounding box."""
+    prefixes, box6 = _u64(prefixes), _f64(box6)
+    n = prefixes.size
+    centers = np.empty((3, n), dtype=np.float64)
+    half = np.empty((3, n), dtype=np.float64)
+    lib().orc_node_geometry(_p(prefixes), C.c_uint32(n), _p(box6), _p(centers), _p(half))
+    return centers, half
+
+
+def centers_of_mass(xs, ys, zs, node_first, node_count, child_offsets, centers):
+    """O9: com[3, n] by an upward pass over the linked tree; xs, ys, zs are the coordinates in SORTED order."""
+    xs, ys, zs, centers = _f64(xs), _f64(ys), _f64(zs), _f64(centers)
+    node_first, node_count, child_offsets = _u32(node_first), _u32(node_count), _u32(child_offsets)
+    n = node_first.size
+    com = np.empty((3, n), dtype=np.float64)
+    lib().orc_centers_of_mass(_p(xs), _p(ys), _p(zs), _p(node_first), _p(node_count), _p(child_offsets), _p(centers),
+                              C.c_uint32(n), _p(com))
+    return com
+
+
+def mac_min_distance(centers, half_sizes, focus6, theta):
+    """O10: Eq. 12 against an axis-aligned focus box; uint8[n], 1 = fulfilled."""
+    centers, half_sizes, focus6 = _f64(centers), _f64(half_sizes), _f64(focus6)
+    n = centers.shape[1]
+    out = np.empty(n, dtype=np.uint8)
+    lib().orc_mac_min_distance(_p(centers), _p(half_sizes), C.c_uint32(n), _p(focus6), C.c_double(theta), _p(out))
     return out

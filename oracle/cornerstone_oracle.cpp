@@ -15,7 +15,8 @@
 // Every function cites the PAPER.md passage it follows; readings of silent or garbled
 // passages are the "A<n>" items of DESIGN.md ("Readings of the paper").
 // Parity pins: tests/test_oracle_*.py (all functions here are pinned; nothing is
-// "parity unpinned").
+// "parity unpinned").  O8-O10 (node properties, the first row past the hot path) are pinned in
+// tests/test_oracle_props.py.
 // =====================================================================================
 #include <algorithm>
 #include <cmath>
@@ -377,6 +378,104 @@ void orc_node_counts(const uint32_t* leafCounts, uint32_t nl, const uint32_t* ch
     for (uint32_t i = 0; i < nl; ++i) leafFirst[i + 1] = leafFirst[i] + leafCounts[i];
     Upsweep up{childOffsets, nodeToLeaf, &leafFirst, leafCounts, nodeFirst, nodeCount};
     up.visit(0);
+}
+
+
+// -------------------------------------------------------------------------------------
+// O8  node geometry (NEXT-1 of SURVEY 8f; "additional node properties ...
+// stored in separate arrays of length n").  A node with placeholder-bit key NK (a 1 followed
+// by `level` octal digits) is the cell (ix, iy, iz) of the 2^level grid over
+// the bounding box; digit = 4*xbit + 2*ybit + zbit (A3).  Reading A25: cell edge
+// h_d = (hi_d - lo_d) / 2^level, centre c_d = lo_d + (i_d + 0.5) * h_d, half size 0.5 * h_d,
+// each operation rounded once in binary64 (no contraction).  SoA outputs: centers[3][n],
+// halfSizes[3][n].
+// -------------------------------------------------------------------------------------
+void orc_node_geometry(const uint64_t* prefixes, uint32_t n, const double* box6, double* centers, double* halfSizes)
+{
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint64_t p = prefixes[i];
+        int bits = 0;
+        while ((p >> bits) > 1) ++bits;                  // position of the placeholder bit
+        const int level = bits / 3;
+        uint64_t g[3] = {0, 0, 0};
+        for (int l = 1; l <= level; ++l) {               // octal digits, most significant first
+            const unsigned digit = (unsigned)((p >> (3 * (level - l))) & 7u);
+            g[0] = (g[0] << 1) | ((digit >> 2) & 1u);
+            g[1] = (g[1] << 1) | ((digit >> 1) & 1u);
+            g[2] = (g[2] << 1) | (digit & 1u);
+        }
+        const double cells = (double)(1ull << level);
+        for (int d = 0; d < 3; ++d) {
+            const double lo = box6[2 * d], e = box6[2 * d + 1] - box6[2 * d];
+            const double h = e / cells;
+            centers[(size_t)d * n + i] = lo + ((double)g[d] + 0.5) * h;
+            halfSizes[(size_t)d * n + i] = 0.5 * h;
+        }
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O9  centres of mass by an upward pass ("properties where the leaves depend
+// on the contained particles and internal nodes on their children ... center-of-mass for
+// gravity").  Unit masses (the path carries coordinates only).  Reading A26: a leaf's centre
+// is the sum of its particles' coordinates, taken in sorted order (xs = x[perm], first ..
+// first + count - 1), divided by count; an internal node's is sum_c count_c * com_c over its 8
+// children in order, divided by its count; a node without particles takes its geometric
+// centre.  Nodes are visited from the last index to the first: children have larger indices
+// than their parent in the breadth-first layout.
+// -------------------------------------------------------------------------------------
+void orc_centers_of_mass(const double* xs, const double* ys, const double* zs, const uint32_t* nodeFirst,
+                         const uint32_t* nodeCount, const uint32_t* childOffsets, const double* centers, uint32_t n,
+                         double* com)
+{
+    const double* c[3] = {xs, ys, zs};
+    for (uint32_t ii = n; ii-- > 0;) {
+        for (int d = 0; d < 3; ++d) {
+            double s = 0.0;
+            if (nodeCount[ii] == 0) {
+                com[(size_t)d * n + ii] = centers[(size_t)d * n + ii];
+                continue;
+            }
+            if (childOffsets[ii] == 0) {
+                for (uint32_t j = nodeFirst[ii]; j < nodeFirst[ii] + nodeCount[ii]; ++j) s = s + c[d][j];
+            } else {
+                for (uint32_t k = 0; k < 8; ++k) {
+                    const uint32_t ch = childOffsets[ii] + k;
+                    s = s + (double)nodeCount[ch] * com[(size_t)d * n + ch];
+                }
+            }
+            com[(size_t)d * n + ii] = s / (double)nodeCount[ii];
+        }
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O10  minimum-distance MAC, Eq. 12: fulfilled if r_min > l / theta, with
+// r_min the minimum distance between source node and target, l the source node's edge
+// length.  Target = an axis-aligned focus box F ("with respect to any point in
+// F").  Reading A27: per dimension the gap between the two boxes is
+// max(|c - fc| - (h + fh), 0) with fc, fh centre and half size of F; r_min^2 is the sum of the
+// squared gaps (x, y, z in that order); l = 2 * max(hx, hy, hz) (the boxes need not be cubes);
+// the decision is taken without the square root, as (r_min^2 * (theta * theta)) > (l * l),
+// every operation rounded once in binary64.  pass[i] = 1 if fulfilled.
+// -------------------------------------------------------------------------------------
+void orc_mac_min_distance(const double* centers, const double* halfSizes, uint32_t n, const double* focus6, double theta,
+                          uint8_t* pass)
+{
+    const double t2 = theta * theta;
+    for (uint32_t i = 0; i < n; ++i) {
+        double r2 = 0.0, hmax = 0.0;
+        for (int d = 0; d < 3; ++d) {
+            const double fc = 0.5 * (focus6[2 * d] + focus6[2 * d + 1]), fh = 0.5 * (focus6[2 * d + 1] - focus6[2 * d]);
+            const double cc = centers[(size_t)d * n + i], h = halfSizes[(size_t)d * n + i];
+            double gap = std::fabs(cc - fc) - (h + fh);
+            if (!(gap > 0.0)) gap = 0.0;
+            r2 = r2 + gap * gap;
+            if (h > hmax) hmax = h;
+        }
+        const double l = 2.0 * hmax;
+        pass[i] = (r2 * t2 > l * l) ? 1 : 0;
+    }
 }
 
 }  // extern "C"
