@@ -247,6 +247,43 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
                              uint32_t bucketSize, const cs_octree_buffers* host, cs_octree_sizes* sizes,
                              void* stream);
 
+/* ---- node properties on the linked octree (first row past the hot path: "additional octree
+ *      node properties ... can be stored in separate arrays of length n"; readings A25-A27) --------
+ * All arrays are device pointers owned by the caller; the calls enqueue on `stream` and return.  Three-component
+ * outputs are structure-of-arrays: component d of node i at [d * numNodes + i].
+ */
+
+/* cs_gatherParticles -- the coordinates in SFC order: xs[j] = x[perm[j]] (perm as written by cs_sortKeys,
+ *   PAPER.md:168).  Not in place.  n == 0 is a no-op. */
+cs_status cs_gatherParticles(cs_context* ctx, const double* x, const double* y, const double* z, const uint32_t* perm,
+                             uint64_t n, double* xs, double* ys, double* zs, void* stream);
+
+/* cs_nodeGeometry -- the cell of every node in the bounding box: a node with placeholder-bit key NK of `level`
+ *   octal digits is cell (ix, iy, iz) of the 2^level grid (digit = 4 xbit + 2 ybit + zbit);
+ *   edge h_d = (hi_d - lo_d) / 2^level, centers[d] = lo_d + (i_d + 0.5) * h_d, halfSizes[d] = 0.5 * h_d, one
+ *   binary64 rounding per operation.  box6: dev, as written by cs_computeBox. */
+cs_status cs_nodeGeometry(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
+                          double* centers, double* halfSizes, void* stream);
+
+/* cs_nodeMassCenters -- centres of mass (unit masses) by an upward pass over the links: a leaf's
+ *   is the sum of its particles' sorted coordinates xs[first .. first + count) in that order over count, an
+ *   internal node's the sum over its 8 children in order of count_c * com_c over its count, an empty node takes
+ *   its geometric centre.  xs, ys, zs: coordinates in SFC order (cs_gatherParticles); nodeFirst / nodeCount /
+ *   childOffsets / levelRange: as written by cs_linkOctree + cs_nodeCounts or cs_buildOctree; centers: from
+ *   cs_nodeGeometry.  One launch per level, deepest first; no host synchronisation. */
+cs_status cs_nodeMassCenters(cs_context* ctx, const double* xs, const double* ys, const double* zs,
+                             const uint32_t* nodeFirst, const uint32_t* nodeCount, const uint32_t* childOffsets,
+                             const double* centers, const uint32_t* levelRange, uint32_t numNodes, double* com,
+                             void* stream);
+
+/* cs_macMinDistance -- the minimum-distance multipole acceptance criterion, Eq. 12: pass[i] = 1
+ *   iff r_min > l / theta for source node i and the axis-aligned target box focus6 = {xmin, xmax, ymin, ymax, zmin,
+ *   zmax} (HOST array; "with respect to any point in F").  r_min^2 = sum of squared per-dimension
+ *   gaps max(|c - fc| - (h + fh), 0), l = 2 * max_d h_d, decided as r_min^2 * theta^2 > l^2 in binary64.
+ *   Errors: INVALID_ARG (null pointer, theta <= 0). */
+cs_status cs_macMinDistance(cs_context* ctx, const double* centers, const double* halfSizes, uint32_t numNodes,
+                            const double* focus6, double theta, uint8_t* pass, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -89,6 +89,10 @@ def lib():
                                      C.POINTER(OctreeSizes), vp]),
         "cs_buildOctreeHost": (C.c_int, [vp, vp, vp, vp, u64, u32, C.POINTER(OctreeBuffers),
                                          C.POINTER(OctreeSizes), vp]),
+        "cs_gatherParticles": (C.c_int, [vp, vp, vp, vp, vp, u64, vp, vp, vp, vp]),
+        "cs_nodeGeometry": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
+        "cs_nodeMassCenters": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp, vp]),
+        "cs_macMinDistance": (C.c_int, [vp, vp, vp, u32, C.POINTER(C.c_double), C.c_double, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(l, name)
@@ -341,3 +345,41 @@ def buildOctreeHost(ctx: Context, x, y, z, bucketSize: int, host: HostBuffers):
                                   C.byref(sizes), _stream())
     ctx.check(st)
     return {"numLeaves": int(sizes.numLeaves), "numNodes": int(sizes.numNodes), "rounds": int(sizes.rounds)}
+
+
+# ---- node properties on the linked octree (include/cornerstone.h, last section) ---------------------------
+
+def gatherParticles(ctx: Context, x, y, z, perm):
+    """Coordinates in SFC order: (xs, ys, zs) with xs[j] = x[perm[j]]."""
+    out = [torch.empty_like(x) for _ in range(3)]
+    ctx.check(lib().cs_gatherParticles(ctx.handle, _ptr(x), _ptr(y), _ptr(z), _ptr(perm), x.numel(), _ptr(out[0]),
+                                       _ptr(out[1]), _ptr(out[2]), _stream()))
+    return tuple(out)
+
+
+def nodeGeometry(ctx: Context, prefixes, box6):
+    """(centers[3, n], halfSizes[3, n]) float64 tensors."""
+    n = prefixes.numel()
+    centers = torch.empty((3, n), dtype=torch.float64, device=ctx.device)
+    half = torch.empty((3, n), dtype=torch.float64, device=ctx.device)
+    ctx.check(lib().cs_nodeGeometry(ctx.handle, _ptr(prefixes), n, _ptr(box6), _ptr(centers), _ptr(half), _stream()))
+    return centers, half
+
+
+def nodeMassCenters(ctx: Context, xs, ys, zs, tree, centers):
+    """com[3, n] from the sorted coordinates and the dict returned by buildOctree."""
+    n = tree["numNodes"]
+    com = torch.empty((3, n), dtype=torch.float64, device=ctx.device)
+    ctx.check(lib().cs_nodeMassCenters(ctx.handle, _ptr(xs), _ptr(ys), _ptr(zs), _ptr(tree["nodeFirst"]),
+                                       _ptr(tree["nodeCount"]), _ptr(tree["childOffsets"]), _ptr(centers),
+                                       _ptr(tree["levelRange"]), n, _ptr(com), _stream()))
+    return com
+
+
+def macMinDistance(ctx: Context, centers, halfSizes, focus6, theta: float):
+    """uint8[n]: 1 where Eq. 12 holds against the focus box (6 host floats)."""
+    n = centers.shape[1]
+    out = torch.empty(n, dtype=torch.uint8, device=ctx.device)
+    f = (C.c_double * 6)(*[float(v) for v in focus6])
+    ctx.check(lib().cs_macMinDistance(ctx.handle, _ptr(centers), _ptr(halfSizes), n, f, float(theta), _ptr(out), _stream()))
+    return out

@@ -284,4 +284,51 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
     return CS_OK;
 }
 
+cs_status cs_gatherParticles(cs_context* ctx, const double* x, const double* y, const double* z, const uint32_t* perm,
+                             uint64_t n, double* xs, double* ys, double* zs, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_gatherParticles: ctx is null");
+    if (n == 0) return CS_OK;
+    if (!x || !y || !z || !perm || !xs || !ys || !zs) return fail(ctx, CS_ERR_INVALID_ARG, "cs_gatherParticles: null pointer");
+    if (xs == x || ys == y || zs == z) return fail(ctx, CS_ERR_INVALID_ARG, "cs_gatherParticles: in place is not supported");
+    if (n >= (1ull << 32)) return fail(ctx, CS_ERR_INVALID_ARG, "cs_gatherParticles: n >= 2^32");
+    DeviceGuard g(ctx->device);
+    return enqueueGather(ctx, x, y, z, perm, n, xs, ys, zs, (cudaStream_t)stream);
+}
+
+cs_status cs_nodeGeometry(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
+                          double* centers, double* halfSizes, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_nodeGeometry: ctx is null");
+    if (numNodes == 0) return CS_OK;
+    if (!prefixes || !box6 || !centers || !halfSizes) return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeGeometry: null pointer");
+    DeviceGuard g(ctx->device);
+    return enqueueNodeGeometry(ctx, (const u64*)prefixes, numNodes, box6, centers, halfSizes, (cudaStream_t)stream);
+}
+
+cs_status cs_nodeMassCenters(cs_context* ctx, const double* xs, const double* ys, const double* zs,
+                             const uint32_t* nodeFirst, const uint32_t* nodeCount, const uint32_t* childOffsets,
+                             const double* centers, const uint32_t* levelRange, uint32_t numNodes, double* com,
+                             void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_nodeMassCenters: ctx is null");
+    if (numNodes == 0) return CS_OK;
+    if (!xs || !ys || !zs || !nodeFirst || !nodeCount || !childOffsets || !centers || !levelRange || !com)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeMassCenters: null pointer");
+    DeviceGuard g(ctx->device);
+    return enqueueMassCenters(ctx, xs, ys, zs, nodeFirst, nodeCount, childOffsets, centers, levelRange, numNodes, com,
+                              (cudaStream_t)stream);
+}
+
+cs_status cs_macMinDistance(cs_context* ctx, const double* centers, const double* halfSizes, uint32_t numNodes,
+                            const double* focus6, double theta, uint8_t* pass, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_macMinDistance: ctx is null");
+    if (numNodes == 0) return CS_OK;
+    if (!centers || !halfSizes || !focus6 || !pass) return fail(ctx, CS_ERR_INVALID_ARG, "cs_macMinDistance: null pointer");
+    if (!(theta > 0.0)) return fail(ctx, CS_ERR_INVALID_ARG, "cs_macMinDistance: theta must be positive");
+    DeviceGuard g(ctx->device);
+    return enqueueMac(ctx, centers, halfSizes, numNodes, focus6, theta, pass, (cudaStream_t)stream);
+}
+
 }  // extern "C"

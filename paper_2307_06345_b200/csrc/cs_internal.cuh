@@ -215,5 +215,15 @@ cs_status enqueueNodeCounts(cs_context*, const u64* sortedKeys, u64 n, const u64
 // device-wide exclusive scan of u32 (decoupled look-back): out[i] = sum_{j<i} in[j], out[n] = total
 cs_status enqueueExclusiveScan(cs_context*, const u32* in, u32* out, u32 n, cudaStream_t);
 cs_status readCtrl(cs_context*, cudaStream_t);   // D2H of the control block + stream sync
+// node properties on the linked tree (cs_props.cu)
+cs_status enqueueGather(cs_context*, const double* x, const double* y, const double* z, const u32* perm, u64 n,
+                        double* xs, double* ys, double* zs, cudaStream_t);
+cs_status enqueueNodeGeometry(cs_context*, const u64* prefixes, u32 n, const double* box6, double* centers,
+                              double* halfSizes, cudaStream_t);
+cs_status enqueueMassCenters(cs_context*, const double* xs, const double* ys, const double* zs, const u32* nodeFirst,
+                             const u32* nodeCount, const u32* childOffsets, const double* centers, const u32* levelRange,
+                             u32 n, double* com, cudaStream_t);
+cs_status enqueueMac(cs_context*, const double* centers, const double* halfSizes, u32 n, const double* focus6,
+                     double theta, unsigned char* pass, cudaStream_t);
 
 }  // namespace cs
