@@ -300,3 +300,24 @@ def test_host_path_matches(cs, ctx):
         assert np.array_equal(hb.t[k].numpy().view(np.uint32)[:nn], ref[k]), k
     assert np.array_equal(hb.t["leafToNode"].numpy().view(np.uint32)[:nl], ref["leafToNode"])
     assert np.array_equal(hb.t["levelRange"].numpy().view(np.uint32), ref["levelRange"])
+
+
+def test_two_contexts_and_a_side_stream(cs):
+    """Contexts share nothing: two of them used alternately, one on a non-default stream, give the oracle's trees."""
+    xa, ya, za = W.blobs(150001, 41, nblobs=20)
+    xb, yb, zb = W.plummer(90000, 42)
+    ra, rb = oracle.full_build(xa, ya, za, 64), oracle.full_build(xb, yb, zb, 16)
+    ca = cs.Context(max_particles=200000, max_leaves=100000)
+    cb = cs.Context(max_particles=100000, max_leaves=100000)
+    da, db = [dev(a) for a in (xa, ya, za)], [dev(a) for a in (xb, yb, zb)]
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    for _ in range(3):
+        ga = cs.buildOctree(ca, da[0], da[1], da[2], 64)
+        with torch.cuda.stream(side):
+            gb = cs.buildOctree(cb, db[0], db[1], db[2], 16)
+        assert_tree_equal(cs, ga, ra, "context a")
+        assert_tree_equal(cs, gb, rb, "context b")
+        assert np.array_equal(cs.u32(ga["perm"]), ra["perm"]) and np.array_equal(cs.u32(gb["perm"]), rb["perm"])
+    ca.close()
+    cb.close()
