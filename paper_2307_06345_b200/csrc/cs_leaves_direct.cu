@@ -230,14 +230,18 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
 
 // One tile of kDirTile positions per CTA: d of every particle (dArr), which positions own K entries
 // (flags, one bit per position) and how many entries the tile owns (totals).  No CTA waits for another.
+// BFIX: bucket size known at compile time (the layout, loop counts and offsets of the sliding maximum become
+// constants), or 0 for any bucket size.
+template <u32 BFIX>
 __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
-    leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 b, unsigned char* __restrict__ dArr,
+    leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 bAny, unsigned char* __restrict__ dArr,
                        unsigned char* __restrict__ flags, u32* __restrict__ totals, u32* __restrict__ listSize,
                        ulonglong2* __restrict__ listKeys, u32* __restrict__ listMeta)
 {
     extern __shared__ __align__(16) unsigned char dsm[];
     __shared__ u32 sTotal, sMaxLevel;
     __shared__ u32 warpSums[kDirBlock / 32 + 1];
+    const u32 b = BFIX ? BFIX : bAny;
     const DirLayout L = dirLayout(b);
     DirSmem sm;
     sm.K = reinterpret_cast<u64*>(dsm);
@@ -410,7 +414,7 @@ __global__ void leavesDirectRootKernel(DeviceCtrl* ctrl, u64* K, u32* off, u32 n
 // dynamic shared memory of the levels kernel up to the largest bucket size it takes (per device: once per cs_create)
 cs_status leavesDirectInit(cs_context* ctx)
 {
-    CS_CUDA(ctx, cudaFuncSetAttribute(leavesLevelsKernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    CS_CUDA(ctx, cudaFuncSetAttribute(leavesLevelsKernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)dirLayout(kDirectMaxBucket).total));
     return CS_OK;
 }
@@ -431,9 +435,10 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
     }
     const DirLayout L = dirLayout(bucket);
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
-    leavesLevelsKernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags,
-                                                         ctx->dirTotals, ctx->dirListSize, ctx->dirListKeys,
-                                                         ctx->dirListMeta);
+    // the bucket sizes of BASELINE.json's configurations get kernels with the bucket size folded in
+    auto* kernel = bucket == 64 ? leavesLevelsKernel<64> : bucket == 16 ? leavesLevelsKernel<16> : leavesLevelsKernel<0>;
+    kernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags, ctx->dirTotals,
+                                             ctx->dirListSize, ctx->dirListKeys, ctx->dirListMeta);
     CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
     CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));
     leavesEmitDirectKernel<<<tiles, kEmitBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
