@@ -49,8 +49,14 @@ __device__ __forceinline__ u32 digitSum(u64 key, int lo, int hi)
 }
 __device__ __forceinline__ u32 digitAt(u64 key, int l) { return (u32)(key >> (3 * (kL - l))) & 7u; }
 __device__ __forceinline__ int sharedDigits(u64 a, u64 c) { return (__clzll((long long)(a ^ c)) - 1) / 3; }   // 21 if equal
-// the same from x = a ^ c (bit 63 clear): (clz - 1) / 3 for clz in 1..64, by multiplication
-__device__ __forceinline__ u32 sharedDigitsX(u64 x) { return ((u32)__clzll((long long)x) - 1u) * 43u >> 7; }
+// the same from x = a ^ c (bit 63 clear), without the 64-bit count of leading zeros: converted to float with
+// rounding toward zero, x keeps its binary exponent e = floor(log2 x), and (clz - 1) / 3 = (62 - e) / 3, the
+// division by multiplication (exact for 0 .. 189).  x = 0 converts to 0.0f (e = -127): 63, capped by the callers.
+__device__ __forceinline__ u32 sharedDigitsX(u64 x)
+{
+    const u32 e = (__float_as_uint(__ull2float_rz(x)) >> 23);   // e + 127
+    return ((62u + 127u) - e) * 43u >> 7;
+}
 
 // number of K entries owned by position j.  Da = D_{j-1}, Dc = D_j.
 __device__ __forceinline__ u32 dirCount(u64 a, u64 c, int Da, int Dc, u32 j, u32 n)
