@@ -138,6 +138,15 @@ struct DirSmem {
     unsigned short* list;     // positions p (tile-local) that own K entries, ascending
 };
 
+// byte-wise maximum of two words whose bytes are all below 128 (levels are at most 21): the SIMD video
+// instruction behind __vmaxu4 is emulated on this architecture (9 SASS), this takes 6
+__device__ __forceinline__ u32 maxBytes(u32 a, u32 b)
+{
+    const u32 ge = ((a | 0x80808080u) - b) & 0x80808080u;   // bit 7 of a byte set <=> a's byte >= b's (no borrow crosses bytes)
+    const u32 m = (ge >> 7) * 0xFFu;                        // 0xFF in those bytes
+    return (a & m) | (b & ~m);
+}
+
 // bytes [4q + o, 4q + o + 4) of the word array a
 __device__ __forceinline__ u32 dirShifted(const u32* a, u32 q, u32 o)
 {
@@ -208,12 +217,12 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
         if ((len & 3u) == 0) {                             // whole-word offsets: no funnel shifts
             const u32 o = len >> 2;
             for (u32 q = tid; q < L.words; q += kDirBlock)
-                dst[q] = __vmaxu4(__vmaxu4(src[q], src[q + o]), __vmaxu4(src[q + 2 * o], src[q + 3 * o]));
+                dst[q] = maxBytes(maxBytes(src[q], src[q + o]), maxBytes(src[q + 2 * o], src[q + 3 * o]));
         } else {
             for (u32 q = tid; q < L.words; q += kDirBlock) {
-                const u32 a = __vmaxu4(src[q], dirShifted(src, q, len));
-                const u32 c = __vmaxu4(dirShifted(src, q, 2 * len), dirShifted(src, q, 3 * len));
-                dst[q] = __vmaxu4(a, c);
+                const u32 a = maxBytes(src[q], dirShifted(src, q, len));
+                const u32 c = maxBytes(dirShifted(src, q, 2 * len), dirShifted(src, q, 3 * len));
+                dst[q] = maxBytes(a, c);
             }
         }
         __syncthreads();
@@ -221,13 +230,13 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
         len *= 4;
     }
     if (len * 2 <= W) {
-        for (u32 q = tid; q < L.words; q += kDirBlock) dst[q] = __vmaxu4(src[q], dirShifted(src, q, len));
+        for (u32 q = tid; q < L.words; q += kDirBlock) dst[q] = maxBytes(src[q], dirShifted(src, q, len));
         __syncthreads();
         u32* t = src; src = dst; dst = t;
         len *= 2;
     }
     if (len < W) {                                         // two overlapping windows of length len cover b+1
-        for (u32 q = tid; q < (kDirTile + 1 + 3) / 4 + 1; q += kDirBlock) dst[q] = __vmaxu4(src[q], dirShifted(src, q, W - len));
+        for (u32 q = tid; q < (kDirTile + 1 + 3) / 4 + 1; q += kDirBlock) dst[q] = maxBytes(src[q], dirShifted(src, q, W - len));
         __syncthreads();
         src = dst;
     }
