@@ -170,10 +170,12 @@ cs_status enqueueBox(cs_context* ctx, const double* x, const double* y, const do
 __device__ __forceinline__ u32 spread11(u32 v)
 {
     v &= 0x7FFu;
-    v = (v | (v << 16)) & 0x070000FFu;
-    v = (v | (v << 8)) & 0x0700F00Fu;
-    v = (v | (v << 4)) & 0x430C30C3u;
-    v = (v | (v << 2)) & 0x49249249u;
+    // v | (v << s) without overlapping bits == v * (2^s + 1): the multiplications issue on the FMA pipe, which
+    // idles in this kernel, the shifts would compete with the rest for the half-rate ALU pipe
+    v = (v * 0x00010001u) & 0x070000FFu;
+    v = (v * 0x00000101u) & 0x0700F00Fu;
+    v = (v * 0x00000011u) & 0x430C30C3u;
+    v = (v * 0x00000005u) & 0x49249249u;
     return v;
 }
 
