@@ -35,7 +35,33 @@ def lib():
         _lib.orc_node_geometry.restype = None
         _lib.orc_centers_of_mass.restype = None
         _lib.orc_mac_min_distance.restype = None
+        _lib.orc_set_L.restype = C.c_int
+        _lib.orc_hilbert_keys.restype = None
+        _lib.orc_hilbert_from_grid.restype = None
+        _lib.orc_global_round.restype = C.c_int64
+        _lib.orc_partition.restype = None
     return _lib
+
+
+class key_levels:
+    """``with oracle.key_levels(10): ...`` -- run the oracle with L octal digits per key (L = 10 for 32-bit
+    keys, 21 for 64-bit keys).  Keys stay in uint64 arrays; 8^L is the terminal element of K."""
+
+    def __init__(self, levels: int):
+        self.levels = int(levels)
+
+    def __enter__(self):
+        global L, KEY_END
+        self.old = lib().orc_set_L(self.levels)
+        if self.old < 0:
+            raise ValueError("L must be in 1..21")
+        L, KEY_END = self.levels, 1 << (3 * self.levels)
+        return self
+
+    def __exit__(self, *a):
+        global L, KEY_END
+        lib().orc_set_L(self.old)
+        L, KEY_END = self.old, 1 << (3 * self.old)
 
 
 def _p(a):
@@ -72,6 +98,22 @@ def keys(x, y, z, box6):
     return out
 
 
+def hilbert_keys(x, y, z, box6):
+    """O2h: Hilbert keys of the particles (reading A28), L octal digits."""
+    x, y, z, box6 = _f64(x), _f64(y), _f64(z), _f64(box6)
+    out = np.empty(x.size, dtype=np.uint64)
+    lib().orc_hilbert_keys(_p(x), _p(y), _p(z), C.c_uint64(x.size), _p(box6), _p(out))
+    return out
+
+
+def hilbert_from_grid(gx, gy, gz, levels):
+    """O2h on integer grid points of the 2^levels grid."""
+    gx, gy, gz = _u32(gx), _u32(gy), _u32(gz)
+    out = np.empty(gx.size, dtype=np.uint64)
+    lib().orc_hilbert_from_grid(_p(gx), _p(gy), _p(gz), C.c_uint64(gx.size), C.c_int(levels), _p(out))
+    return out
+
+
 def sort(keys_in):
     """O3: stable sort; returns (sortedKeys, perm) with perm the gather map."""
     keys_in = _u64(keys_in)
@@ -96,13 +138,41 @@ def round_(P, K, bucket_size, cap=None):
     return {"N": N, "O": O, "Oprime": Op, "K": None if nn < 0 else Kout[:nn + 1].copy()}
 
 
+def global_round(shards, K, bucket_size, cap=None):
+    """O11: one round of the distributed build: f on every shard (each a sorted key array), the
+    element-wise sum f_r, then g.  Returns dict(N, O, Oprime, K) like round_ (N = the summed counts)."""
+    shards = [_u64(p) for p in shards]
+    K = _u64(K)
+    nl = K.size - 1
+    if cap is None:
+        cap = 8 * nl
+    Pall = np.concatenate(shards) if shards else np.empty(0, dtype=np.uint64)
+    start = np.zeros(len(shards) + 1, dtype=np.uint64)
+    start[1:] = np.cumsum([p.size for p in shards])
+    N = np.empty(nl, dtype=np.uint32)
+    O = np.empty(nl, dtype=np.uint32)
+    Op = np.empty(nl + 1, dtype=np.uint32)
+    Kout = np.empty(cap + 1, dtype=np.uint64)
+    nn = lib().orc_global_round(_p(Pall), _p(start), C.c_uint32(len(shards)), _p(K), C.c_uint32(nl),
+                                C.c_uint32(bucket_size), _p(N), _p(O), _p(Op), _p(Kout), C.c_uint32(cap))
+    return {"N": N, "O": O, "Oprime": Op, "K": None if nn < 0 else Kout[:nn + 1].copy()}
+
+
+def partition(counts, n_ranks):
+    """O12: leaf-index bounds b_0 = 0 <= ... <= b_{n_ranks} = n_l of the SFC domain decomposition (reading A29)."""
+    counts = _u32(counts)
+    out = np.empty(n_ranks + 1, dtype=np.uint32)
+    lib().orc_partition(_p(counts), C.c_uint32(counts.size), C.c_uint32(n_ranks), _p(out))
+    return out
+
+
 def leaves_iterative(P, bucket_size, K_start=None, max_rounds=0, cap=None):
     """O5b: iterate f, g from K_start (default: the root {0, 8^21}).
 
     Returns (K, counts, rounds, converged)."""
     P = _u64(P)
     if K_start is None:
-        K_start = np.array([0, KEY_END], dtype=np.uint64)
+        K_start = np.array([0, 1 << (3 * L)], dtype=np.uint64)
     K_start = _u64(K_start)
     user_cap = cap is not None
     if cap is None:
@@ -175,10 +245,10 @@ def node_counts(leaf_counts, tree):
     return first, count
 
 
-def full_build(x, y, z, bucket_size):
+def full_build(x, y, z, bucket_size, curve="morton"):
     """The whole path, stage by stage; returns a dict with every array."""
     b = box(x, y, z)
-    k = keys(x, y, z, b)
+    k = keys(x, y, z, b) if curve == "morton" else hilbert_keys(x, y, z, b)
     P, perm = sort(k)
     K, counts = leaves_topdown(P, bucket_size)
     tree = link(K)

@@ -14,9 +14,12 @@
 //
 // Every function cites the PAPER.md passage it follows; readings of silent or garbled
 // passages are the "A<n>" items of DESIGN.md ("Readings of the paper").
-// Parity pins: tests/test_oracle_*.py (all functions here are pinned; nothing is
-// "parity unpinned").  O8-O10 (node properties, the first row past the hot path) are pinned in
-// tests/test_oracle_props.py.
+// Parity pins: tests/test_oracle_*.py (every function here is pinned).  O8-O10 (node properties, the
+// first row past the hot path) are pinned in tests/test_oracle_props.py; O2h (Hilbert keys), the
+// L = 10 setting, O11 (one round of the distributed build) and O12 (SFC domain decomposition) in
+// tests/test_oracle_next.py.  PARITY UNPINNED: which 3D Hilbert curve the paper's own code walks --
+// the paper names none (its reference [11] lists millions); O2h's pins fix the properties the paper
+// relies on (bijection, face-continuity, octant by octant), not that choice (reading A28).
 // =====================================================================================
 #include <algorithm>
 #include <cmath>
@@ -26,8 +29,10 @@
 
 namespace {
 
-constexpr int L = 21;                       // octree depth of a 64-bit key
-constexpr uint64_t KEY_END = 1ull << 63;    // 8^L, PAPER.md:66 (Eq. 2)
+// Octree depth a key resolves: "reasonable choices for L are 10 or 21" (32- or 64-bit keys).
+// 21 unless orc_set_L changes it; keys are held in uint64_t either way (a key of L octal digits is < 8^L).
+int L = 21;
+#define KEY_END (1ull << (3 * L))           /* 8^L, PAPER.md:66 (Eq. 2) */
 
 // length of the key range of a node at division level l: 8^(L-l)
 inline uint64_t nodeRange(int level) { return 1ull << (3 * (L - level)); }
@@ -35,6 +40,15 @@ inline uint64_t nodeRange(int level) { return 1ull << (3 * (L - level)); }
 }  // namespace
 
 extern "C" {
+
+// L = 10 (30-bit keys) or 21 (63-bit keys); returns the previous value, or -1 if refused.
+int orc_set_L(int newL)
+{
+    if (newL < 1 || newL > 21) return -1;
+    const int old = L;
+    L = newL;
+    return old;
+}
 
 // -------------------------------------------------------------------------------------
 // O1  bounding box.  The paper is silent (it starts from grid coordinates,
@@ -59,20 +73,21 @@ int orc_box(const double* x, const double* y, const double* z, uint64_t n, doubl
 }
 
 // -------------------------------------------------------------------------------------
-// O2  64-bit Morton keys, 21 bits per dimension.  PAPER.md:54-60 (Sec. 3, Eq. 1): the
-// key is L octal digits, digit i selecting the octant at division level i.
+// O2  Morton keys, L bits per dimension (L = 21: 63-bit keys; L = 10: 30-bit keys).
+// (Sec. 3, Eq. 1): the key is L octal digits, digit i selecting the octant at division level i.
 // Grid coordinate (north_star; readings A2, A3):
-//     g = clamp(floor(((c - lo) / (hi - lo)) * 2^21), 0, 2^21 - 1)
+//     g = clamp(floor(((c - lo) / (hi - lo)) * 2^L), 0, 2^L - 1)
 // evaluated in binary64, one rounding per operation, in exactly this order.
-// Octal digit = 4*xbit + 2*ybit + zbit; key bit 62 is x bit 20; bit 63 is 0.
+// Octal digit = 4*xbit + 2*ybit + zbit; key bit 3L-1 is x bit L-1; higher bits are 0.
 // -------------------------------------------------------------------------------------
 static uint32_t gridCoordinate(double c, double lo, double e)
 {
+    const double cells = (double)(1u << L);   // 2^L, exact
     double t = (c - lo) / e;
-    t = t * 2097152.0;
+    t = t * cells;
     double g = std::floor(t);
     if (!(g >= 0.0)) g = 0.0;            // negatives and NaN (0/0 for a flat box, A1)
-    if (g > 2097151.0) g = 2097151.0;    // c == hi gives exactly 2^21
+    if (g > cells - 1.0) g = cells - 1.0;   // c == hi gives exactly 2^L
     return (uint32_t)g;
 }
 
@@ -93,6 +108,61 @@ void orc_keys(const double* x, const double* y, const double* z, uint64_t n, con
         }
         keys[i] = k;
     }
+}
+
+// -------------------------------------------------------------------------------------
+// O2h  Hilbert keys ("a 3D version of the Hilbert curve [11, 13]", "any type of SFC that
+// traverses a cube octant by octant"; Table 1 has rows for it).  The paper gives no encoding and its
+// reference [11] is an inventory of millions of 3D Hilbert curves, so the curve is a choice: reading A28
+// takes the curve of the Butz algorithm in Hamilton's formulation ("compact Hilbert indices"), n = 3:
+//   gc(i) = i xor (i >> 1)                         the reflected Gray code: order of the octants in a cube
+//   e(w)  = 0 if w = 0, else gc(2 floor((w-1)/2))  entry corner of the w-th sub-cube
+//   d(w)  = 0 if w = 0, else tsb(w-1) mod 3 (w even), tsb(w) mod 3 (w odd), tsb = number of trailing 1 bits:
+//           axis along which the curve leaves the w-th sub-cube
+//   T_(e,d)(b) = (b xor e) rotated right by d+1 bits (within 3 bits)
+// and, level by level from the most significant bit, with l = 4 xbit + 2 ybit + zbit (as A3):
+//   l' = T_(e,d)(l);  w = gc^-1(l');  key = 8 key + w;  e = e xor rotl(e(w), d+1);  d = (d + d(w) + 1) mod 3.
+// The grid coordinates are those of O2.  orc_hilbert_from_grid encodes integer grid points of an m-level
+// grid (pins on small grids); orc_hilbert_keys takes coordinates and the box, m = L.
+// -------------------------------------------------------------------------------------
+namespace {
+inline unsigned gc3(unsigned i) { return i ^ (i >> 1); }
+inline unsigned gc3inv(unsigned g) { unsigned i = g; i ^= i >> 1; i ^= i >> 2; return i & 7u; }
+inline unsigned tsb(unsigned i) { unsigned c = 0; while (i & 1u) { ++c; i >>= 1; } return c; }
+inline unsigned rotr3(unsigned b, unsigned r) { r %= 3; return ((b >> r) | (b << (3 - r))) & 7u; }
+inline unsigned rotl3(unsigned b, unsigned r) { r %= 3; return ((b << r) | (b >> (3 - r))) & 7u; }
+inline unsigned entry3(unsigned w) { return w == 0 ? 0u : gc3(2 * ((w - 1) / 2)); }
+inline unsigned dir3(unsigned w) { return w == 0 ? 0u : ((w % 2 == 0) ? tsb(w - 1) % 3 : tsb(w) % 3); }
+
+uint64_t hilbertOfGrid(uint32_t gx, uint32_t gy, uint32_t gz, int m)
+{
+    uint64_t key = 0;
+    unsigned e = 0, d = 0;
+    for (int i = m - 1; i >= 0; --i) {
+        unsigned l = 4u * ((gx >> i) & 1u) + 2u * ((gy >> i) & 1u) + ((gz >> i) & 1u);
+        l = rotr3(l ^ e, d + 1);
+        const unsigned w = gc3inv(l);
+        key = 8 * key + w;
+        e = e ^ rotl3(entry3(w), d + 1);
+        d = (d + dir3(w) + 1) % 3;
+    }
+    return key;
+}
+}  // namespace
+
+void orc_hilbert_from_grid(const uint32_t* gx, const uint32_t* gy, const uint32_t* gz, uint64_t n, int m, uint64_t* keys)
+{
+    for (uint64_t i = 0; i < n; ++i) keys[i] = hilbertOfGrid(gx[i], gy[i], gz[i], m);
+}
+
+void orc_hilbert_keys(const double* x, const double* y, const double* z, uint64_t n, const double* box6, uint64_t* keys)
+{
+    const double ex = box6[1] - box6[0];
+    const double ey = box6[3] - box6[2];
+    const double ez = box6[5] - box6[4];
+    for (uint64_t i = 0; i < n; ++i)
+        keys[i] = hilbertOfGrid(gridCoordinate(x[i], box6[0], ex), gridCoordinate(y[i], box6[2], ey),
+                                gridCoordinate(z[i], box6[4], ez), L);
 }
 
 // -------------------------------------------------------------------------------------
@@ -127,11 +197,10 @@ void orc_sort(const uint64_t* keysIn, uint64_t n, uint64_t* keysOut, uint32_t* p
 // K has nl+1 entries.  N (nl), O (nl), Oprime (nl+1) are outputs (may be null).
 // Kout must hold capOut+1 entries.  Returns the new leaf count, or -1 if > capOut.
 // -------------------------------------------------------------------------------------
-int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl, uint32_t bucketSize,
-                  uint32_t* N, uint32_t* O, uint32_t* Oprime, uint64_t* Kout, uint32_t capOut)
+namespace {
+// f (Eq. 3): literal per-leaf counting with a moving cursor over the sorted keys P
+void countF(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl, std::vector<uint32_t>& Nv)
 {
-    std::vector<uint32_t> Nv(nl), Ov(nl), Op(nl + 1);
-    // f: literal per-leaf counting
     uint64_t cur = 0;
     for (uint32_t i = 0; i < nl; ++i) {
         while (cur < n && P[cur] < K[i]) ++cur;    // keys below K_0 = 0 do not exist
@@ -139,6 +208,13 @@ int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl,
         while (cur < n && P[cur] < K[i + 1]) { ++cur; ++c; }
         Nv[i] = (uint32_t)c;
     }
+}
+
+// g = g3 o g2 o g1 (Eqs. 4-9) from the counts Nv.  Returns the new leaf count, or -1 if > capOut.
+int64_t rebalanceG(const uint64_t* K, uint32_t nl, uint32_t bucketSize, const std::vector<uint32_t>& Nv,
+                   uint32_t* O, uint32_t* Oprime, uint64_t* Kout, uint32_t capOut)
+{
+    std::vector<uint32_t> Ov(nl), Op(nl + 1);
     // g1
     for (uint32_t i = 0; i < nl; ++i) {
         uint64_t delta = K[i + 1] - K[i];
@@ -158,7 +234,6 @@ int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl,
     uint64_t run = 0;
     for (uint32_t i = 0; i < nl; ++i) { Op[i] = (uint32_t)run; run += Ov[i]; }
     Op[nl] = (uint32_t)run;
-    if (N) std::copy(Nv.begin(), Nv.end(), N);
     if (O) std::copy(Ov.begin(), Ov.end(), O);
     if (Oprime) std::copy(Op.begin(), Op.end(), Oprime);
     if (run > capOut) return -1;
@@ -172,6 +247,59 @@ int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl,
     }
     Kout[run] = KEY_END;
     return (int64_t)run;
+}
+}  // namespace
+
+int64_t orc_round(const uint64_t* P, uint64_t n, const uint64_t* K, uint32_t nl, uint32_t bucketSize,
+                  uint32_t* N, uint32_t* O, uint32_t* Oprime, uint64_t* Kout, uint32_t capOut)
+{
+    std::vector<uint32_t> Nv(nl);
+    countF(P, n, K, nl, Nv);
+    if (N) std::copy(Nv.begin(), Nv.end(), N);
+    return rebalanceG(K, nl, bucketSize, Nv, O, Oprime, Kout, capOut);
+}
+
+// -------------------------------------------------------------------------------------
+// O11  one round of the distributed build, Sec. 6 (Eq. 11): the particles'
+// sorted keys are spread over R ranks, shard r = Pall[shardStart[r] .. shardStart[r+1]) (each shard
+// sorted on its own).  f_glob = f_r o f: every rank counts its own shard (f, Eq. 3), f_r is the
+// element-wise sum of the R count arrays ("a single call to MPI_Allreduce"), then g is applied to
+// the summed counts, identically on every rank.  Nglob (nl) receives the summed counts.
+// -------------------------------------------------------------------------------------
+int64_t orc_global_round(const uint64_t* Pall, const uint64_t* shardStart, uint32_t R, const uint64_t* K, uint32_t nl,
+                         uint32_t bucketSize, uint32_t* Nglob, uint32_t* O, uint32_t* Oprime, uint64_t* Kout,
+                         uint32_t capOut)
+{
+    std::vector<uint32_t> sum(nl, 0), Nr(nl);
+    for (uint32_t r = 0; r < R; ++r) {
+        countF(Pall + shardStart[r], shardStart[r + 1] - shardStart[r], K, nl, Nr);   // f on rank r
+        for (uint32_t i = 0; i < nl; ++i) sum[i] += Nr[i];                            // f_r
+    }
+    if (Nglob) std::copy(sum.begin(), sum.end(), Nglob);
+    return rebalanceG(K, nl, bucketSize, sum, O, Oprime, Kout, capOut);
+}
+
+// -------------------------------------------------------------------------------------
+// O12  SFC domain decomposition: "The global domain can then be partitioned into
+// n_ranks subdomains by grouping K into n_ranks bins of consecutive leaves such that each bin contains
+// approximately N_tot / n_ranks of the total particle count."  The paper gives no rule for
+// "approximately"; reading A29: with C_i = N_0 + ... + N_{i-1}, bin r = leaves [b_r, b_{r+1}), b_0 = 0,
+// b_{n_ranks} = n_l, and for 0 < r < n_ranks b_r is the first leaf boundary i with
+// C_i * n_ranks >= r * N_tot (the first boundary at or past the ideal split r N_tot / n_ranks, compared
+// in exact integer arithmetic).  bounds has nRanks + 1 entries; rank r owns keys [K[b_r], K[b_{r+1}]).
+// -------------------------------------------------------------------------------------
+void orc_partition(const uint32_t* N, uint32_t nl, uint32_t nRanks, uint32_t* bounds)
+{
+    uint64_t total = 0;
+    for (uint32_t i = 0; i < nl; ++i) total += N[i];
+    bounds[0] = 0;
+    uint64_t C = 0;          // C_i
+    uint32_t i = 0;
+    for (uint32_t r = 1; r < nRanks; ++r) {
+        while (i < nl && (unsigned __int128)C * nRanks < (unsigned __int128)r * total) { C += N[i]; ++i; }
+        bounds[r] = i;
+    }
+    bounds[nRanks] = nl;
 }
 
 // -------------------------------------------------------------------------------------
