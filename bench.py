@@ -330,6 +330,55 @@ def run_ours(args):
         stages_roofline[k] = {"ms": stages[k], "mparticles_per_s": n / (stages[k] * 1e-3) / 1e6 if stages[k] > 0 else None,
                               "share_of_step": stages[k] / ms_instrumented}
 
+    # ---- H4-H7 as kernels (the default build reaches the fixpoint in one pass and never runs them): the same sorted
+    # keys through the literal rounds f, g1, g2, g3 from {0, 8^21} (CS_LEAVES_ITERATIVE), and the update of PAPER.md:126:
+    # every particle displaced by a seeded Gaussian step, full rebuild starting from the previous leaf array
+    def timed_ms(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); out = fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.mean(ts)), out
+
+    leaves_iterative = None
+    update = None
+    if not args.no_rounds:
+        reps = max(3, min(args.steps, 10))
+        P = tree["keys"]
+        lv, ct = torch.empty_like(bufs.t["leaves"]), torch.empty_like(bufs.t["counts"])
+        t_direct, _ = timed_ms(lambda: cs.buildLeaves(ctx, P, bucket, leaves=lv, counts=ct), reps)
+        ctx.setLeafMode(cs.LEAVES_ITERATIVE)
+        t_iter, it = timed_ms(lambda: cs.buildLeaves(ctx, P, bucket, leaves=lv, counts=ct), reps)
+        ctx.setLeafMode(cs.LEAVES_AUTO)
+        leaves_iterative = {"ms": t_iter, "rounds": it[2], "one_pass_ms": t_direct,
+                            "what": "cs_buildLeaves on the sorted keys of the step, from {0, 8^21}: rounds of f, g1, g2, g3 "
+                                    "(one cooperative launch) vs the default one-pass fixpoint; both include the call's "
+                                    "read-back of sizes"}
+        del lv, ct
+        from paper_2307_06345_b200.workloads import displace
+        sigma = cfg.step_sigma or 1e-3
+        x1, y1, z1 = displace(x, y, z, sigma, cfg_rank.seed + 1000)
+        d1 = [torch.from_numpy(a).cuda() for a in (x1, y1, z1)]
+        prev = tree["leaves"].clone()
+        nl0 = tree["numLeaves"]
+        ctx.setProfiling(True)
+        t_upd, tr1 = timed_ms(lambda: cs.buildOctree(ctx, d1[0], d1[1], d1[2], bucket, buffers=bufs, prevLeaves=prev), reps)
+        st_upd = ctx.stageTimes()
+        t_scr, tr2 = timed_ms(lambda: cs.buildOctree(ctx, d1[0], d1[1], d1[2], bucket, buffers=bufs), reps)
+        st_scr = ctx.stageTimes()
+        ctx.setProfiling(False)
+        update = {"sigma": sigma, "ms_per_rebuild_from_prev_leaves": t_upd, "ms_per_build_from_scratch": t_scr,
+                  "leaves_stage_ms_from_prev_leaves": st_upd["leaves"], "leaves_stage_ms_one_pass": st_scr["leaves"],
+                  "rounds": tr1["rounds"], "leaves_before": nl0, "leaves_after": tr1["numLeaves"],
+                  "what": "box + keys + sort + buildLeaves(previous leaves) + link + counts on the displaced particles "
+                          "(stage timers on), against the same build from {0, 8^21}"}
+        tree = cs.buildOctree(ctx, dx, dy, dz, bucket, buffers=bufs)     # restore the step's tree for what follows
+        del d1, x1, y1, z1, prev
+
     # ---- incremental rebuilds (config 5's recipe: displace every particle, rebuild from the previous leaves) ---
     incremental = None
     if args.rebuilds and cfg.incremental_steps:
@@ -403,7 +452,8 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (1.5 GiB of coordinates per step at N=2^26)",
                    "input_checksum_first_1Mi": in_sum},
         "roofline": roofline, "full_build": full_build, "cpu_baseline": cpu, "e2e": e2e,
-        "stages_roofline": stages_roofline, "incremental": incremental, "node_properties": props,
+        "stages_roofline": stages_roofline, "leaves_iterative": leaves_iterative, "incremental": update,
+        "incremental_rebuilds": incremental, "node_properties": props,
         "gpu_launches": int(launches), "stages_ms": stages, "ms_per_step_with_stage_timers": ms_instrumented,
         "clocks": clocks.summary(),
     }
@@ -426,6 +476,8 @@ def main():
                     help="after the timed builds, time this many incremental rebuilds (workloads with a step recipe: c5)")
     ap.add_argument("--props", action="store_true",
                     help="also time the node-property kernels on the finished tree (reported beside the step)")
+    ap.add_argument("--no-rounds", action="store_true",
+                    help="skip the extra legs that time the leaf rounds (H4-H7) and the incremental update")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -101,6 +101,21 @@ cs_status cs_computeBox(cs_context* ctx, const double* x, const double* y, const
 cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
                          const double* box6, uint64_t* keys, void* stream);
 
+/* cs_computeKeysHilbert -- keys on a 3D Hilbert curve instead of the Morton Z-curve (Table 1
+ *   has rows for both).  Same grid coordinates g_d as cs_computeKeys; the key is again 21 octal digits and its
+ *   first i digits name the level-i cell that holds the particle ("any type of SFC that traverses a cube octant
+ *   by octant"), so cs_sortKeys, cs_buildLeaves, cs_linkOctree and cs_nodeCounts apply unchanged.
+ *   The paper gives no encoding; reading A28 takes the curve of the Butz algorithm in Hamilton's
+ *   formulation: octants of a cube in reflected-Gray-code order, sub-cube w entered at corner e(w) and left
+ *   along axis d(w).  Cells of consecutive keys share a face.  Arguments and errors as cs_computeKeys.
+ *   (cs_nodeGeometry decodes Morton prefixes only.) */
+cs_status cs_computeKeysHilbert(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                                const double* box6, uint64_t* keys, void* stream);
+
+/* cs_setCurve -- the curve cs_buildOctree / cs_buildOctreeHost compute their keys on (default CS_CURVE_MORTON). */
+enum { CS_CURVE_MORTON = 0, CS_CURVE_HILBERT = 1 };
+cs_status cs_setCurve(cs_context* ctx, int curve);
+
 /* cs_sortKeys -- stable ascending radix sort of the keys, carrying the particle index
  *   ("keys ... and the identity permutation as values"; A5).
  *   keys: dev, in: n keys < 2^63 in any order, out: sorted.  perm: dev, n uint32 out,
@@ -139,7 +154,12 @@ int cs_sortPasses(const cs_context* ctx);
  *   the returned leaves (capacity leafCapacity).  numLeaves, rounds: host out (rounds counts
  *   f evaluations including the confirming one).  Synchronises `stream`.
  *   Errors: CAPACITY if a round would exceed leafCapacity or the context's maxLeaves
- *   (leaves / counts are then left untouched), NOT_CORNERSTONE, INVALID_ARG, CUDA.
+ *   (leaves / counts are then left untouched when the build started from the root; with prevLeaves
+ *   they may hold the array of an earlier round), NOT_CORNERSTONE, INVALID_ARG, CUDA.
+ *   Cost: from the root (default mode) one pass over sortedKeys.  With prevLeaves: one merge pass over
+ *   sortedKeys and prevLeaves that locates every previous K_i (Eq. 3), then the rounds, all in one
+ *   cooperative launch that ends with the first round that changes nothing: a small time step costs
+ *   one update and the confirming round.
  */
 cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, uint32_t bucketSize,
                          const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds,

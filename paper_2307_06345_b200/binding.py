@@ -27,6 +27,7 @@ NO_LEAF = 0xFFFFFFFF
 NUM_STAGES = 9
 STAGE_NAMES = ("box", "keys", "sort", "leaves", "link", "counts", "sort_hist", "sort_passes", "sort_fixup")
 
+CURVE_MORTON, CURVE_HILBERT = 0, 1
 LEAVES_AUTO, LEAVES_ITERATIVE = 0, 1
 SORT_AUTO, SORT_PLAIN = 0, 1
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_NOT_CORNERSTONE, ERR_NOT_CONVERGED, ERR_CUDA = range(6)
@@ -81,6 +82,8 @@ def lib():
         "cs_sortPasses": (C.c_int, [vp]),
         "cs_computeBox": (C.c_int, [vp, vp, vp, vp, u64, vp, vp]),
         "cs_computeKeys": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
+        "cs_computeKeysHilbert": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
+        "cs_setCurve": (C.c_int, [vp, C.c_int]),
         "cs_sortKeys": (C.c_int, [vp, vp, vp, u64, vp]),
         "cs_buildLeaves": (C.c_int, [vp, vp, u64, u32, vp, u32, u32, vp, vp, u32, C.POINTER(u32), C.POINTER(u32), vp]),
         "cs_linkOctree": (C.c_int, [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp, u32, C.POINTER(u32), vp]),
@@ -179,6 +182,10 @@ class Context:
         """LEAVES_AUTO (one-pass fixpoint from the root) or LEAVES_ITERATIVE (always the rounds f, g)."""
         self.check(lib().cs_setLeafMode(self.handle, int(mode)))
 
+    def setCurve(self, curve: int):
+        """CURVE_MORTON (default) or CURVE_HILBERT: the curve buildOctree / buildOctreeHost compute keys on."""
+        self.check(lib().cs_setCurve(self.handle, int(curve)))
+
     def setSortMode(self, mode: int):
         """SORT_AUTO (5 passes + fix-up of the low bits, plain passes behind it if needed) or SORT_PLAIN."""
         self.check(lib().cs_setSortMode(self.handle, int(mode)))
@@ -216,6 +223,14 @@ def computeKeys(ctx: Context, x, y, z, box6, keys=None):
         keys = _i64(x.numel(), ctx.device)
     ctx.check(lib().cs_computeKeys(ctx.handle, _ptr(x), _ptr(y), _ptr(z), x.numel(), _ptr(box6), _ptr(keys),
                                    _stream()))
+    return keys
+
+
+def computeKeysHilbert(ctx: Context, x, y, z, box6, keys=None):
+    if keys is None:
+        keys = _i64(x.numel(), ctx.device)
+    ctx.check(lib().cs_computeKeysHilbert(ctx.handle, _ptr(x), _ptr(y), _ptr(z), x.numel(), _ptr(box6), _ptr(keys),
+                                          _stream()))
     return keys
 
 

@@ -7,20 +7,6 @@ using namespace cs;
 
 namespace {
 
-struct DeviceGuard {
-    int prev = -1;
-    explicit DeviceGuard(int dev)
-    {
-        cudaGetDevice(&prev);
-        if (prev != dev) cudaSetDevice(dev);
-        else prev = -1;
-    }
-    ~DeviceGuard()
-    {
-        if (prev >= 0) cudaSetDevice(prev);
-    }
-};
-
 cs_status statusFromCtrl(cs_context* ctx, const char* where)
 {
     const u32 st = ctx->hostCtrl->c.status;
@@ -67,7 +53,27 @@ cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, cons
     if (!x || !y || !z || !box6 || !keys) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeKeys: null pointer");
     CS_TRY(checkParticles(ctx, "cs_computeKeys", n));
     DeviceGuard g(ctx->device);
-    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, (cudaStream_t)stream);
+    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, CS_CURVE_MORTON, (cudaStream_t)stream);
+}
+
+cs_status cs_computeKeysHilbert(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                                const double* box6, uint64_t* keys, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_computeKeysHilbert: ctx is null");
+    if (n == 0) return CS_OK;
+    if (!x || !y || !z || !box6 || !keys) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeKeysHilbert: null pointer");
+    CS_TRY(checkParticles(ctx, "cs_computeKeysHilbert", n));
+    DeviceGuard g(ctx->device);
+    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, CS_CURVE_HILBERT, (cudaStream_t)stream);
+}
+
+cs_status cs_setCurve(cs_context* ctx, int curve)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setCurve: ctx is null");
+    if (curve != CS_CURVE_MORTON && curve != CS_CURVE_HILBERT)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_setCurve: unknown curve %d", curve);
+    ctx->curve = curve;
+    return CS_OK;
 }
 
 cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream)
@@ -202,7 +208,7 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
     // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
-    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), /*withHist=*/true, s));
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), /*withHist=*/true, ctx->curve, s));
     CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
                          (u64*)b->leaves, b->counts, leafCap, s));

@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, divLevel, tileLookback, dirFlags, dirTotals, dirBases, dirListSize, dirListKeys, dirListMeta, linkTileHist, ctrl, total;
+        leafOffFinal, leafTasks, leafOpk, leafTileInfo, divLevel, tileLookback, dirFlags, dirTotals, dirBases, dirListSize, dirListKeys, dirListMeta, linkTileHist, hilbertTable, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -57,7 +57,10 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.leafOff0 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOff1 = take(((size_t)maxLeaves + 2) * sizeof(u32));
     L.leafOffFinal = take(((size_t)maxLeaves + 2) * sizeof(u32));
-    L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint2));   // linear list, search list
+    L.leafTasks = take(2 * ((size_t)maxLeaves / 8 + 8) * sizeof(uint4));   // linear list, search list
+    const size_t roundTiles = ((size_t)maxLeaves + kLeafTile - 1) / kLeafTile + 1;
+    L.leafOpk = take(roundTiles * kLeafBlock * sizeof(u32));
+    L.leafTileInfo = take(roundTiles * sizeof(uint4));
     L.divLevel = take(dirTiles << kDirectTileLog2);                        // 1 byte per particle, whole tiles
     L.tileLookback = take(leafTiles * sizeof(u64));                        // one counter per tile (leaf rounds, scan)
     L.dirFlags = take(dirTiles << (kDirectTileLog2 - 3));                  // one-pass leaf build: 1 bit per position
@@ -67,6 +70,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.dirListKeys = take(dirTiles * kDirectCompact * sizeof(ulonglong2));   // 2 B per particle
     L.dirListMeta = take(dirTiles * kDirectCompact * sizeof(u32));          // 0.5 B per particle
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
+    L.hilbertTable = take(24 * 64 * sizeof(unsigned short));
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
     return L;
@@ -74,17 +78,23 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
 
 constexpr int kBoxGridMax = 148 * 8;
 
-u32 nextEpoch(cs_context* ctx, cudaStream_t s)
+// Look-back words carry the epoch of the launch that wrote them, so the arrays are never cleared between
+// launches; only when the 30-bit epoch counter would wrap are they zeroed once (epoch 0 is never handed out).
+u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s)
 {
-    ctx->epoch++;
-    if (ctx->epoch >= (1u << 30)) {   // wrap: clear every look-back array once
+    if (ctx->epoch + count >= (1u << 30)) {
         Layout L = makeLayout(ctx->maxParticles, ctx->maxLeaves, kBoxGridMax);
-        cudaMemsetAsync(ctx->sortLookback, 0, L.boxPartials - L.sortLookback, s);
-        cudaMemsetAsync(ctx->tileLookback, 0, L.dirFlags - L.tileLookback, s);
-        ctx->epoch = 1;
+        cudaError_t e = cudaMemsetAsync(ctx->sortLookback, 0, L.boxPartials - L.sortLookback, s);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctx->tileLookback, 0, L.dirFlags - L.tileLookback, s);
+        if (e != cudaSuccess) cudaFail(ctx, e, "reserveEpochs (look-back reset)");   // the next launch check reports it
+        ctx->epoch = 0;
     }
-    return ctx->epoch;
+    const u32 first = ctx->epoch + 1;
+    ctx->epoch += count;
+    return first;
 }
+
+u32 nextEpoch(cs_context* ctx, cudaStream_t s) { return reserveEpochs(ctx, 1, s); }
 
 cs_status readCtrl(cs_context* ctx, cudaStream_t s)
 {
@@ -189,7 +199,8 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->maxParticles = maxParticles;
     ctx->maxLeaves = maxLeaves;
     ctx->maxNodes = maxLeaves + (maxLeaves - 1) / 7 + 1;
-    cudaError_t e = cudaSetDevice(device);
+    DeviceGuard guard(device);                 // the caller's current device is restored on return
+    cudaError_t e = guard.err;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->numSMs, cudaDevAttrMultiProcessorCount, device);
     Layout L = makeLayout(maxParticles, maxLeaves, kBoxGridMax);
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slab, L.total);
@@ -217,7 +228,9 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->leafOff[0] = (u32*)(ctx->slab + L.leafOff0);
     ctx->leafOff[1] = (u32*)(ctx->slab + L.leafOff1);
     ctx->leafOffFinal = (u32*)(ctx->slab + L.leafOffFinal);
-    ctx->leafTasks = (uint2*)(ctx->slab + L.leafTasks);
+    ctx->leafTasks = (uint4*)(ctx->slab + L.leafTasks);
+    ctx->leafOpk = (u32*)(ctx->slab + L.leafOpk);
+    ctx->leafTileInfo = (uint4*)(ctx->slab + L.leafTileInfo);
     ctx->divLevel = (unsigned char*)(ctx->slab + L.divLevel);
     ctx->maxTasks = maxLeaves / 8 + 8;
     ctx->tileLookback = (u64*)(ctx->slab + L.tileLookback);
@@ -229,8 +242,20 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->dirListMeta = (u32*)(ctx->slab + L.dirListMeta);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
+    ctx->hilbertTable = (unsigned short*)(ctx->slab + L.hilbertTable);
+    {
+        unsigned short table[24 * 64];
+        hilbertBuildTable(table);
+        e = cudaMemcpy(ctx->hilbertTable, table, sizeof(table), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            cs_status stc = cudaFail(nullptr, e, "cs_create (Hilbert table)");
+            cs_destroy(ctx);
+            return stc;
+        }
+    }
     cs_status st = sortInit(ctx);
     if (st == CS_OK) st = leavesDirectInit(ctx);
+    if (st == CS_OK) st = leavesInit(ctx);
     if (st != CS_OK) {
         cs_destroy(ctx);
         return st;
@@ -242,7 +267,7 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
 void cs_destroy(cs_context* ctx)
 {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    DeviceGuard guard(ctx->device);
     if (ctx->slab) cudaFree(ctx->slab);
     if (ctx->hostPathSlab) cudaFree(ctx->hostPathSlab);
     if (ctx->hostCtrl) cudaFreeHost(ctx->hostCtrl);

@@ -113,6 +113,10 @@ struct cs_context {
     cs::u32 epoch = 0;                 // look-back epoch, bumped per launch that uses a look-back array
     bool sortPlain = false;            // run the 7 plain radix passes (set once a build needed the redo, or by cs_setSortMode)
 
+    // keys
+    unsigned short* hilbertTable = nullptr;   // [24][64] two-level transitions of the Hilbert curve (cs_particles.cu)
+    int curve = CS_CURVE_MORTON;              // cs_setCurve: the curve cs_buildOctree computes keys on
+
     // box
     double* boxPartials = nullptr;     // [grid][6]
     cs::u32* boxCounter = nullptr;
@@ -120,12 +124,14 @@ struct cs_context {
     // leaves
     cs::u64* leafK[2] = {nullptr, nullptr};
     cs::u32* leafOff[2] = {nullptr, nullptr};
-    unsigned char* divLevel = nullptr; // iterative path: D[i] = (digits shared by P[i-1], P[i]) << 3 | next digit;
-                                       // one-pass build: d_j = level of the deepest internal node above particle j
-    uint2* leafTasks = nullptr;        // (first child slot, end of the parent's particle range) per split leaf
+    unsigned char* divLevel = nullptr; // one-pass build: d_j = level of the deepest internal node above particle j
+    uint4* leafTasks = nullptr;        // (first child slot, particle range, shift of the child digit) per split leaf
     cs::u32 maxTasks = 0;
     cs::u32* leafOffFinal = nullptr;   // off[] of the returned leaves (prefix sum of counts), n_l + 1 entries
     cs::u64* tileLookback = nullptr;   // [tiles] look-back words of the leaf rounds and the scan
+    cs::u32* leafOpk = nullptr;        // [leaf tiles][kLeafBlock] rounds: O of 8 leaves per word (decide -> scatter phase)
+    uint4* leafTileInfo = nullptr;     // [leaf tiles] rounds: sum of O, split leaves per tile
+    cs::u32 roundsGrid = 0;            // CTAs of leafRoundsKernel that are resident together (cooperative launch)
     unsigned char* dirFlags = nullptr; // one-pass leaf build: bit j set <=> position j owns entries of K
     cs::u32* dirTotals = nullptr;      // [tiles] K entries owned by the positions of a tile
     cs::u32* dirBases = nullptr;       // [tiles + 1] exclusive prefix of dirTotals
@@ -173,6 +179,21 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what);
         if (e__ != cudaSuccess) return ::cs::cudaFail((ctx), e__, name);       \
     } while (0)
 
+struct DeviceGuard {              // makes `dev` current for the scope and restores the caller's device
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev)
+    {
+        cudaGetDevice(&prev);
+        if (prev != dev) err = cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
 struct StageTimer {               // records CUDA events around a stage when profiling is on
     cs_context* ctx; int stage; cudaStream_t s;
     StageTimer(cs_context* c, int st, cudaStream_t stream) : ctx(c), stage(st), s(stream)
@@ -187,15 +208,18 @@ struct StageTimer {               // records CUDA events around a stage when pro
 
 inline u32 divUp(u64 a, u64 b) { return (u32)((a + b - 1) / b); }
 u32 nextEpoch(cs_context* ctx, cudaStream_t s);
+u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s);   // first of `count` consecutive look-back epochs
 
 // ---- stage enqueue functions (no synchronisation; sizes device-resident) ---------------
 cs_status enqueueBox(cs_context*, const double* x, const double* y, const double* z, u64 n, double* box6,
                      cudaStream_t);
 // withHist: also accumulate the 8 digit histograms of the radix sort into ctx->sortHist
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, bool withHist, cudaStream_t);
+                      u64* keys, bool withHist, int curve, cudaStream_t);
+void hilbertBuildTable(unsigned short* table /*[24 * 64], host*/);
 cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
 cs_status leavesDirectInit(cs_context*);
+cs_status leavesInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
 u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
 cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t);

@@ -236,6 +236,63 @@ __device__ __forceinline__ u64 mortonKey(double x, double y, double z, const Box
     return ((u64)hi << 32) | lo;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Hilbert keys (reading A28: the curve of the Butz algorithm in Hamilton's
+// formulation).  The curve walks every cube octant by octant, so a Hilbert key is the Morton key
+// re-labelled digit by digit: the octant taken at a level (the Morton digit, 4x + 2y + z) and the
+// orientation of the curve in the current cube (its entry corner e and exit axis d: 8 x 3 = 24 states)
+// give the Hilbert digit and the orientation in the sub-cube.  Two levels are resolved per table
+// look-up: hilbertTable[state][6 Morton bits] = 6 Hilbert bits | next state << 6 (24 x 64 entries of 16
+// bits, 3 KB, staged in shared memory).  21 levels = a leading zero digit + 21 digits = 11 pairs; the
+// start state (e = 0, d = 2) is the one that the zero digit turns into the curve's initial orientation
+// (e = 0, d = 0).
+// The table is generated on the host when a context is created, from the curve's definition:
+//   gc(i) = i ^ (i >> 1);  e(w) = 0 (w = 0), gc(2 floor((w - 1) / 2));  d(w) = 0 (w = 0), tsb(w - 1) mod 3
+//   (w even), tsb(w) mod 3 (w odd);  in state (e, d) octant l is the w-th of the cube, w = gc^-1(rotr3(l ^ e,
+//   d + 1)), and its sub-cube has state (e ^ rotl3(e(w), d + 1), (d + d(w) + 1) mod 3).
+// ---------------------------------------------------------------------------------------------
+constexpr int kHilbertStates = 24;
+constexpr u32 kHilbertStart = 0 * 3 + 2;        // state index = 3 e + d
+
+static void hilbertStep(u32 state, u32 l, u32& w, u32& next)
+{
+    auto rot = [](u32 b, u32 r, bool left) {
+        r %= 3;
+        return (left ? ((b << r) | (b >> (3 - r))) : ((b >> r) | (b << (3 - r)))) & 7u;
+    };
+    auto trailingOnes = [](u32 i) { u32 c = 0; for (; i & 1u; i >>= 1) ++c; return c; };
+    const u32 e = state / 3, d = state % 3;
+    const u32 t = rot(l ^ e, d + 1, false);
+    w = t ^ (t >> 1) ^ (t >> 2);                                       // inverse Gray code on 3 bits
+    const u32 ew = w == 0 ? 0u : (2 * ((w - 1) / 2)) ^ ((2 * ((w - 1) / 2)) >> 1);
+    const u32 dw = w == 0 ? 0u : ((w & 1u) ? trailingOnes(w) % 3 : trailingOnes(w - 1) % 3);
+    next = (e ^ rot(ew, d + 1, true)) * 3 + (d + dw + 1) % 3;
+}
+
+void hilbertBuildTable(unsigned short* table /*[24 * 64]*/)
+{
+    for (u32 s = 0; s < (u32)kHilbertStates; ++s)
+        for (u32 o = 0; o < 64; ++o) {
+            u32 w1, s1, w2, s2;
+            hilbertStep(s, o >> 3, w1, s1);
+            hilbertStep(s1, o & 7u, w2, s2);
+            table[s * 64 + o] = (unsigned short)((w1 << 3) | w2 | (s2 << 6));
+        }
+}
+
+__device__ __forceinline__ u64 hilbertFromMorton(u64 m, const unsigned short* __restrict__ tab)
+{
+    u32 ent = tab[kHilbertStart * 64 + (u32)(m >> 60)];               // (0, first digit)
+    u64 h = ent & 63u;
+#pragma unroll
+    for (int p = 1; p <= 10; ++p) {
+        const u32 o = (u32)(m >> (60 - 6 * p)) & 63u;
+        ent = tab[(ent >> 6) * 64 + o];
+        h = (h << 6) | (ent & 63u);
+    }
+    return h;
+}
+
 template <bool HIST>
 __device__ __forceinline__ void histAdd(u32* sh, u64 key)
 {
@@ -246,18 +303,26 @@ __device__ __forceinline__ void histAdd(u32* sh, u64 key)
     }
 }
 
-template <bool VEC, bool HIST>
+template <bool VEC, bool HIST, bool HILBERT>
 __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
                                                          const double* __restrict__ z, u64 n,
                                                          const double* __restrict__ box6, u64* __restrict__ keys,
-                                                         u32* gHist)
+                                                         u32* gHist, const unsigned short* __restrict__ hilbertTable)
 {
     __shared__ u32 sh[HIST ? kSortPasses * kRadix : 1];
+    __shared__ unsigned short sTab[HILBERT ? kHilbertStates * 64 : 1];
     if (HIST) {
         for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) sh[i] = 0;
-        __syncthreads();
     }
+    if (HILBERT) {
+        for (int i = threadIdx.x; i < kHilbertStates * 64; i += kKeysBlock) sTab[i] = hilbertTable[i];
+    }
+    if (HIST || HILBERT) __syncthreads();
     const BoxParams b = loadBox(box6);
+    auto sfcKey = [&](double px, double py, double pz) -> u64 {
+        const u64 m = mortonKey(px, py, pz, b);
+        return HILBERT ? hilbertFromMorton(m, sTab) : m;
+    };
     const u64 tid = (u64)blockIdx.x * kKeysBlock + threadIdx.x;
     const u64 nthreads = (u64)gridDim.x * kKeysBlock;
     if (VEC) {
@@ -268,13 +333,13 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
             const u64 i2 = i + nthreads;
             double2 ax = ldStreamD2(x + 2 * i), ay = ldStreamD2(y + 2 * i), az = ldStreamD2(z + 2 * i);
             double2 bx = ldStreamD2(x + 2 * i2), by = ldStreamD2(y + 2 * i2), bz = ldStreamD2(z + 2 * i2);
-            u64 k0 = mortonKey(ax.x, ay.x, az.x, b);
-            u64 k1 = mortonKey(ax.y, ay.y, az.y, b);
+            u64 k0 = sfcKey(ax.x, ay.x, az.x);
+            u64 k1 = sfcKey(ax.y, ay.y, az.y);
             stStreamU2(keys + 2 * i, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
-            k0 = mortonKey(bx.x, by.x, bz.x, b);
-            k1 = mortonKey(bx.y, by.y, bz.y, b);
+            k0 = sfcKey(bx.x, by.x, bz.x);
+            k1 = sfcKey(bx.y, by.y, bz.y);
             stStreamU2(keys + 2 * i2, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
@@ -283,20 +348,20 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
             double2 vx = ldStreamD2(x + 2 * i);
             double2 vy = ldStreamD2(y + 2 * i);
             double2 vz = ldStreamD2(z + 2 * i);
-            u64 k0 = mortonKey(vx.x, vy.x, vz.x, b);
-            u64 k1 = mortonKey(vx.y, vy.y, vz.y, b);
+            u64 k0 = sfcKey(vx.x, vy.x, vz.x);
+            u64 k1 = sfcKey(vx.y, vy.y, vz.y);
             stStreamU2(keys + 2 * i, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
         }
         if ((n & 1) && tid == 0) {
-            u64 k = mortonKey(x[n - 1], y[n - 1], z[n - 1], b);
+            u64 k = sfcKey(x[n - 1], y[n - 1], z[n - 1]);
             keys[n - 1] = k;
             histAdd<HIST>(sh, k);
         }
     } else {
         for (u64 i = tid; i < n; i += nthreads) {
-            u64 k = mortonKey(ldStreamD(x + i), ldStreamD(y + i), ldStreamD(z + i), b);
+            u64 k = sfcKey(ldStreamD(x + i), ldStreamD(y + i), ldStreamD(z + i));
             keys[i] = k;
             histAdd<HIST>(sh, k);
         }
@@ -311,7 +376,7 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
 }
 
 cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, bool withHist, cudaStream_t s)
+                      u64* keys, bool withHist, int curve, cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_KEYS, s);
     if (n == 0) return CS_OK;
@@ -322,10 +387,20 @@ cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const d
     u32 need = divUp(work, kKeysBlock);
     if (need < grid) grid = need ? need : 1;
     u32* h = ctx->sortHist;
-    if (vec && withHist) keysKernel<true, true><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
-    else if (vec) keysKernel<true, false><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
-    else if (withHist) keysKernel<false, true><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
-    else keysKernel<false, false><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h);
+    const unsigned short* tab = ctx->hilbertTable;
+#define CS_KEYS_LAUNCH(V, H, C) keysKernel<V, H, C><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h, tab)
+    if (curve == CS_CURVE_HILBERT) {
+        if (vec && withHist) CS_KEYS_LAUNCH(true, true, true);
+        else if (vec) CS_KEYS_LAUNCH(true, false, true);
+        else if (withHist) CS_KEYS_LAUNCH(false, true, true);
+        else CS_KEYS_LAUNCH(false, false, true);
+    } else {
+        if (vec && withHist) CS_KEYS_LAUNCH(true, true, false);
+        else if (vec) CS_KEYS_LAUNCH(true, false, false);
+        else if (withHist) CS_KEYS_LAUNCH(false, true, false);
+        else CS_KEYS_LAUNCH(false, false, false);
+    }
+#undef CS_KEYS_LAUNCH
     CS_LAUNCH_CHECK(ctx, "keysKernel");
     return CS_OK;
 }
