@@ -22,6 +22,9 @@
  *   - Arrays are structure-of-arrays, densely packed, naturally aligned; x, y, z, keys and
  *     leaves must be 16-byte aligned (any cudaMalloc / torch allocation is).
  *   - n < 2^32 particles (indices are uint32_t).
+ *   - One stream at a time per context: all calls on a context share its workspace, and calls without a host
+ *     out argument return before their work is done, so a context must not be used from two streams or host
+ *     threads at once (calls are ordered only within the stream they are given).  Use one context per stream.
  * ===================================================================================== */
 #ifndef CORNERSTONE_B200_H
 #define CORNERSTONE_B200_H
@@ -54,7 +57,7 @@ enum {
     CS_STAGE_BOX = 0, CS_STAGE_KEYS = 1, CS_STAGE_SORT = 2, CS_STAGE_LEAVES = 3, CS_STAGE_LINK = 4,
     CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6,
     CS_STAGE_SORT_PASSES = 7,    /* the plain radix passes: 4 (CS_SORT_AUTO) or 7 (CS_SORT_PLAIN) */
-    CS_STAGE_SORT_FIXUP = 8,     /* CS_SORT_AUTO: fifth pass, which also orders the low 18 bits, + the gated redo passes */
+    CS_STAGE_SORT_FIXUP = 8,     /* CS_SORT_AUTO: fifth pass, which also orders the low 18 bits, + the gated redo launch */
     CS_NUM_STAGES = 9
 };
 
@@ -125,17 +128,19 @@ cs_status cs_setCurve(cs_context* ctx, int curve);
 cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t n, void* stream);
 
 /* cs_setSortMode -- how cs_sortKeys / cs_buildOctree reach the (unique) stable order.
- *   CS_SORT_AUTO (default): 5 radix passes over the 5 leading 9-bit digits; the fifth also
- *   orders the low 18 bits inside every run of equal leading digits; if some run is longer than
- *   257 elements (particles deeper than octree level 15 in bulk) the 7 plain passes are run
- *   behind it instead, decided on the device with no host round trip.  cs_buildOctree
- *   remembers that outcome and uses the plain passes directly from then on.
+ *   CS_SORT_AUTO (default): 5 radix passes over the 5 leading 9-bit digits (4 plain passes + a fifth that
+ *   also orders the low 18 bits inside every run of equal leading digits); if some run is longer than 257
+ *   elements (particles deeper than octree level 15 in bulk) one more launch behind it redoes the sort with
+ *   the 7 plain passes, decided on the device with no host round trip.  The context remembers that outcome
+ *   (cs_buildOctree reads it with its sizes; after cs_sortKeys it follows the stream to the host) and runs
+ *   the 7 plain passes directly for the next 16 sorts, then tries the short cut again.
  *   CS_SORT_PLAIN: always the 7 plain LSD passes (9 bits each).
- *   The sorted keys and perm are identical in both modes.  Errors: INVALID_ARG. */
+ *   Setting a mode also forgets an earlier redo.  The sorted keys and perm are identical in both modes.
+ *   Errors: INVALID_ARG. */
 enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1 };
 cs_status cs_setSortMode(cs_context* ctx, int mode);
-/* Plain radix passes of the next sort on this context (the ones CS_STAGE_SORT_PASSES times): 4 or 7
- * (0 if ctx is NULL). */
+/* Plain radix passes of the next sort on this context (the ones CS_STAGE_SORT_PASSES times): 4 (followed by the
+ * fused fifth pass) or 7 (0 if ctx is NULL). */
 int cs_sortPasses(const cs_context* ctx);
 
 /* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1

@@ -53,7 +53,7 @@ cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, cons
     if (!x || !y || !z || !box6 || !keys) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeKeys: null pointer");
     CS_TRY(checkParticles(ctx, "cs_computeKeys", n));
     DeviceGuard g(ctx->device);
-    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, CS_CURVE_MORTON, (cudaStream_t)stream);
+    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, -1, CS_CURVE_MORTON, (cudaStream_t)stream);
 }
 
 cs_status cs_computeKeysHilbert(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
@@ -64,7 +64,7 @@ cs_status cs_computeKeysHilbert(cs_context* ctx, const double* x, const double* 
     if (!x || !y || !z || !box6 || !keys) return fail(ctx, CS_ERR_INVALID_ARG, "cs_computeKeysHilbert: null pointer");
     CS_TRY(checkParticles(ctx, "cs_computeKeysHilbert", n));
     DeviceGuard g(ctx->device);
-    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, false, CS_CURVE_HILBERT, (cudaStream_t)stream);
+    return enqueueKeys(ctx, x, y, z, n, box6, (u64*)keys, -1, CS_CURVE_HILBERT, (cudaStream_t)stream);
 }
 
 cs_status cs_setCurve(cs_context* ctx, int curve)
@@ -83,7 +83,7 @@ cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t 
     if (!keys || !perm) return fail(ctx, CS_ERR_INVALID_ARG, "cs_sortKeys: null pointer");
     CS_TRY(checkParticles(ctx, "cs_sortKeys", n));
     DeviceGuard g(ctx->device);
-    return enqueueSort(ctx, (u64*)keys, perm, n, false, (cudaStream_t)stream);
+    return enqueueSort(ctx, (u64*)keys, perm, n, false, sortDecidePlain(ctx), (cudaStream_t)stream);
 }
 
 cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, uint32_t bucketSize,
@@ -118,11 +118,16 @@ cs_status cs_setSortMode(cs_context* ctx, int mode)
     if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setSortMode: ctx is null");
     if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN)
         return fail(ctx, CS_ERR_INVALID_ARG, "cs_setSortMode: unknown mode %d", mode);
-    ctx->sortPlain = mode == CS_SORT_PLAIN;
+    ctx->sortMode = mode;
+    ctx->autoPlainLeft = 0;
     return CS_OK;
 }
 
-int cs_sortPasses(const cs_context* ctx) { return ctx ? (ctx->sortPlain ? 7 : 4) : 0; }
+int cs_sortPasses(const cs_context* ctx)
+{
+    if (!ctx) return 0;
+    return (ctx->sortMode == CS_SORT_PLAIN || ctx->autoPlainLeft > 0 || ctx->hostCtrl->sortRedoHint) ? 7 : 4;
+}
 
 cs_status cs_setLeafMode(cs_context* ctx, int mode)
 {
@@ -208,8 +213,9 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
     // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
-    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), /*withHist=*/true, ctx->curve, s));
-    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, s));
+    const bool plain = sortDecidePlain(ctx);
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
+    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plain, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
                          (u64*)b->leaves, b->counts, leafCap, s));
     // link and node counts in one pass: the leaves' particle offsets are still in the workspace
@@ -217,7 +223,10 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
                        b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,
                        ctx->leafOffFinal, b->nodeFirst, b->nodeCount, s));
     CS_TRY(readCtrl(ctx, s));
-    if (ctx->hostCtrl->sortRedo) ctx->sortPlain = true;   // deep clustering: skip the short cut from now on
+    if (ctx->hostCtrl->sortRedo) {                        // deep clustering: skip the short cut for a while
+        ctx->autoPlainLeft = kPlainHold;
+        ctx->hostCtrl->sortRedoHint = 0;
+    }
     const DeviceCtrl& c = ctx->hostCtrl->c;
     sizes->rounds = c.rounds;
     sizes->converged = c.converged;

@@ -26,6 +26,8 @@ constexpr int kRoundSlots = kMaxRounds + 2;
 constexpr int kRadixBits = CS_RADIX_BITS;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits: 7 passes of 9 bits
+constexpr int kSortTopFirst = 2;      // the default sort plan orders by the digits 2..6 (bits 18..62) and fixes up the rest (cs_sort.cu)
+constexpr int kPlainHold = 16;        // sorts that run the plain plan after one needed the redo, before the short cut is tried again
 #ifndef CS_SORT_BLOCK
 #define CS_SORT_BLOCK 512
 #endif
@@ -89,6 +91,7 @@ struct DeviceCtrl {
 struct HostCtrl {                // pinned mirror read back once per call
     DeviceCtrl c;
     u32 sortRedo;                // the sort's fix-up gave up and the plain passes ran (cs_sort.cu)
+    u32 sortRedoHint;            // the same flag, copied behind every default-plan sort without a synchronisation
 };
 constexpr int kSortRedoSlot = 63;   // ctx->sortTickets[kSortRedoSlot]: that flag on the device
 
@@ -111,7 +114,9 @@ struct cs_context {
     cs::u32* sortTickets = nullptr;
     cs::u64* sortLookback = nullptr;   // [tiles][kRadix]
     cs::u32 epoch = 0;                 // look-back epoch, bumped per launch that uses a look-back array
-    bool sortPlain = false;            // run the 7 plain radix passes (set once a build needed the redo, or by cs_setSortMode)
+    int sortMode = CS_SORT_AUTO;       // cs_setSortMode
+    int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after one needed the redo
+    cs::u32 redoGrid = 0;              // CTAs of onesweepRedoKernel that are resident together (cooperative launch)
 
     // keys
     unsigned short* hilbertTable = nullptr;   // [24][64] two-level transitions of the Hilbert curve (cs_particles.cu)
@@ -213,16 +218,17 @@ u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s);   // first of `co
 // ---- stage enqueue functions (no synchronisation; sizes device-resident) ---------------
 cs_status enqueueBox(cs_context*, const double* x, const double* y, const double* z, u64 n, double* box6,
                      cudaStream_t);
-// withHist: also accumulate the 8 digit histograms of the radix sort into ctx->sortHist
+// histFrom: also accumulate the digit histograms of the radix sort, digits histFrom..6, into ctx->sortHist (-1: none)
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, bool withHist, int curve, cudaStream_t);
+                      u64* keys, int histFrom, int curve, cudaStream_t);
 void hilbertBuildTable(unsigned short* table /*[24 * 64], host*/);
 cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
 cs_status leavesDirectInit(cs_context*);
 cs_status leavesInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
 u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
-cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t);
+bool sortDecidePlain(cs_context*);            // plan of the next sort: 7 plain passes, or the short cut
+cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, bool plain, cudaStream_t);
 cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
                         u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity,
                         cudaStream_t);

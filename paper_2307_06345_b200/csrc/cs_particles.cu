@@ -293,31 +293,33 @@ __device__ __forceinline__ u64 hilbertFromMorton(u64 m, const unsigned short* __
     return h;
 }
 
-template <bool HIST>
+// HIST: first digit that is counted (the default sort plan needs the digits kSortTopFirst..6 only), or -1 for none
+template <int HIST>
 __device__ __forceinline__ void histAdd(u32* sh, u64 key)
 {
-    if (HIST) {
+    if (HIST >= 0) {
 #pragma unroll
-        for (int p = 0; p < kSortPasses; ++p)
-            atomicAdd(&sh[p * kRadix + (u32)((key >> (p * kRadixBits)) & (kRadix - 1))], 1u);
+        for (int p = HIST; p < kSortPasses; ++p)
+            atomicAdd(&sh[(p - HIST) * kRadix + (u32)((key >> (p * kRadixBits)) & (kRadix - 1))], 1u);
     }
 }
 
-template <bool VEC, bool HIST, bool HILBERT>
+template <bool VEC, int HIST, bool HILBERT>
 __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
                                                          const double* __restrict__ z, u64 n,
                                                          const double* __restrict__ box6, u64* __restrict__ keys,
                                                          u32* gHist, const unsigned short* __restrict__ hilbertTable)
 {
-    __shared__ u32 sh[HIST ? kSortPasses * kRadix : 1];
+    constexpr int kHistWords = HIST >= 0 ? (kSortPasses - HIST) * kRadix : 1;
+    __shared__ u32 sh[kHistWords];
     __shared__ unsigned short sTab[HILBERT ? kHilbertStates * 64 : 1];
-    if (HIST) {
-        for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) sh[i] = 0;
+    if (HIST >= 0) {
+        for (int i = threadIdx.x; i < kHistWords; i += kKeysBlock) sh[i] = 0;
     }
     if (HILBERT) {
         for (int i = threadIdx.x; i < kHilbertStates * 64; i += kKeysBlock) sTab[i] = hilbertTable[i];
     }
-    if (HIST || HILBERT) __syncthreads();
+    if (HIST >= 0 || HILBERT) __syncthreads();
     const BoxParams b = loadBox(box6);
     auto sfcKey = [&](double px, double py, double pz) -> u64 {
         const u64 m = mortonKey(px, py, pz, b);
@@ -366,17 +368,17 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
             histAdd<HIST>(sh, k);
         }
     }
-    if (HIST) {
+    if (HIST >= 0) {
         __syncthreads();
-        for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kKeysBlock) {
+        for (int i = threadIdx.x; i < kHistWords; i += kKeysBlock) {
             u32 v = sh[i];
-            if (v) atomicAdd(&gHist[i], v);
+            if (v) atomicAdd(&gHist[HIST * kRadix + i], v);
         }
     }
 }
 
 cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, bool withHist, int curve, cudaStream_t s)
+                      u64* keys, int histFrom, int curve, cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_KEYS, s);
     if (n == 0) return CS_OK;
@@ -389,17 +391,20 @@ cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const d
     u32* h = ctx->sortHist;
     const unsigned short* tab = ctx->hilbertTable;
 #define CS_KEYS_LAUNCH(V, H, C) keysKernel<V, H, C><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h, tab)
+#define CS_KEYS_HIST(V, C)                                        \
+    do {                                                          \
+        if (histFrom < 0) CS_KEYS_LAUNCH(V, -1, C);               \
+        else if (histFrom == 0) CS_KEYS_LAUNCH(V, 0, C);          \
+        else CS_KEYS_LAUNCH(V, kSortTopFirst, C);                 \
+    } while (0)
     if (curve == CS_CURVE_HILBERT) {
-        if (vec && withHist) CS_KEYS_LAUNCH(true, true, true);
-        else if (vec) CS_KEYS_LAUNCH(true, false, true);
-        else if (withHist) CS_KEYS_LAUNCH(false, true, true);
-        else CS_KEYS_LAUNCH(false, false, true);
+        if (vec) CS_KEYS_HIST(true, true);
+        else CS_KEYS_HIST(false, true);
     } else {
-        if (vec && withHist) CS_KEYS_LAUNCH(true, true, false);
-        else if (vec) CS_KEYS_LAUNCH(true, false, false);
-        else if (withHist) CS_KEYS_LAUNCH(false, true, false);
-        else CS_KEYS_LAUNCH(false, false, false);
+        if (vec) CS_KEYS_HIST(true, false);
+        else CS_KEYS_HIST(false, false);
     }
+#undef CS_KEYS_HIST
 #undef CS_KEYS_LAUNCH
     CS_LAUNCH_CHECK(ctx, "keysKernel");
     return CS_OK;

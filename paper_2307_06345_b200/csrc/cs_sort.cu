@@ -20,11 +20,16 @@
 //
 // Model bytes per particle (SURVEY 8d, 8 passes of 8 bits): 196; moved by the default path:
 // pass 0 (8 read, 12 written) + 4 x 24 = 116 (histograms come from the key kernel).
+#include <cooperative_groups.h>
+
 #include "cs_device.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace cs {
 
 constexpr int kHistBlock = 512;
+constexpr int kTopFirst = kSortTopFirst;                    // first digit the default path sorts by (bits 18..)
 constexpr int kSortWarps = kSortBlock / 32;
 static_assert(kSortBlock >= kRadix, "one thread per digit in the per-digit phases of a radix pass");
 static_assert(kSortItems * 32 < 65536 && kSortTile < 65536, "16-bit per-warp digit counters and tile-local slots");
@@ -33,8 +38,9 @@ __device__ __forceinline__ u32 digitOf(u64 key, int shift) { return (u32)(key >>
 
 // ---- global digit histograms of all passes ----------------------------------------------------
 // copyTo (nullable): the keys are also copied there (the buffer the first pass reads, see sortSource)
+// firstPass: digits below it are not counted (their counts stay zero: the default path does not sort by them)
 __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restrict__ keys, u64 n, u32* gHist,
-                                                             u64* __restrict__ copyTo)
+                                                             u64* __restrict__ copyTo, int firstPass)
 {
     __shared__ u32 sh[kSortPasses * kRadix];
     for (int i = threadIdx.x; i < kSortPasses * kRadix; i += kHistBlock) sh[i] = 0;
@@ -44,7 +50,8 @@ __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restri
     const bool vec = (((uintptr_t)keys) & 15u) == 0;
     auto add = [&](u64 k) {
 #pragma unroll
-        for (int p = 0; p < kSortPasses; ++p) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
+        for (int p = 0; p < kSortPasses; ++p)
+            if (p >= firstPass) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
     };
     if (vec) {
         const u64 pairs = n >> 1;
@@ -487,34 +494,85 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     tileWriteOutFixup<SHIFT, LOW>(sm, sHeadMask, keysOut, valsOut, valid, redo);
 }
 
-// The redo passes behind the fix-up: persistent CTAs that leave at once unless *gate != 0, so that
-// the default path pays a few microseconds for them, not a wave of empty CTAs per pass.
+// The redo behind the fix-up: ONE cooperative launch of persistent CTAs that leaves at once unless *gate != 0
+// (the default path pays a few microseconds for it).  Otherwise it sorts the (still complete) input of the fifth
+// pass by all 7 digits, least significant first, with a grid barrier between the passes.  The key kernel only
+// counts the digits the default path needs, so the histograms of the two lowest digits are made here first.
+struct RedoArgs {
+    u64* k[2];
+    u32* v[2];
+    u32 n;
+    u32* hist;                  // [kSortPasses][kRadix]: scanned for the digits >= kTopFirst, zero below
+    u32* tickets;               // kSortPasses ticket counters
+    u64* lookback;
+    u32 epoch0;                 // pass p uses look-back epoch epoch0 + p
+    const u32* gate;
+};
+
 template <int SHIFT>
-__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
-    onesweepGatedKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
-                        u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase, u32* ticket, u64* lookback,
-                        u32 epoch, const u32* gate)
+__device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in)
 {
-    extern __shared__ __align__(16) unsigned char smemRaw[];
-    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
     const u32 tid = threadIdx.x;
-    if (*reinterpret_cast<const volatile u32*>(gate) == 0) return;
-    const u32 tiles = (n + kSortTile - 1) / kSortTile;
+    const u32 tiles = (a.n + kSortTile - 1) / kSortTile;
     u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
+    constexpr int pass = SHIFT / kRadixBits;
     for (;;) {
         __syncthreads();                                   // the previous tile is written out
-        if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+        if (tid == 0) sm.tile = atomicAdd(a.tickets + pass, 1u);
         for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
         __syncthreads();
         const u32 tile = sm.tile;
         if (tile >= tiles) break;
         const u64 base = (u64)tile * kSortTile;
-        const u32 valid = (u32)((n - base) < (u64)kSortTile ? (n - base) : (u64)kSortTile);
+        const u32 valid = (u32)((a.n - base) < (u64)kSortTile ? (a.n - base) : (u64)kSortTile);
         if (valid == kSortTile)
-            onesweepTile<SHIFT, false, true>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
+            onesweepTile<SHIFT, false, true>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
+                                             a.hist + pass * kRadix, a.lookback, a.epoch0 + pass);
         else
-            onesweepTile<SHIFT, false, false>(sm, keysIn, valsIn, keysOut, valsOut, tile, valid, digitBase, lookback, epoch);
+            onesweepTile<SHIFT, false, false>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
+                                              a.hist + pass * kRadix, a.lookback, a.epoch0 + pass);
     }
+}
+
+__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks) onesweepRedoKernel(const RedoArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smemRaw[];
+    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    if (*reinterpret_cast<const volatile u32*>(a.gate) == 0) return;
+    cg::grid_group grid = cg::this_grid();
+    const u32 tid = threadIdx.x;
+    {   // digit counts of the passes the key kernel did not count (zero so far), then their exclusive scans
+        u32* sh = reinterpret_cast<u32*>(smemRaw);
+        for (int i = tid; i < kTopFirst * kRadix; i += kSortBlock) sh[i] = 0;
+        __syncthreads();
+        for (u64 i = (u64)blockIdx.x * kSortBlock + tid; i < a.n; i += (u64)gridDim.x * kSortBlock) {
+            const u64 k = a.k[0][i];
+#pragma unroll
+            for (int p = 0; p < kTopFirst; ++p) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
+        }
+        __syncthreads();
+        for (int i = tid; i < kTopFirst * kRadix; i += kSortBlock)
+            if (sh[i]) atomicAdd(&a.hist[i], sh[i]);
+        grid.sync();
+        for (u32 p = blockIdx.x; p < (u32)kTopFirst; p += gridDim.x) {   // block-uniform trip count
+            u32 total;
+            u32* warpSums = reinterpret_cast<u32*>(smemRaw);
+            const u32 idx = p * kRadix + tid;
+            const u32 c = tid < kRadix ? *reinterpret_cast<volatile u32*>(&a.hist[idx]) : 0u;
+            __syncthreads();
+            const u32 ex = blockExclusiveScan<kSortBlock>(c, warpSums, &total);
+            if (tid < kRadix) a.hist[idx] = ex;
+            __syncthreads();
+        }
+        grid.sync();
+    }
+    redoPass<0>(sm, a, 0);  grid.sync();
+    redoPass<9>(sm, a, 1);  grid.sync();
+    redoPass<18>(sm, a, 0); grid.sync();
+    redoPass<27>(sm, a, 1); grid.sync();
+    redoPass<36>(sm, a, 0); grid.sync();
+    redoPass<45>(sm, a, 1); grid.sync();
+    redoPass<54>(sm, a, 0);
 }
 
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
@@ -548,29 +606,13 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
     return CS_OK;
 }
 
-template <int SHIFT>
-static cs_status launchGatedPass(cs_context* ctx, PassPlan& pl, const u32* gate, cudaStream_t s)
-{
-    const u32 epoch = nextEpoch(ctx, s);
-    const int in = pl.cur, out = in ^ 1;
-    const u32 resident = (u32)ctx->numSMs * kSortMinBlocks;
-    onesweepGatedKernel<SHIFT><<<pl.tiles < resident ? pl.tiles : resident, kSortBlock, sizeof(SortSmem), s>>>(
-        pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
-        ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, gate);
-    CS_LAUNCH_CHECK(ctx, "onesweepGatedKernel");
-    pl.cur = out;
-    return CS_OK;
-}
-
 // The radix kernels need more dynamic shared memory than the default limit: opt in on the context's device
 // (function attributes are per device, so this runs once per cs_create, not once per process).
 template <int SHIFT>
 static cudaError_t sortInitShift()
 {
     const int bytes = (int)sizeof(SortSmem);
-    cudaError_t e = cudaFuncSetAttribute(onesweepKernel<SHIFT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(onesweepGatedKernel<SHIFT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    return e;
+    return cudaFuncSetAttribute(onesweepKernel<SHIFT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 cs_status sortInit(cs_context* ctx)
 {
@@ -585,6 +627,11 @@ cs_status sortInit(cs_context* ctx)
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepRedoKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    int perSM = 0;
+    CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, onesweepRedoKernel, kSortBlock, bytes));
+    if (perSM < 1) return fail(ctx, CS_ERR_CUDA, "onesweepRedoKernel does not fit on an SM");
+    ctx->redoGrid = (u32)perSM * (u32)ctx->numSMs;
     return CS_OK;
 }
 
@@ -595,7 +642,22 @@ u64* sortSource(cs_context* ctx, u64*) { return ctx->keysAlt; }
 
 // fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
 // (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
-cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, cudaStream_t s)
+// Which plan the next sort on this context runs: the 7 plain passes if the caller asked for them (cs_setSortMode)
+// or if a recent sort had to be redone (runs too long for the short cut); in the latter case the short cut is
+// tried again after kPlainHold sorts.
+bool sortDecidePlain(cs_context* ctx)
+{
+    if (ctx->hostCtrl->sortRedoHint) {                      // written by the stream behind an earlier sort
+        ctx->hostCtrl->sortRedoHint = 0;
+        ctx->autoPlainLeft = kPlainHold;
+    }
+    if (ctx->sortMode == CS_SORT_PLAIN) return true;
+    if (ctx->autoPlainLeft == 0) return false;
+    --ctx->autoPlainLeft;
+    return true;
+}
+
+cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, bool plain, cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_SORT, s);
     if (n == 0) return CS_OK;
@@ -607,7 +669,8 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
             u32 grid = (u32)ctx->numSMs * 4;
             u32 need = divUp((n + 1) / 2, kHistBlock);
             if (need < grid) grid = need ? need : 1;
-            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first);
+            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first,
+                                                       plain ? 0 : kTopFirst);
             CS_LAUNCH_CHECK(ctx, "sortHistKernel");
         }
         sortScanHistKernel<<<kSortPasses, kRadix, 0, s>>>(ctx->sortHist);
@@ -622,7 +685,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     pl.n = (u32)n;
     pl.tiles = divUp(n, kSortTile);
     pl.ticketSlot = 0;
-    if (ctx->sortPlain) {                                   // all 7 digits, least significant first
+    if (plain) {                                            // all 7 digits, least significant first
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
         CS_TRY((launchPass<0, true>(ctx, pl, s)));
         CS_TRY((launchPass<9, false>(ctx, pl, s)));
@@ -651,13 +714,24 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     }
     // gated redo from the input of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
     // which is where the fifth pass wrote
-    CS_TRY((launchGatedPass<0>(ctx, pl, redo, s)));
-    CS_TRY((launchGatedPass<9>(ctx, pl, redo, s)));
-    CS_TRY((launchGatedPass<18>(ctx, pl, redo, s)));
-    CS_TRY((launchGatedPass<27>(ctx, pl, redo, s)));
-    CS_TRY((launchGatedPass<36>(ctx, pl, redo, s)));
-    CS_TRY((launchGatedPass<45>(ctx, pl, redo, s)));
-    return launchGatedPass<54>(ctx, pl, redo, s);
+    RedoArgs a;
+    a.k[0] = pl.k[pl.cur]; a.k[1] = pl.k[pl.cur ^ 1];
+    a.v[0] = pl.v[pl.cur]; a.v[1] = pl.v[pl.cur ^ 1];
+    a.n = pl.n;
+    a.hist = ctx->sortHist;
+    a.tickets = ctx->sortTickets + pl.ticketSlot;
+    a.lookback = ctx->sortLookback;
+    a.epoch0 = reserveEpochs(ctx, kSortPasses, s);
+    a.gate = redo;
+    const u32 grid = pl.tiles < ctx->redoGrid ? pl.tiles : ctx->redoGrid;
+    void* args[] = {(void*)&a};
+    CS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)onesweepRedoKernel, dim3(grid), dim3(kSortBlock), args,
+                                             sizeof(SortSmem), s));
+    CS_LAUNCH_CHECK(ctx, "onesweepRedoKernel");
+    // a hint for callers that never read the control block (cs_sortKeys): the outcome reaches the host with the
+    // stream, and the next sort on this context looks at it
+    CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedoHint, redo, sizeof(u32), cudaMemcpyDeviceToHost, s));
+    return CS_OK;
 }
 
 }  // namespace cs

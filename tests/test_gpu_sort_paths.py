@@ -33,7 +33,11 @@ def ctx(cs):
     c.close()
 
 
-def check(cs, ctx, k):
+def check(cs, ctx, k, mode=0):
+    """mode: SORT_AUTO (0) / SORT_PLAIN (1) is set first (which also forgets an earlier redo); None leaves the context as
+    it is."""
+    if mode is not None:
+        ctx.setSortMode(mode)
     P, perm = oracle.sort(k)
     dk = cs.from_u64(k, ctx.device)
     dperm = cs.sortKeys(ctx, dk)
@@ -100,10 +104,8 @@ def test_plain_mode_equals_default(cs, ctx):
     rng = np.random.default_rng(8)
     for n in (1, 257, 6656, 6657, 123457):
         k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
-        ctx.setSortMode(cs.SORT_PLAIN)
-        check(cs, ctx, k)
-        ctx.setSortMode(cs.SORT_AUTO)
-        check(cs, ctx, k)
+        check(cs, ctx, k, cs.SORT_PLAIN)
+        check(cs, ctx, k, cs.SORT_AUTO)
     with pytest.raises(cs.CornerstoneError):
         ctx.setSortMode(7)
 
@@ -118,12 +120,35 @@ def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
     z = np.concatenate([rng.random(n - 4000), 0.5 + 1e-7 * rng.random(4000)])
     ref = oracle.full_build(x, y, z, 64)
     d = [torch.from_numpy(a).cuda() for a in (x, y, z)]
-    for _ in range(3):
+    ctx.setSortMode(cs.SORT_AUTO)
+    plans = []
+    for _ in range(20):
+        plans.append(ctx.sortPasses())
         got = cs.buildOctree(ctx, d[0], d[1], d[2], 64)
         assert np.array_equal(cs.u64(got["keys"]), ref["sortedKeys"])
         assert np.array_equal(cs.u32(got["perm"]), ref["perm"])
         assert np.array_equal(cs.u64(got["leaves"]), ref["leaves"])
         assert np.array_equal(cs.u32(got["nodeCount"]), ref["nodeCount"])
+    # the short cut (4 plain passes + the fused fifth), redone on the device; then the 7 plain passes for 16 builds;
+    # then the short cut is tried again (and redone again): one pathological step does not cost every later one
+    assert plans == [4] + [7] * 16 + [4] + [7] * 2
+    ctx.setSortMode(cs.SORT_AUTO)
+
+
+def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
+    """cs_sortKeys never reads the control block; the redo flag follows the stream to the host and the next sort on the
+    context takes the plain passes."""
+    rng = np.random.default_rng(5)
+    k = np.concatenate([rng.integers(0, 1 << 63, 50000, dtype=np.uint64),
+                        (np.uint64(0x1234567) << np.uint64(30)) | rng.integers(0, 1 << LOW, 3000, dtype=np.uint64)])
+    rng.shuffle(k)
+    ctx.setSortMode(cs.SORT_AUTO)
+    assert ctx.sortPasses() == 4
+    check(cs, ctx, k)                                           # check() synchronises when it copies the result back
+    assert ctx.sortPasses() == 7
+    check(cs, ctx, k, mode=None)
+    ctx.setSortMode(cs.SORT_AUTO)
+    assert ctx.sortPasses() == 4
 
 
 def test_workload_shapes(cs, ctx):
