@@ -272,6 +272,56 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
                              uint32_t bucketSize, const cs_octree_buffers* host, cs_octree_sizes* sizes,
                              void* stream);
 
+/* ---- 32-bit keys: L = 10 ("reasonable choices for L are 10 or 21") --------------------------------
+ *
+ * The same path with keys of 10 octal digits (30 bits, in a uint32_t): the tree resolves 10 levels, 8^10 = 2^30
+ * terminates a cornerstone array, leaves at level 10 may hold more than bucketSize particles (A7), prefixes are
+ * placeholder-bit keys of at most 31 bits.  The grid coordinate is clamp(floor(((c - lo) / (hi - lo)) * 2^10), 0,
+ * 2^10 - 1) with the same quotient as for L = 21, so a 30-bit key equals the 63-bit key of the same particle
+ * shifted right by 33 bits.  The sort moves 8 instead of 12 bytes per element and needs 4 passes of 9-bit digits.
+ * Arguments, ownership, synchronisation and errors are those of the 64-bit calls of the same name; levelRange
+ * still has CS_NUM_LEVEL_OFFSETS entries (those past level 11 equal numNodes).  The tree stages widen keys and
+ * leaf arrays into the context's workspace (the first call allocates 26 bytes per leaf of capacity for it).
+ */
+#define CS_MAX_LEVEL32 10u
+#define CS_KEY_END32 (1u << 30)
+
+/* curve: CS_CURVE_MORTON or CS_CURVE_HILBERT */
+cs_status cs_computeKeys32(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                           const double* box6, int curve, uint32_t* keys, void* stream);
+cs_status cs_sortKeys32(cs_context* ctx, uint32_t* keys, uint32_t* perm, uint64_t n, void* stream);
+cs_status cs_buildLeaves32(cs_context* ctx, const uint32_t* sortedKeys, uint64_t n, uint32_t bucketSize,
+                           const uint32_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, uint32_t* leaves,
+                           uint32_t* counts, uint32_t leafCapacity, uint32_t* numLeaves, uint32_t* rounds, void* stream);
+cs_status cs_linkOctree32(cs_context* ctx, const uint32_t* leaves, uint32_t numLeaves, uint32_t* prefixes,
+                          uint32_t* levels, uint32_t* childOffsets, uint32_t* parents, uint32_t* levelRange,
+                          uint32_t* leafToNode, uint32_t* nodeToLeaf, uint32_t nodeCapacity, uint32_t* numNodes,
+                          void* stream);
+
+typedef struct cs_octree_buffers32 {   /* cs_octree_buffers with 32-bit keys, leaves and prefixes */
+    double*   box6;
+    uint32_t* keys;
+    uint32_t* perm;
+    uint32_t* leaves;
+    uint32_t* counts;
+    uint32_t* prefixes;
+    uint32_t* levels;        /* nullable */
+    uint32_t* childOffsets;
+    uint32_t* parents;       /* nullable */
+    uint32_t* levelRange;
+    uint32_t* leafToNode;    /* nullable */
+    uint32_t* nodeToLeaf;
+    uint32_t* nodeFirst;
+    uint32_t* nodeCount;
+    uint32_t  leafCapacity;
+    uint32_t  nodeCapacity;
+} cs_octree_buffers32;
+
+/* box, 30-bit keys (on the curve of cs_setCurve), sort, leaves from {0, 8^10}, links and node counts in one call. */
+cs_status cs_buildOctree32(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
+                           uint32_t bucketSize, const cs_octree_buffers32* buffers, cs_octree_sizes* sizes,
+                           void* stream);
+
 /* ---- node properties on the linked octree (first row past the hot path: "additional octree
  *      node properties ... can be stored in separate arrays of length n"; readings A25-A27) --------
  * All arrays are device pointers owned by the caller; the calls enqueue on `stream` and return.  Three-component

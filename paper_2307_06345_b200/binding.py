@@ -49,6 +49,11 @@ class OctreeBuffers(C.Structure):
         ("leafCapacity", C.c_uint32), ("nodeCapacity", C.c_uint32)]
 
 
+class OctreeBuffers32(C.Structure):
+    """Mirror of cs_octree_buffers32 (same members; keys, leaves and prefixes are uint32)."""
+    _fields_ = OctreeBuffers._fields_
+
+
 class OctreeSizes(C.Structure):
     """Mirror of cs_octree_sizes."""
     _fields_ = [("numLeaves", C.c_uint32), ("numNodes", C.c_uint32), ("rounds", C.c_uint32),
@@ -92,6 +97,11 @@ def lib():
                                      C.POINTER(OctreeSizes), vp]),
         "cs_buildOctreeHost": (C.c_int, [vp, vp, vp, vp, u64, u32, C.POINTER(OctreeBuffers),
                                          C.POINTER(OctreeSizes), vp]),
+        "cs_computeKeys32": (C.c_int, [vp, vp, vp, vp, u64, vp, C.c_int, vp, vp]),
+        "cs_sortKeys32": (C.c_int, [vp, vp, vp, u64, vp]),
+        "cs_buildLeaves32": (C.c_int, [vp, vp, u64, u32, vp, u32, u32, vp, vp, u32, C.POINTER(u32), C.POINTER(u32), vp]),
+        "cs_linkOctree32": (C.c_int, [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp, u32, C.POINTER(u32), vp]),
+        "cs_buildOctree32": (C.c_int, [vp, vp, vp, vp, u64, u32, C.POINTER(OctreeBuffers32), C.POINTER(OctreeSizes), vp]),
         "cs_gatherParticles": (C.c_int, [vp, vp, vp, vp, vp, u64, vp, vp, vp, vp]),
         "cs_nodeGeometry": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
         "cs_nodeMassCenters": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp, vp]),
@@ -360,6 +370,94 @@ def buildOctreeHost(ctx: Context, x, y, z, bucketSize: int, host: HostBuffers):
                                   C.byref(sizes), _stream())
     ctx.check(st)
     return {"numLeaves": int(sizes.numLeaves), "numNodes": int(sizes.numNodes), "rounds": int(sizes.rounds)}
+
+
+# ---- 32-bit keys, L = 10 (include/cornerstone.h, "32-bit keys") ------------------------------------------------------
+# keys, leaves and prefixes are int32 tensors holding uint32 bit patterns
+
+KEY_END32 = 1 << 30
+
+
+def computeKeys32(ctx: Context, x, y, z, box6, curve: int = CURVE_MORTON, keys=None):
+    if keys is None:
+        keys = _i32(x.numel(), ctx.device)
+    ctx.check(lib().cs_computeKeys32(ctx.handle, _ptr(x), _ptr(y), _ptr(z), x.numel(), _ptr(box6), int(curve), _ptr(keys),
+                                     _stream()))
+    return keys
+
+
+def sortKeys32(ctx: Context, keys, perm=None):
+    """Sorts ``keys`` (int32 tensor of 30-bit keys) in place; returns perm."""
+    if perm is None:
+        perm = _i32(keys.numel(), ctx.device)
+    ctx.check(lib().cs_sortKeys32(ctx.handle, _ptr(keys), _ptr(perm), keys.numel(), _stream()))
+    return perm
+
+
+def buildLeaves32(ctx: Context, sortedKeys, bucketSize: int, prevLeaves=None, maxRounds: int = 0,
+                  leafCapacity: int | None = None, allow_not_converged: bool = False):
+    cap = int(leafCapacity if leafCapacity is not None else ctx.max_leaves)
+    leaves, counts = _i32(cap + 1, ctx.device), _i32(cap, ctx.device)
+    nl, rounds = C.c_uint32(0), C.c_uint32(0)
+    prev_n = 0 if prevLeaves is None else prevLeaves.numel() - 1
+    st = lib().cs_buildLeaves32(ctx.handle, _ptr(sortedKeys), sortedKeys.numel(), bucketSize, _ptr(prevLeaves), prev_n,
+                                maxRounds, _ptr(leaves), _ptr(counts), cap, C.byref(nl), C.byref(rounds), _stream())
+    ctx.check(st, allow=(ERR_NOT_CONVERGED,) if allow_not_converged else ())
+    n = int(nl.value)
+    return leaves[:n + 1], counts[:n], int(rounds.value), st == OK
+
+
+def linkOctree32(ctx: Context, leaves):
+    nl = leaves.numel() - 1
+    cap = nl + max(nl - 1, 0) // 7 + 1
+    dev = ctx.device
+    out = {"prefixes": _i32(cap, dev), "levels": _i32(cap, dev), "childOffsets": _i32(cap, dev),
+           "parents": _i32(cap, dev), "levelRange": _i32(NUM_LEVEL_OFFSETS, dev), "leafToNode": _i32(max(nl, 1), dev),
+           "nodeToLeaf": _i32(cap, dev)}
+    nn = C.c_uint32(0)
+    ctx.check(lib().cs_linkOctree32(ctx.handle, _ptr(leaves), nl, _ptr(out["prefixes"]), _ptr(out["levels"]),
+                                    _ptr(out["childOffsets"]), _ptr(out["parents"]), _ptr(out["levelRange"]),
+                                    _ptr(out["leafToNode"]), _ptr(out["nodeToLeaf"]), cap, C.byref(nn), _stream()))
+    n = int(nn.value)
+    for k in ("prefixes", "levels", "childOffsets", "parents", "nodeToLeaf"):
+        out[k] = out[k][:n]
+    out["leafToNode"] = out["leafToNode"][:nl]
+    out["numNodes"] = n
+    return out
+
+
+class TreeBuffers32:
+    """Pre-allocated device outputs of cs_buildOctree32."""
+
+    def __init__(self, ctx: Context, n: int, leafCapacity: int | None = None):
+        dev = ctx.device
+        self.leafCapacity = int(leafCapacity if leafCapacity is not None else ctx.max_leaves)
+        self.nodeCapacity = self.leafCapacity + (self.leafCapacity - 1) // 7 + 1
+        lc, nc = self.leafCapacity, self.nodeCapacity
+        self.t = {
+            "box6": torch.empty(6, dtype=torch.float64, device=dev), "keys": _i32(n, dev), "perm": _i32(n, dev),
+            "leaves": _i32(lc + 1, dev), "counts": _i32(lc, dev), "prefixes": _i32(nc, dev), "levels": _i32(nc, dev),
+            "childOffsets": _i32(nc, dev), "parents": _i32(nc, dev), "levelRange": _i32(NUM_LEVEL_OFFSETS, dev),
+            "leafToNode": _i32(lc, dev), "nodeToLeaf": _i32(nc, dev), "nodeFirst": _i32(nc, dev),
+            "nodeCount": _i32(nc, dev)}
+        self.c = OctreeBuffers32(**{k: v.data_ptr() for k, v in self.t.items()}, leafCapacity=lc, nodeCapacity=nc)
+
+
+def buildOctree32(ctx: Context, x, y, z, bucketSize: int, buffers: TreeBuffers32 | None = None):
+    n = x.numel()
+    if buffers is None:
+        buffers = TreeBuffers32(ctx, n)
+    sizes = OctreeSizes()
+    ctx.check(lib().cs_buildOctree32(ctx.handle, _ptr(x), _ptr(y), _ptr(z), n, bucketSize, C.byref(buffers.c),
+                                     C.byref(sizes), _stream()))
+    nl, nn = int(sizes.numLeaves), int(sizes.numNodes)
+    t = buffers.t
+    out = {"box6": t["box6"], "keys": t["keys"], "perm": t["perm"], "leaves": t["leaves"][:nl + 1],
+           "counts": t["counts"][:nl], "levelRange": t["levelRange"], "leafToNode": t["leafToNode"][:nl]}
+    for k in ("prefixes", "levels", "childOffsets", "parents", "nodeToLeaf", "nodeFirst", "nodeCount"):
+        out[k] = t[k][:nn]
+    out.update(numLeaves=nl, numNodes=nn, rounds=int(sizes.rounds), converged=bool(sizes.converged))
+    return out
 
 
 # ---- node properties on the linked octree (include/cornerstone.h, last section) ---------------------------

@@ -105,7 +105,7 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
     DeviceGuard g(ctx->device);
     cudaStream_t s = (cudaStream_t)stream;
     CS_TRY(enqueueLeaves(ctx, (const u64*)sortedKeys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
-                         (u64*)leaves, counts, leafCapacity, s));
+                         (u64*)leaves, counts, leafCapacity, kL, s));
     CS_TRY(readCtrl(ctx, s));
     const DeviceCtrl& c = ctx->hostCtrl->c;
     *rounds = c.rounds;
@@ -217,7 +217,7 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
     CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
     CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plain, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
-                         (u64*)b->leaves, b->counts, leafCap, s));
+                         (u64*)b->leaves, b->counts, leafCap, kL, s));
     // link and node counts in one pass: the leaves' particle offsets are still in the workspace
     CS_TRY(enqueueLink(ctx, (const u64*)b->leaves, &ctx->ctrl->numLeaves, 0, leafCap, (u64*)b->prefixes, b->levels,
                        b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,

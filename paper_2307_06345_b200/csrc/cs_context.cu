@@ -270,6 +270,7 @@ void cs_destroy(cs_context* ctx)
     DeviceGuard guard(ctx->device);
     if (ctx->slab) cudaFree(ctx->slab);
     if (ctx->hostPathSlab) cudaFree(ctx->hostPathSlab);
+    if (ctx->wideSlab) cudaFree(ctx->wideSlab);
     if (ctx->hostCtrl) cudaFreeHost(ctx->hostCtrl);
     for (int i = 0; i < CS_NUM_STAGES; ++i) {
         if (ctx->evBegin[i]) cudaEventDestroy(ctx->evBegin[i]);

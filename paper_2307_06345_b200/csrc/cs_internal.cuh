@@ -148,6 +148,12 @@ struct cs_context {
     cs::DeviceCtrl* ctrl = nullptr;
     cs::HostCtrl* hostCtrl = nullptr;  // pinned
 
+    // 64-bit staging of the L = 10 entry points (cs_api32.cu; allocated on first use)
+    char* wideSlab = nullptr;
+    cs::u64* wideLeaves = nullptr;     // [maxLeaves + 2]
+    cs::u64* widePrev = nullptr;       // [maxLeaves + 2]
+    cs::u64* widePrefixes = nullptr;   // [maxNodes + 2]
+
     // buffers for cs_buildOctreeHost (allocated lazily)
     char* hostPathSlab = nullptr;
     size_t hostPathBytes = 0;
@@ -220,20 +226,22 @@ cs_status enqueueBox(cs_context*, const double* x, const double* y, const double
                      cudaStream_t);
 // histFrom: also accumulate the digit histograms of the radix sort, digits histFrom..6, into ctx->sortHist (-1: none)
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, int histFrom, int curve, cudaStream_t);
+                      u64* keys, int histFrom, int curve, cudaStream_t, u32* keys32 = nullptr /*30-bit keys instead*/);
 void hilbertBuildTable(unsigned short* table /*[24 * 64], host*/);
 cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
 cs_status leavesDirectInit(cs_context*);
 cs_status leavesInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
 u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
+cs_status enqueueSort32(cs_context*, u32* keys, u32* perm, u64 n, cudaStream_t);   // 30-bit keys: 4 plain passes
 bool sortDecidePlain(cs_context*);            // plan of the next sort: 7 plain passes, or the short cut
 cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, bool plain, cudaStream_t);
+// maxLevel: depth below which no leaf is split: kL, or 10 for 30-bit keys held in the top 10 digits (cs_api32.cu)
 cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
-                        u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity,
+                        u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, u32 maxLevel,
                         cudaStream_t);
 bool leavesDirectSupported(const cs_context*, u32 bucketSize);
-cs_status enqueueLeavesDirect(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, u32 cap, cudaStream_t);
+cs_status enqueueLeavesDirect(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, u32 cap, u32 maxLevel, cudaStream_t);
 // leaves/numLeaves: if dNumLeaves is null the host value is used
 cs_status enqueueLink(cs_context*, const u64* leaves, const u32* dNumLeaves, u32 hNumLeaves, u32 leafBound,
                       u64* prefixes, u32* levels, u32* childOffsets, u32* parents, u32* levelRange,

@@ -180,7 +180,7 @@ __device__ __forceinline__ void leafStageTile(LeafTileSmem& sm, const u64* Kin, 
 // returns true (in every thread of every CTA) ... after the grid barrier that follows: see leafRoundsKernel
 __device__ __forceinline__ void
     leafDecideBody(LeafTileSmem& sm, DeviceCtrl* ctrl, u32 n, u32 nl, const u64* Kin, const u32* offIn, u32* opk,
-                   TileInfo* info, u32 r, u32 bucket, bool emit, u64* __restrict__ leaves, u32* __restrict__ counts,
+                   TileInfo* info, u32 r, u32 bucket, u64 minDelta, bool emit, u64* __restrict__ leaves, u32* __restrict__ counts,
                    u32* __restrict__ offFinal)
 {
     const u32 tiles = (nl + kLeafTile - 1) / kLeafTile;
@@ -214,7 +214,7 @@ __device__ __forceinline__ void
                 const u64 delta = Kn - Kk;
                 const u32 cnt = offn - offk;                              // f: N_i
                 o = 1;
-                if (cnt > bucket && delta > 1) o = 8;                    // split (A7: not at depth L)
+                if (cnt > bucket && delta > minDelta) o = 8;             // split (A7: not at depth L)
                 else if (delta != kKeyEnd) {                             // the root never merges (A9)
                     const u32 j = (u32)(Kk >> (__ffsll((long long)delta) - 1)) & 7u;   // octant among siblings (delta = 8^m)
                     if (j != 0 && i >= j && i - j + 8 <= nl) {
@@ -474,6 +474,7 @@ struct RoundsArgs {
     uint4* tasksSearch;
     u32 maxTasks;
     u32 bucket, cap, roundsToLaunch;
+    u64 minDelta;               // key range of a leaf at the maximum depth: 1, or 8^11 for 30-bit keys held in the top digits
     bool emitEarly;             // rounds after the first also hand their input array to the caller: if such a round turns out to
                                 // be the confirming one, the result is already in place (incremental starts: round 1, normally)
     u64* leaves;
@@ -492,7 +493,7 @@ __global__ void __launch_bounds__(kLeafBlock, 5) leafRoundsKernel(const RoundsAr
     for (u32 r = 0; r < a.roundsToLaunch; ++r) {
         const u32 in = r & 1, out = in ^ 1;
         const bool emitNow = a.emitEarly && r > 0;
-        leafDecideBody(sm, ctrl, a.n, nl, a.K[in], a.off[in], a.opk, a.info, r, a.bucket, emitNow, a.leaves, a.counts,
+        leafDecideBody(sm, ctrl, a.n, nl, a.K[in], a.off[in], a.opk, a.info, r, a.bucket, a.minDelta, emitNow, a.leaves, a.counts,
                        a.offFinal);
         grid.sync();
         if (ldVolatile(&ctrl->changed[r]) == 0) {            // O_i = 1 for all i: converged, K' = K
@@ -533,7 +534,7 @@ cs_status leavesInit(cs_context* ctx)
 }
 
 cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const u64* prevLeaves, u32 prevNumLeaves,
-                        u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, cudaStream_t s)
+                        u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, u32 maxLevel, cudaStream_t s)
 {
     StageTimer t(ctx, CS_STAGE_LEAVES, s);
     const u32 cap = leafCapacity < ctx->maxLeaves ? leafCapacity : ctx->maxLeaves;
@@ -543,7 +544,7 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
     // From the root and to convergence the fixpoint is built in one pass over P (cs_leaves_direct.cu);
     // the rounds below serve incremental starts, bounded round counts and cs_setLeafMode(ITERATIVE).
     if (!prevLeaves && maxRounds == 0 && ctx->leafMode != CS_LEAVES_ITERATIVE && leavesDirectSupported(ctx, bucket)) {
-        CS_TRY(enqueueLeavesDirect(ctx, P, n, bucket, cap, s));
+        CS_TRY(enqueueLeavesDirect(ctx, P, n, bucket, cap, maxLevel, s));
         u32 g = divUp((u64)cap + 1, 256);
         if (g > persistentGrid) g = persistentGrid;
         leavesEmitKernel<<<g, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafOff[0], leaves, counts, ctx->leafOffFinal);
@@ -570,6 +571,7 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
     a.opk = ctx->leafOpk; a.info = reinterpret_cast<TileInfo*>(ctx->leafTileInfo);
     a.roundsToLaunch = (maxRounds == 0 || maxRounds > (u32)kMaxRounds) ? (u32)kMaxRounds : maxRounds;
     a.bucket = bucket; a.cap = cap;
+    a.minDelta = 1ull << (3 * (kL - (int)maxLevel));
     a.emitEarly = prevLeaves != nullptr;
     a.leaves = leaves; a.counts = counts; a.offFinal = ctx->leafOffFinal;
     // every CTA must be resident (grid barriers): at most what the device holds, at most one CTA per tile

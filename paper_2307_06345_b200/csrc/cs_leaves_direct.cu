@@ -8,6 +8,7 @@
 // is not).  Because P is sorted, (*) can be decided from windows of b+1 = N_crit+1 consecutive
 // keys: a node holds more than b particles iff it contains such a window, so with
 //   w_i = min(#leading octal digits shared by P[i] and P[i+b], L-1)       (0 <= i < n-b)
+// (L = 21; for the 30-bit keys of the L = 10 entry points, held in the top digits, the cap is 9: wcap below)
 // the deepest internal node on the path of particle j has level
 //   d_j = max{ w_i : j-b <= i <= j }                                       (sliding maximum)
 // and the leaf that holds particle j has level D_j = d_j + 1 (D_j = 0, the root, if n <= b).
@@ -158,7 +159,8 @@ __device__ __forceinline__ u32 dirShifted(const u32* a, u32 q, u32 o)
 // dmax[q'] = d of particle T0 - 1 + q'.  EDGE: the tile touches the ends of P.
 template <bool EDGE>
 __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm, const DirLayout& L,
-                                                              const u64* __restrict__ P, u32 n, u32 b, long long T0)
+                                                              const u64* __restrict__ P, u32 n, u32 b, long long T0,
+                                                              u32 wcap)
 {
     const u32 tid = threadIdx.x;
     const long long G0 = T0 - (long long)b - 1;
@@ -189,7 +191,7 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
         const u32 i = k * kDirBlock + tid;
         const u64 kb = sm.K[i + b];
         u32 w = sharedDigitsX(sm.K[i] ^ kb);
-        w = w < (u32)kL - 1 ? w : (u32)kL - 1;
+        w = w < wcap ? w : wcap;
         u32 sv = sharedDigitsX(kb ^ sm.K[i + b + 1]);
         if (EDGE) {
             if (!(G0 + i >= 0 && G0 + i + b < (long long)n)) w = 0;
@@ -202,7 +204,7 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
     }
     for (u32 i = kDirTile + tid; i <= kDirTile + b; i += kDirBlock) {
         u32 w = sharedDigitsX(sm.K[i] ^ sm.K[i + b]);
-        w = w < (u32)kL - 1 ? w : (u32)kL - 1;
+        w = w < wcap ? w : wcap;
         if (EDGE && !(G0 + i >= 0 && G0 + i + b < (long long)n)) w = 0;
         w0[i] = (unsigned char)w;
     }
@@ -249,7 +251,7 @@ __device__ __forceinline__ const unsigned char* dirTileLevels(const DirSmem& sm,
 // constants), or 0 for any bucket size.
 template <u32 BFIX>
 __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
-    leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 bAny, unsigned char* __restrict__ dArr,
+    leavesLevelsKernel(DeviceCtrl* ctrl, const u64* __restrict__ P, u32 n, u32 bAny, u32 wcap, unsigned char* __restrict__ dArr,
                        unsigned char* __restrict__ flags, u32* __restrict__ totals, u32* __restrict__ listSize,
                        ulonglong2* __restrict__ listKeys, u32* __restrict__ listMeta)
 {
@@ -273,7 +275,7 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
     const long long T0 = (long long)tile * kDirTile;
     const long long G0 = T0 - (long long)b - 1;
     const bool edge = G0 < 0 || G0 + (long long)L.nKeys > (long long)n;
-    const unsigned char* dmax = edge ? dirTileLevels<true>(sm, L, P, n, b, T0) : dirTileLevels<false>(sm, L, P, n, b, T0);
+    const unsigned char* dmax = edge ? dirTileLevels<true>(sm, L, P, n, b, T0, wcap) : dirTileLevels<false>(sm, L, P, n, b, T0, wcap);
     const u32* dm = reinterpret_cast<const u32*>(dmax);
 
     // ---- which positions own K entries: S[p] <= d_{T0+p}, 8 consecutive positions per thread ----
@@ -440,7 +442,7 @@ bool leavesDirectSupported(const cs_context* ctx, u32 bucket)
 }
 
 // enqueue the one-pass build into the workspace arrays leafK[0] / leafOff[0]; ctrl must be zeroed
-cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, u32 cap, cudaStream_t s)
+cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, u32 cap, u32 maxLevel, cudaStream_t s)
 {
     DeviceCtrl* ctrl = ctx->ctrl;
     if (n <= bucket) {                                     // no window of bucket+1 keys: the root is not split
@@ -452,7 +454,7 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
     // the bucket sizes of BASELINE.json's configurations get kernels with the bucket size folded in
     auto* kernel = bucket == 64 ? leavesLevelsKernel<64> : bucket == 16 ? leavesLevelsKernel<16> : leavesLevelsKernel<0>;
-    kernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, ctx->divLevel, ctx->dirFlags, ctx->dirTotals,
+    kernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, maxLevel - 1, ctx->divLevel, ctx->dirFlags, ctx->dirTotals,
                                              ctx->dirListSize, ctx->dirListKeys, ctx->dirListMeta);
     CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
     CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));

@@ -308,7 +308,8 @@ template <bool VEC, int HIST, bool HILBERT>
 __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(const double* __restrict__ x, const double* __restrict__ y,
                                                          const double* __restrict__ z, u64 n,
                                                          const double* __restrict__ box6, u64* __restrict__ keys,
-                                                         u32* gHist, const unsigned short* __restrict__ hilbertTable)
+                                                         u32* gHist, const unsigned short* __restrict__ hilbertTable,
+                                                         u32* __restrict__ keys32)
 {
     constexpr int kHistWords = HIST >= 0 ? (kSortPasses - HIST) * kRadix : 1;
     __shared__ u32 sh[kHistWords];
@@ -325,6 +326,16 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
         const u64 m = mortonKey(px, py, pz, b);
         return HILBERT ? hilbertFromMorton(m, sTab) : m;
     };
+    // keys32 (L = 10): floor(t 2^10) = floor(t 2^21) >> 11 for the same quotient t (scaling by a power of
+    // two is exact) and the clamps agree, so the 30-bit key is the 63-bit key without its low 33 bits
+    auto put2 = [&](u64 i2, u64 k0, u64 k1) {
+        if (HIST < 0 && keys32) *reinterpret_cast<uint2*>(keys32 + i2) = make_uint2((u32)(k0 >> 33), (u32)(k1 >> 33));
+        else stStreamU2(keys + i2, k0, k1);
+    };
+    auto put1 = [&](u64 i1, u64 k) {
+        if (HIST < 0 && keys32) keys32[i1] = (u32)(k >> 33);       // (never together with the 63-bit sort's histograms)
+        else keys[i1] = k;
+    };
     const u64 tid = (u64)blockIdx.x * kKeysBlock + threadIdx.x;
     const u64 nthreads = (u64)gridDim.x * kKeysBlock;
     if (VEC) {
@@ -337,12 +348,12 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
             double2 bx = ldStreamD2(x + 2 * i2), by = ldStreamD2(y + 2 * i2), bz = ldStreamD2(z + 2 * i2);
             u64 k0 = sfcKey(ax.x, ay.x, az.x);
             u64 k1 = sfcKey(ax.y, ay.y, az.y);
-            stStreamU2(keys + 2 * i, k0, k1);
+            put2(2 * i, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
             k0 = sfcKey(bx.x, by.x, bz.x);
             k1 = sfcKey(bx.y, by.y, bz.y);
-            stStreamU2(keys + 2 * i2, k0, k1);
+            put2(2 * i2, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
         }
@@ -352,19 +363,19 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
             double2 vz = ldStreamD2(z + 2 * i);
             u64 k0 = sfcKey(vx.x, vy.x, vz.x);
             u64 k1 = sfcKey(vx.y, vy.y, vz.y);
-            stStreamU2(keys + 2 * i, k0, k1);
+            put2(2 * i, k0, k1);
             histAdd<HIST>(sh, k0);
             histAdd<HIST>(sh, k1);
         }
         if ((n & 1) && tid == 0) {
             u64 k = sfcKey(x[n - 1], y[n - 1], z[n - 1]);
-            keys[n - 1] = k;
+            put1(n - 1, k);
             histAdd<HIST>(sh, k);
         }
     } else {
         for (u64 i = tid; i < n; i += nthreads) {
             u64 k = sfcKey(ldStreamD(x + i), ldStreamD(y + i), ldStreamD(z + i));
-            keys[i] = k;
+            put1(i, k);
             histAdd<HIST>(sh, k);
         }
     }
@@ -378,19 +389,19 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
 }
 
 cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const double* z, u64 n, const double* box6,
-                      u64* keys, int histFrom, int curve, cudaStream_t s)
+                      u64* keys, int histFrom, int curve, cudaStream_t s, u32* keys32)
 {
     StageTimer t(ctx, CS_STAGE_KEYS, s);
     if (n == 0) return CS_OK;
-    const bool vec =
-        ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z) | ((uintptr_t)keys)) & 15u) == 0;
+    const bool vec = ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z)) & 15u) == 0 &&
+                     (keys32 ? (((uintptr_t)keys32) & 7u) == 0 : (((uintptr_t)keys) & 15u) == 0);
     u64 work = vec ? (n + 1) / 2 : n;
     u32 grid = (u32)ctx->numSMs * kKeysBlocksPerSM;
     u32 need = divUp(work, kKeysBlock);
     if (need < grid) grid = need ? need : 1;
     u32* h = ctx->sortHist;
     const unsigned short* tab = ctx->hilbertTable;
-#define CS_KEYS_LAUNCH(V, H, C) keysKernel<V, H, C><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h, tab)
+#define CS_KEYS_LAUNCH(V, H, C) keysKernel<V, H, C><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h, tab, keys32)
 #define CS_KEYS_HIST(V, C)                                        \
     do {                                                          \
         if (histFrom < 0) CS_KEYS_LAUNCH(V, -1, C);               \

@@ -35,6 +35,9 @@ static_assert(kSortBlock >= kRadix, "one thread per digit in the per-digit phase
 static_assert(kSortItems * 32 < 65536 && kSortTile < 65536, "16-bit per-warp digit counters and tile-local slots");
 
 __device__ __forceinline__ u32 digitOf(u64 key, int shift) { return (u32)(key >> shift) & (kRadix - 1); }
+__device__ __forceinline__ u32 digitOf(u32 key, int shift) { return (key >> shift) & (kRadix - 1); }
+__device__ __forceinline__ u64 ldStreamKey(const u64* p) { return ldStreamU64(p); }
+__device__ __forceinline__ u32 ldStreamKey(const u32* p) { return ldStreamU32(p); }
 
 // ---- global digit histograms of all passes ----------------------------------------------------
 // copyTo (nullable): the keys are also copied there (the buffer the first pass reads, see sortSource)
@@ -102,14 +105,16 @@ __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 }
 
 // ---- one radix pass ------------------------------------------------------------------------------
-struct SortSmem {
-    u64 keys[kSortTile];                           // tile in digit order
+template <typename KeyT>
+struct SortSmemT {
+    KeyT keys[kSortTile];                          // tile in digit order
     u32 vals[kSortTile];
     unsigned short warpHist[kSortWarps][kRadix];   // per-warp digit counts, then first tile-local slot of (warp, digit)
     u32 globalBase[kRadix];                        // global slot of (digit d, tile-local slot i) = globalBase[d] + i
     u32 warpSums[kSortWarps + 1];
     u32 tile;
 };
+typedef SortSmemT<u64> SortSmem;                   // 63-bit keys (L = 21); SortSmemT<u32>: 30-bit keys (L = 10)
 
 #ifndef CS_SORT_LOOKBATCH
 #define CS_SORT_LOOKBATCH 4
@@ -166,20 +171,20 @@ __device__ __forceinline__ u32 matchDigit(u32 d)
 }
 
 // keys of one tile: warp-striped, so that (warp, item, lane) order == memory order (stability); pads sort last
-template <bool FULL>
-__device__ __forceinline__ void tileLoadKeys(u64 (&key)[kSortItems], const u64* __restrict__ keysIn, u64 base, u32 valid)
+template <bool FULL, typename KeyT>
+__device__ __forceinline__ void tileLoadKeys(KeyT (&key)[kSortItems], const KeyT* __restrict__ keysIn, u64 base, u32 valid)
 {
     const u32 warpOff = (threadIdx.x >> 5) * (32 * kSortItems) + laneId();
-    const u64* src = keysIn + base + warpOff;
+    const KeyT* src = keysIn + base + warpOff;
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j)
-        key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamU64(src + j * 32) : ~0ull;
+        key[j] = (FULL || warpOff + j * 32 < valid) ? ldStreamKey(src + j * 32) : (KeyT)~(KeyT)0;
 }
 
 // From the loaded keys to the tile staged in digit order in shared memory, with globalBase[] set
 // (ranking, per-digit prefixes, scatter of keys and values, look-back).  Ends with a barrier.
-template <int SHIFT, bool FIRST, bool FULL>
-__device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], const u32* __restrict__ valsIn, u32 tile,
+template <int SHIFT, bool FIRST, bool FULL, typename KeyT>
+__device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSortItems], const u32* __restrict__ valsIn, u32 tile,
                                           u64 base, u32 valid, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
@@ -267,15 +272,15 @@ __device__ __forceinline__ void tileStage(SortSmem& sm, u64 (&key)[kSortItems], 
 }
 
 // write out: consecutive threads -> consecutive slots of a digit's run
-template <int SHIFT, bool FULL>
-__device__ __forceinline__ void tileWriteOut(const SortSmem& sm, u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 valid)
+template <int SHIFT, bool FULL, typename KeyT>
+__device__ __forceinline__ void tileWriteOut(const SortSmemT<KeyT>& sm, KeyT* __restrict__ keysOut, u32* __restrict__ valsOut, u32 valid)
 {
     const u32 tid = threadIdx.x;
 #pragma unroll
     for (int k = 0; k < kSortItems; ++k) {
         const u32 i = tid + k * kSortBlock;
         if (FULL || i < valid) {
-            const u64 kk = sm.keys[i];
+            const KeyT kk = sm.keys[i];
             const u32 dst = sm.globalBase[digitOf(kk, SHIFT)] + i;
             keysOut[dst] = kk;
             valsOut[dst] = sm.vals[i];
@@ -283,12 +288,12 @@ __device__ __forceinline__ void tileWriteOut(const SortSmem& sm, u64* __restrict
     }
 }
 
-template <int SHIFT, bool FIRST, bool FULL>
-__device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict__ keysIn, const u32* __restrict__ valsIn,
-                                             u64* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
+template <int SHIFT, bool FIRST, bool FULL, typename KeyT>
+__device__ __forceinline__ void onesweepTile(SortSmemT<KeyT>& sm, const KeyT* __restrict__ keysIn, const u32* __restrict__ valsIn,
+                                             KeyT* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
                                              const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
-    u64 key[kSortItems];
+    KeyT key[kSortItems];
     const u64 base = (u64)tile * kSortTile;
     tileLoadKeys<FULL>(key, keysIn, base, valid);
     tileStage<SHIFT, FIRST, FULL>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
@@ -296,14 +301,14 @@ __device__ __forceinline__ void onesweepTile(SortSmem& sm, const u64* __restrict
 }
 
 // One tile per CTA (grid = tiles): the passes of the default path and of cs_setSortMode(PLAIN).
-template <int SHIFT, bool FIRST>
+template <int SHIFT, bool FIRST, typename KeyT>
 __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
-    onesweepKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
+    onesweepKernel(const KeyT* __restrict__ keysIn, const u32* __restrict__ valsIn, KeyT* __restrict__ keysOut,
                    u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase /*scanned hist*/, u32* ticket,
                    u64* lookback, u32 epoch)
 {
     extern __shared__ __align__(16) unsigned char smemRaw[];
-    SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
+    SortSmemT<KeyT>& sm = *reinterpret_cast<SortSmemT<KeyT>*>(smemRaw);
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
     u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
@@ -360,24 +365,23 @@ __device__ __forceinline__ u32 groupStartBefore(const u64* __restrict__ keysIn, 
     return b - back;
 }
 
-// Write out with the fix-up, warp-cooperative and free of divergence.  The staged tile is ordered by the
-// bits >= LOW, so a run (equal bits >= LOW) is a contiguous range of slots; "head" = first slot of a run.
-// First every thread marks the heads among its slots into a bit mask in shared memory (headMask, bit i of
-// the mask <-> slot i; slot `valid` counts as a head).  Then every warp takes a range of slots that starts
-// and ends at heads and walks it in windows of up to 32 slots that again start at a head and hold whole
-// runs only (the last, unfinished run of a window opens the next one).  Inside a window a lane learns its
-// run [rs, re) from the window's head bits and counts the run members that must precede it from shuffled
-// low words: d = 1 .. longest run - 1 steps for the whole window; a window of heads only goes straight
-// out.  A run of more than 32 slots is ranked against all of its members read from shared memory.  Slot of
-// an element = run start + (members with smaller low bits) + (earlier members with equal low bits); it is
-// stored straight to its place in the output.
-constexpr int kHeadWords = kSortTile / 32 + 2;
+// Write out with the fix-up.  The staged tile is ordered by the bits >= LOW, so a run (equal bits >= LOW) is a
+// contiguous range of slots; "head" = first slot of a run.  First every thread marks the heads among its slots
+// into a bit mask in shared memory (headMask, bit i <-> slot i; the slots from `valid` on count as heads).  Then,
+// as in the plain write-out, consecutive lanes take consecutive slots, 32 slots (one mask word) per warp step.
+// A lane learns the part of its run inside the warp's 32 slots from the mask word and counts the members there
+// that must precede it from shuffled low words (d = 1 .. longest part - 1 steps for the whole warp; a word of
+// heads only goes straight out).  The (at most two) runs that continue beyond the 32 slots are completed by
+// their lanes from shared memory.  Slot of an element = run start + (members with smaller low bits) + (earlier
+// members with equal low bits); it is stored straight to its place in the output.  A run longer than
+// kFixupMaxRun + 1 raises *redo instead.
+constexpr int kHeadWords = kSortTile / 32 + 2 + (kFixupMaxRun + 64) / 32;   // + sentinels past the tile
 
 template <int SHIFT, int LOW>
 __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headMask, u64* __restrict__ keysOut,
                                                   u32* __restrict__ valsOut, u32 valid, u32* redo)
 {
-    const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
+    const u32 tid = threadIdx.x, lane = laneId();
     const u64* keys = sm.keys;
     const u32* low = reinterpret_cast<const u32*>(sm.keys);
     // ---- head bits: consecutive threads <-> consecutive slots, one ballot per 32 slots -----------------
@@ -388,73 +392,59 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headM
         const u32 H = __ballot_sync(kFull, head);
         if (lane == 0) headMask[i >> 5] = H;
     }
-    if (tid < 2) headMask[kSortTile / 32 + tid] = kFull;
+    if (tid < kHeadWords - kSortTile / 32) headMask[kSortTile / 32 + tid] = kFull;
     __syncthreads();
-    // the 32 head bits of slots x .. x + 31, and the position of the first head at or after x (x <= valid)
-    auto headBits = [&](u32 x) { return __funnelshift_r(headMask[x >> 5], headMask[(x >> 5) + 1], x & 31u); };
-    auto firstHeadFrom = [&](u32 x) -> u32 {
-        for (;; x += 32) {
-            const u32 H = headBits(x);
-            if (H) return x + (u32)__ffs((int)H) - 1u;
-        }
-    };
-    auto emit = [&](u32 q, u32 slot) {
-        const u64 kk = keys[q];
-        const u32 dst = sm.globalBase[digitOf(kk, SHIFT)] + slot;
-        keysOut[dst] = kk;
-        valsOut[dst] = sm.vals[q];
-    };
-    const u32 share = ((valid + kSortWarps - 1) / kSortWarps + 31u) & ~31u;
-    const u32 start = warp * share < valid ? warp * share : valid, stop = (warp + 1) * share < valid ? (warp + 1) * share : valid;
-    u32 p = firstHeadFrom(start);
-    const u32 end = firstHeadFrom(stop);                    // slot `valid` is a head: both are <= valid
     bool tooLong = false;
-    while (p < end) {
-        const u32 H = headBits(p);                          // bit 0 is set: p is a head
-        const bool nextHead = (headMask[(p + 32) >> 5] >> ((p + 32) & 31u)) & 1u;
-        const u32 q = p + lane;
-        if (H == kFull && nextHead) {                       // no two slots share a run (slots from `end` on are heads too)
-            if (q < end) emit(q, q);
-            p += 32;
-            continue;
-        }
-        if (H == 1u && !nextHead) {
-            // ---- one run of more than 32 slots: find its end, rank every member against all of them ----
-            const u32 e = firstHeadFrom(p + 32);
-            if (e - p > kFixupMaxRun + 1) tooLong = true;   // beyond the limit: the gated passes redo the sort
-            else {
-                for (u32 c0 = p; c0 < e; c0 += 32) {
-                    const u32 qc = c0 + lane;
-                    const u32 mc = low[2 * (qc < e ? qc : p)];
-                    u32 before = 0;
-                    for (u32 m = p; m < e; ++m) {
-                        const u32 w = low[2 * m];
-                        before += ((w < mc) || (w == mc && m < qc)) ? 1u : 0u;
-                    }
-                    if (qc < e) emit(qc, p + before);
+#pragma unroll 1
+    for (int k = 0; k < kSortItems; ++k) {
+        const u32 i = tid + k * kSortBlock;
+        const u32 cb = i - lane;                             // first of the warp's 32 slots
+        if (cb >= valid) break;                              // warp-uniform
+        const u32 H = headMask[i >> 5];
+        const bool act = i < valid;
+        const u32 mine = low[2 * (act ? i : cb)];
+        const u32 dstBase = sm.globalBase[digitOf(keys[act ? i : cb], SHIFT)];
+        u32 slot = i;
+        if (H != kFull || !(headMask[(i >> 5) + 1] & 1u)) {  // not heads only, or the last slot's run goes on behind them
+            const u32 below = H & (kFull >> (31u - lane));   // heads at or below this lane
+            const u32 above = (H >> 1) >> lane;              // heads above it, bit 0 <-> lane + 1
+            const u32 rs = below ? 31u - (u32)__clz((int)below) : 0u;           // the run's part in these 32 slots: [rs, re)
+            const u32 re = above ? lane + (u32)__ffs((int)above) : 32u;
+            const u32 roomL = lane - rs, roomR = re - 1u - lane;
+            const u32 longest = __reduce_max_sync(kFull, act ? re - rs : 1u);
+            u32 before = 0;
+            for (u32 d = 1; d < longest; ++d) {
+                const u32 up = __shfl_up_sync(kFull, mine, d), dn = __shfl_down_sync(kFull, mine, d);
+                before += (d <= roomL && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
+                before += (d <= roomR && dn < mine) ? 1u : 0u;      // strictly smaller ones to the right
+            }
+            u32 runStart = cb + rs, runEnd = cb + re;
+            if (act && !below) {                             // the run began before these 32 slots
+                u32 w = (cb - 1u) >> 5, bits = headMask[w], steps = 0;          // cb > 0: slot 0 is a head
+                while (!bits && steps <= kFixupMaxRun / 32) { bits = headMask[--w]; ++steps; }
+                if (!bits) tooLong = true;
+                else {
+                    runStart = (w << 5) + 31u - (u32)__clz((int)bits);
+                    for (u32 m = runStart; m < cb; ++m) before += (low[2 * m] <= mine) ? 1u : 0u;
                 }
             }
-            p = e;
-            continue;
+            if (act && !above) {                             // ... and / or continues behind them
+                u32 w = (cb >> 5) + 1u, bits = headMask[w], steps = 0;          // sentinel words end every run
+                while (!bits && steps <= kFixupMaxRun / 32) { bits = headMask[++w]; ++steps; }
+                if (!bits) tooLong = true;
+                else {
+                    runEnd = (w << 5) + (u32)__ffs((int)bits) - 1u;
+                    for (u32 m = cb + 32u; m < runEnd; ++m) before += (low[2 * m] < mine) ? 1u : 0u;
+                }
+            }
+            if (runEnd - runStart > kFixupMaxRun + 1u) tooLong = true;         // beyond the limit: the redo sorts it all
+            slot = runStart + before;
         }
-        // ---- whole runs inside the window [p, p + wend) -------------------------------------------------------
-        const u32 wend = nextHead ? 32u : 31u - (u32)__clz((int)H);   // the unfinished last run opens the next window
-        const bool act = q < end && lane < wend;
-        const u32 mine = low[2 * (q < end ? q : p)];
-        const u32 rs = 31u - (u32)__clz((int)(H & (0xFFFFFFFFu >> (31u - lane))));   // head at or below this lane
-        const u32 above = (H >> 1) >> lane;                                            // heads above it, bit 0 <-> lane + 1
-        u32 re = above ? lane + (u32)__ffs((int)above) : 32u;
-        re = re < wend ? re : wend;
-        const u32 roomL = lane - rs, roomR = re - 1u - lane;                           // run members to the left / right
-        const u32 longest = __reduce_max_sync(kFull, act ? re - rs : 1u);
-        u32 before = 0;
-        for (u32 d = 1; d < longest; ++d) {
-            const u32 up = __shfl_up_sync(kFull, mine, d), dn = __shfl_down_sync(kFull, mine, d);
-            before += (d <= roomL && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
-            before += (d <= roomR && dn < mine) ? 1u : 0u;      // strictly smaller ones to the right
+        if (act && !tooLong) {
+            const u32 dst = dstBase + slot;
+            keysOut[dst] = keys[i];
+            valsOut[dst] = sm.vals[i];
         }
-        if (act) emit(q, p + rs + before);
-        p += wend;
     }
     if (tooLong) *reinterpret_cast<volatile u32*>(redo) = 1u;
 }
@@ -598,7 +588,7 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 {
     const u32 epoch = nextEpoch(ctx, s);
     const int in = pl.cur, out = in ^ 1;
-    onesweepKernel<SHIFT, FIRST><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
+    onesweepKernel<SHIFT, FIRST, u64><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
         pl.k[in], FIRST ? nullptr : pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
         ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch);
     CS_LAUNCH_CHECK(ctx, "onesweepKernel");
@@ -612,8 +602,9 @@ template <int SHIFT>
 static cudaError_t sortInitShift()
 {
     const int bytes = (int)sizeof(SortSmem);
-    return cudaFuncSetAttribute(onesweepKernel<SHIFT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return cudaFuncSetAttribute(onesweepKernel<SHIFT, false, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
+cs_status sortInit32(cs_context* ctx);
 cs_status sortInit(cs_context* ctx)
 {
     const int bytes = (int)sizeof(SortSmem);
@@ -624,15 +615,15 @@ cs_status sortInit(cs_context* ctx)
     CS_CUDA(ctx, sortInitShift<36>());
     CS_CUDA(ctx, sortInitShift<45>());
     CS_CUDA(ctx, sortInitShift<54>());
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepRedoKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int perSM = 0;
     CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, onesweepRedoKernel, kSortBlock, bytes));
     if (perSM < 1) return fail(ctx, CS_ERR_CUDA, "onesweepRedoKernel does not fit on an SM");
     ctx->redoGrid = (u32)perSM * (u32)ctx->numSMs;
-    return CS_OK;
+    return sortInit32(ctx);
 }
 
 // Where the first radix pass reads the unsorted keys.  The passes alternate between the workspace's
@@ -732,6 +723,84 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     // stream, and the next sort on this context looks at it
     CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedoHint, redo, sizeof(u32), cudaMemcpyDeviceToHost, s));
     return CS_OK;
+}
+
+// ---- 30-bit keys (L = 10) -----------------------------------------------------------------------
+// (u32 key, u32 index): 8 B per element, 16 B per element and pass.  30 bits = 4 digits of 9 bits (the last one 3
+// bits wide): 4 plain passes of the same kernel; with so few bits there is nothing left for a fix-up.  An even
+// number of passes: they start and end in the caller's arrays.
+constexpr int kSortPasses32 = 4;
+
+__global__ void __launch_bounds__(kHistBlock) sortHist32Kernel(const u32* __restrict__ keys, u64 n, u32* gHist)
+{
+    __shared__ u32 sh[kSortPasses32 * kRadix];
+    for (int i = threadIdx.x; i < kSortPasses32 * kRadix; i += kHistBlock) sh[i] = 0;
+    __syncthreads();
+    const u64 tid = (u64)blockIdx.x * kHistBlock + threadIdx.x;
+    const u64 nthreads = (u64)gridDim.x * kHistBlock;
+    auto add = [&](u32 k) {
+#pragma unroll
+        for (int p = 0; p < kSortPasses32; ++p) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
+    };
+    u64 i = tid;
+    for (; i + 3 * nthreads < n; i += 4 * nthreads) {
+        const u32 a = ldStreamU32(keys + i), b = ldStreamU32(keys + i + nthreads), c = ldStreamU32(keys + i + 2 * nthreads),
+                  d = ldStreamU32(keys + i + 3 * nthreads);
+        add(a); add(b); add(c); add(d);
+    }
+    for (; i < n; i += nthreads) add(ldStreamU32(keys + i));
+    __syncthreads();
+    for (int j = threadIdx.x; j < kSortPasses32 * kRadix; j += kHistBlock) {
+        const u32 v = sh[j];
+        if (v) atomicAdd(&gHist[j], v);
+    }
+}
+
+template <int SHIFT, bool FIRST>
+static cs_status launchPass32(cs_context* ctx, u32* const (&k)[2], u32* const (&v)[2], int in, u32 n, u32 tiles, int slot,
+                              cudaStream_t s)
+{
+    const u32 epoch = nextEpoch(ctx, s);
+    onesweepKernel<SHIFT, FIRST, u32><<<tiles, kSortBlock, sizeof(SortSmemT<u32>), s>>>(
+        k[in], FIRST ? nullptr : v[in], k[in ^ 1], v[in ^ 1], n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
+        ctx->sortTickets + slot, ctx->sortLookback, epoch);
+    CS_LAUNCH_CHECK(ctx, "onesweepKernel<u32>");
+    return CS_OK;
+}
+
+cs_status sortInit32(cs_context* ctx)
+{
+    const int bytes = (int)sizeof(SortSmemT<u32>);
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<9, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<27, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    return CS_OK;
+}
+
+cs_status enqueueSort32(cs_context* ctx, u32* keys, u32* perm, u64 n, cudaStream_t s)
+{
+    StageTimer t(ctx, CS_STAGE_SORT, s);
+    if (n == 0) return CS_OK;
+    {
+        StageTimer th(ctx, CS_STAGE_SORT_HIST, s);
+        CS_TRY(enqueueSortReset(ctx, s));
+        u32 grid = (u32)ctx->numSMs * 4;
+        const u32 need = divUp(n, kHistBlock);
+        if (need < grid) grid = need ? need : 1;
+        sortHist32Kernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist);
+        CS_LAUNCH_CHECK(ctx, "sortHist32Kernel");
+        sortScanHistKernel<<<kSortPasses32, kRadix, 0, s>>>(ctx->sortHist);
+        CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
+    }
+    u32* const k[2] = {keys, reinterpret_cast<u32*>(ctx->keysAlt)};
+    u32* const v[2] = {perm, ctx->permAlt};
+    const u32 tiles = divUp(n, kSortTile);
+    StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
+    CS_TRY((launchPass32<0, true>(ctx, k, v, 0, (u32)n, tiles, 0, s)));
+    CS_TRY((launchPass32<9, false>(ctx, k, v, 1, (u32)n, tiles, 1, s)));
+    CS_TRY((launchPass32<18, false>(ctx, k, v, 0, (u32)n, tiles, 2, s)));
+    return launchPass32<27, false>(ctx, k, v, 1, (u32)n, tiles, 3, s);
 }
 
 }  // namespace cs
