@@ -178,8 +178,8 @@ def run_reference(args):
 
 
 def rank_workload(cfg, rank: int):
-    """Replicas only: every rank builds its own tree on its own particle set, so rank r
-    draws the same recipe from another seed."""
+    """Every rank holds its own particle set (weak scaling): rank r draws the same recipe from another seed.  In the
+    sharded mode the sets together are the global domain; in the replicas mode every rank builds its own tree."""
     if rank == 0:
         return cfg
     import dataclasses
@@ -202,6 +202,93 @@ def whole_job_value(n_per_rank: int, world: int, ms_per_step: float) -> float:
     return n_per_rank * world / (ms_per_step * 1e-3) / 1e6
 
 
+def run_sharded(args):
+    """N > 1 (DESIGN.md "Multi-GPU"): the distributed build of PAPER.md:198-204.  Every rank holds its own n particles;
+    a step builds ONE global octree over all of them: box (+ min/max all-reduce), keys and sort on the rank's own
+    particles, rounds of cs_countLeaves -> all-reduce(sum) of N -> cs_rebalance from rank 0's local tree, then the
+    replicated linked octree, its node counts and the SFC partition.  Weak scaling: value = all particles / slowest
+    rank's time."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2307_06345_b200 import binding as cs
+    from paper_2307_06345_b200.distributed import GlobalTreeBuilder
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    if "RANK" in os.environ:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    cfg = _workload(args.workload)
+    n = cfg.n if args.n is None else args.n
+    bucket = cfg.bucket_sizes[-1]
+    x, y, z = rank_workload(cfg, rank).generate(n)
+    dx, dy, dz = (torch.from_numpy(a).cuda() for a in (x, y, z))
+    ctx = cs.Context(max_particles=n, max_leaves=max(1 << 12, world * (n // 4)), device=local_rank)
+    builder = GlobalTreeBuilder(cs, ctx, n, bucket)
+
+    def barrier():
+        if dist.is_initialized():
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 1)):
+        tree = builder.step(dx, dy, dz)
+    barrier()
+    launches0 = ctx.stageTimes()["launches"]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev0.record()
+        for _ in range(args.steps):
+            tree = builder.step(dx, dy, dz)
+        ev1.record()
+        barrier()
+        ms = ev0.elapsed_time(ev1)
+        launches = ctx.stageTimes()["launches"] - launches0
+        # the dominant kernel, timed live by the library's stage timers in a second pass over the same steps
+        ctx.setProfiling(True)
+        sort_ms = passes_ms = 0.0
+        for _ in range(args.steps):
+            builder.step(dx, dy, dz)
+            st = ctx.stageTimes()
+            sort_ms += st["sort"] / args.steps
+            passes_ms += st["sort_passes"] / args.steps
+        ctx.setProfiling(False)
+        barrier()
+    ms = max_over_ranks(ms, world, "cuda")
+    ms_per_step = ms / args.steps
+    if rank == 0:
+        peak, peak_src = _peaks()
+        passes = ctx.sortPasses()
+        pass_ms = passes_ms / passes
+        pass_bytes = sort_pass_bytes_per_particle(passes) * n
+        achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+        tr = _traffic()
+        bounds = cs.u32(tree["bounds"]).tolist()
+        line = {
+            "metric": METRIC, "value": whole_job_value(n, world, ms_per_step), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": cfg.name, "n_particles_per_gpu": n, "n_particles": n * world, "bucketSize": bucket,
+                       "leaves": tree["numLeaves"], "nodes": tree["numNodes"], "global_rounds": tree["rounds"],
+                       "parallelism": "sharded global octree: f per rank, all-reduce(sum) of the leaf counts per round, g "
+                                      "replicated (PAPER.md:198-204); start array = rank 0's local tree, broadcast",
+                       "partition_bounds": bounds if len(bounds) <= 17 else None,
+                       "l2": "inputs larger than L2 (1.5 GiB of coordinates per step and GPU at N=2^26)"},
+            "roofline": {"bound": "hbm", "kernel": "onesweepKernel (one 9-bit radix pass over u64 key + u32 index)",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": (tr or {}).get("onesweep_dram_bytes_per_launch"), "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": pass_bytes, "avg_launch_ms": pass_ms, "launches_per_step": passes},
+            "cpu_baseline": None, "e2e": None, "gpu_launches": int(launches),
+            "stages_ms": {"sort": sort_ms, "sort_passes": passes_ms}, "clocks": clocks.summary(),
+        }
+        print(json.dumps(line), flush=True)
+    if dist.is_initialized():
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -218,7 +305,7 @@ def run_ours(args):
     cfg = _workload(args.workload)
     n = cfg.n if args.n is None else args.n
     bucket = cfg.bucket_sizes[-1]
-    # replicas only: every rank builds its own tree on its own particle set
+    # one GPU, or --mode replicas: every rank builds its own tree on its own particle set
     cfg_rank = rank_workload(cfg, rank)
     x, y, z = cfg_rank.generate(n)
     in_sum = None
@@ -448,7 +535,8 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": cfg.name, "n_particles": n, "bucketSize": bucket, "leaves": tree["numLeaves"],
-                   "nodes": tree["numNodes"], "rounds": tree["rounds"], "parallelism": "replicas only",
+                   "nodes": tree["numNodes"], "rounds": tree["rounds"],
+                   "parallelism": "single GPU" if world == 1 else "replicas only (--mode replicas)",
                    "l2": "inputs larger than L2 (1.5 GiB of coordinates per step at N=2^26)",
                    "input_checksum_first_1Mi": in_sum},
         "roofline": roofline, "full_build": full_build, "cpu_baseline": cpu, "e2e": e2e,
@@ -480,9 +568,15 @@ def main():
                     help="skip the extra legs that time the leaf rounds (H4-H7) and the incremental update")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--mode", default="auto", choices=["auto", "single", "sharded", "replicas"],
+                    help="auto: the one-call build on 1 GPU, the sharded global octree (PAPER.md:198-204) on N > 1; "
+                         "replicas: N independent builds; sharded on 1 GPU runs the distributed step with a world of 1")
     args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "sharded" or (args.mode == "auto" and world > 1):
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -322,6 +322,63 @@ cs_status cs_buildOctree32(cs_context* ctx, const double* x, const double* y, co
                            uint32_t bucketSize, const cs_octree_buffers32* buffers, cs_octree_sizes* sizes,
                            void* stream);
 
+/* ---- the distributed build of Sec. 6, as the calls ONE rank makes (Eq. 11) -----------------------
+ *
+ * "Let us assume that the particles are distributed across multiple compute nodes ... f_glob = f_r o f, where f is
+ * applied to the particles on each node separately and f_r is the element-wise sum of the counts arrays ... computed
+ * with a single call to MPI_Allreduce.  Then we can apply g to N and K as before".  The library
+ * offers f and g as separate calls so that the caller's collective sits between them; it does not communicate:
+ *
+ *     cs_countLeaves(ctx, myKeys, n, K, nl, N)                    f on this rank's particles (async)
+ *     all-reduce(sum, uint32, nl) of N over the ranks             f_r, the caller's (e.g. ncclAllReduce on `stream`)
+ *     cs_rebalance(ctx, K, N, nl, bucket, K', cap, &nl', &changed)  g: identical on every rank
+ *     ... repeat with K', nl' while changed ...
+ *     cs_partitionLeaves(ctx, N, nl, numRanks, bounds)            SFC domain decomposition
+ *     cs_linkOctree(K ...), cs_nodeCountsFromLeaves(K, N ...)     the replicated global octree and its node counts
+ *
+ * All array arguments are device pointers owned by the caller.
+ */
+
+/* cs_countLeaves -- f alone (Eq. 3): counts[i] = number of keys of sortedKeys in [K_i, K_{i+1}).
+ *   sortedKeys: n ascending keys (this rank's particles).  leaves: numLeaves + 1 keys of a cornerstone array
+ *   (precondition: ascending; Eq. 2 is checked by cs_rebalance).  counts: numLeaves uint32 out.
+ *   One merge pass over sortedKeys and leaves.  Does not synchronise.
+ *   Errors: INVALID_ARG, CAPACITY (n > maxParticles, numLeaves > maxLeaves), CUDA. */
+cs_status cs_countLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, const uint64_t* leaves,
+                         uint32_t numLeaves, uint32_t* counts, void* stream);
+
+/* cs_rebalance -- g = g3 o g2 o g1 alone (Eqs. 4-9) on leaves K and given counts N (any counts: one
+ *   rank's, or the element-wise sum over ranks of Eq. 11).  g1: O_i = 8 if N_i > bucketSize and the leaf is above
+ *   depth L (A7); 0 if the leaf is not the first of 8 sibling leaves that hold <= bucketSize particles together (A8;
+ *   the root never merges, A9); else 1.  g2: exclusive prefix sum O'.  g3: K'[O'_i] = K_i, or K'[O'_i + j] = K_i +
+ *   j delta_i / 8 for j = 0..7 (A10); K'[O'_{nl}] = 8^21 (A11).
+ *   newLeaves: out, capacity leafCapacity + 1, must not alias leaves.  newNumLeaves, changed: host out; changed = 0
+ *   iff O_i = 1 for all i (the confirming round: then newLeaves == leaves).  Synchronises `stream`.
+ *   Errors: NOT_CORNERSTONE (leaves violate Eq. 2), CAPACITY (result exceeds leafCapacity or the context's maxLeaves;
+ *   newLeaves untouched), INVALID_ARG, CUDA. */
+cs_status cs_rebalance(cs_context* ctx, const uint64_t* leaves, const uint32_t* counts, uint32_t numLeaves,
+                       uint32_t bucketSize, uint64_t* newLeaves, uint32_t leafCapacity, uint32_t* newNumLeaves,
+                       uint32_t* changed, void* stream);
+
+/* cs_partitionLeaves -- SFC domain decomposition: "the global domain can then be partitioned into n_ranks subdomains
+ *   by grouping K into n_ranks bins of consecutive leaves such that each bin contains approximately N_tot / n_ranks
+ *   of the total particle count".  The paper gives no rule for "approximately"; DESIGN.md reading
+ *   A29: with C_i = N_0 + ... + N_{i-1}, bounds[0] = 0, bounds[numRanks] = numLeaves and, for 0 < r < numRanks,
+ *   bounds[r] = the first leaf boundary i with C_i * numRanks >= r * N_tot (exact integer comparison).  Rank r owns
+ *   the leaves [bounds[r], bounds[r+1]), i.e. the keys [K[bounds[r]], K[bounds[r+1]]).
+ *   counts: numLeaves uint32 (their sum may exceed 2^32).  bounds: numRanks + 1 uint32 out.  Does not synchronise. */
+cs_status cs_partitionLeaves(cs_context* ctx, const uint32_t* counts, uint32_t numLeaves, uint32_t numRanks,
+                             uint32_t* bounds, void* stream);
+
+/* cs_nodeCountsFromLeaves -- particle ranges of the nodes of a linked octree from the counts of its leaves, without
+ *   the particles (the upward pass of PAPER.md:258; for the replicated global octree the counts are the all-reduced
+ *   ones): nodeCount[i] = sum of leafCounts over the leaves inside node i, nodeFirst[i] = sum over the leaves before
+ *   it (sums modulo 2^32: N_tot < 2^32).  leaves / leafCounts: the cornerstone array and its counts; prefixes: NK from
+ *   cs_linkOctree of the same leaves.  Does not synchronise. */
+cs_status cs_nodeCountsFromLeaves(cs_context* ctx, const uint64_t* leaves, const uint32_t* leafCounts, uint32_t numLeaves,
+                                  const uint64_t* prefixes, uint32_t numNodes, uint32_t* nodeFirst, uint32_t* nodeCount,
+                                  void* stream);
+
 /* ---- node properties on the linked octree (first row past the hot path: "additional octree
  *      node properties ... can be stored in separate arrays of length n"; readings A25-A27) --------
  * All arrays are device pointers owned by the caller; the calls enqueue on `stream` and return.  Three-component

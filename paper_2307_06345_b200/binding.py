@@ -102,6 +102,10 @@ def lib():
         "cs_buildLeaves32": (C.c_int, [vp, vp, u64, u32, vp, u32, u32, vp, vp, u32, C.POINTER(u32), C.POINTER(u32), vp]),
         "cs_linkOctree32": (C.c_int, [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp, u32, C.POINTER(u32), vp]),
         "cs_buildOctree32": (C.c_int, [vp, vp, vp, vp, u64, u32, C.POINTER(OctreeBuffers32), C.POINTER(OctreeSizes), vp]),
+        "cs_countLeaves": (C.c_int, [vp, vp, u64, vp, u32, vp, vp]),
+        "cs_rebalance": (C.c_int, [vp, vp, vp, u32, u32, vp, u32, C.POINTER(u32), C.POINTER(u32), vp]),
+        "cs_partitionLeaves": (C.c_int, [vp, vp, u32, u32, vp, vp]),
+        "cs_nodeCountsFromLeaves": (C.c_int, [vp, vp, vp, u32, vp, u32, vp, vp, vp]),
         "cs_gatherParticles": (C.c_int, [vp, vp, vp, vp, vp, u64, vp, vp, vp, vp]),
         "cs_nodeGeometry": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
         "cs_nodeMassCenters": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp, vp]),
@@ -458,6 +462,46 @@ def buildOctree32(ctx: Context, x, y, z, bucketSize: int, buffers: TreeBuffers32
         out[k] = t[k][:nn]
     out.update(numLeaves=nl, numNodes=nn, rounds=int(sizes.rounds), converged=bool(sizes.converged))
     return out
+
+
+# ---- the distributed build of Sec. 6: one rank's calls (include/cornerstone.h, "the distributed build") ------------------
+
+def countLeaves(ctx: Context, sortedKeys, leaves, counts=None):
+    """f alone: counts[i] = keys of sortedKeys in [leaves[i], leaves[i+1]).  No synchronisation."""
+    nl = leaves.numel() - 1
+    if counts is None:
+        counts = _i32(nl, ctx.device)
+    ctx.check(lib().cs_countLeaves(ctx.handle, _ptr(sortedKeys), sortedKeys.numel(), _ptr(leaves), nl, _ptr(counts),
+                                   _stream()))
+    return counts
+
+
+def rebalance(ctx: Context, leaves, counts, bucketSize: int, newLeaves=None, leafCapacity: int | None = None):
+    """g alone on (leaves, counts).  Returns (newLeaves[newNumLeaves + 1], changed)."""
+    nl = leaves.numel() - 1
+    cap = int(leafCapacity if leafCapacity is not None else ctx.max_leaves)
+    if newLeaves is None:
+        newLeaves = _i64(cap + 1, ctx.device)
+    nn, ch = C.c_uint32(0), C.c_uint32(0)
+    ctx.check(lib().cs_rebalance(ctx.handle, _ptr(leaves), _ptr(counts), nl, bucketSize, _ptr(newLeaves), cap,
+                                 C.byref(nn), C.byref(ch), _stream()))
+    return newLeaves[:int(nn.value) + 1], bool(ch.value)
+
+
+def partitionLeaves(ctx: Context, counts, numRanks: int, bounds=None):
+    """bounds[numRanks + 1]: rank r owns the leaves [bounds[r], bounds[r+1]).  No synchronisation."""
+    if bounds is None:
+        bounds = _i32(numRanks + 1, ctx.device)
+    ctx.check(lib().cs_partitionLeaves(ctx.handle, _ptr(counts), counts.numel(), numRanks, _ptr(bounds), _stream()))
+    return bounds
+
+
+def nodeCountsFromLeaves(ctx: Context, leaves, leafCounts, prefixes):
+    n = prefixes.numel()
+    first, count = _i32(n, ctx.device), _i32(n, ctx.device)
+    ctx.check(lib().cs_nodeCountsFromLeaves(ctx.handle, _ptr(leaves), _ptr(leafCounts), leaves.numel() - 1, _ptr(prefixes), n,
+                                            _ptr(first), _ptr(count), _stream()))
+    return first, count
 
 
 # ---- node properties on the linked octree (include/cornerstone.h, last section) ---------------------------

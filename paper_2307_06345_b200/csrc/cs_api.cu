@@ -299,6 +299,68 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
     return CS_OK;
 }
 
+// ---- the distributed build of Sec. 6, one rank's calls (cs_global.cu) ---------------------------------------------------
+
+cs_status cs_countLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, const uint64_t* leaves, uint32_t numLeaves,
+                         uint32_t* counts, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_countLeaves: ctx is null");
+    if ((!sortedKeys && n) || !leaves || !counts) return fail(ctx, CS_ERR_INVALID_ARG, "cs_countLeaves: null pointer");
+    if (numLeaves == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_countLeaves: numLeaves == 0");
+    CS_TRY(checkParticles(ctx, "cs_countLeaves", n));
+    if (numLeaves > ctx->maxLeaves) return fail(ctx, CS_ERR_CAPACITY, "cs_countLeaves: numLeaves exceeds maxLeaves");
+    DeviceGuard g(ctx->device);
+    return enqueueCountLeaves(ctx, (const u64*)sortedKeys, n, (const u64*)leaves, numLeaves, counts, (cudaStream_t)stream);
+}
+
+cs_status cs_rebalance(cs_context* ctx, const uint64_t* leaves, const uint32_t* counts, uint32_t numLeaves,
+                       uint32_t bucketSize, uint64_t* newLeaves, uint32_t leafCapacity, uint32_t* newNumLeaves,
+                       uint32_t* changed, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_rebalance: ctx is null");
+    if (!leaves || !counts || !newLeaves || !newNumLeaves || !changed)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_rebalance: null pointer");
+    if (numLeaves == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_rebalance: numLeaves == 0");
+    if (bucketSize == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_rebalance: bucketSize == 0");
+    if (newLeaves == leaves) return fail(ctx, CS_ERR_INVALID_ARG, "cs_rebalance: in place is not supported");
+    if (numLeaves > ctx->maxLeaves) return fail(ctx, CS_ERR_CAPACITY, "cs_rebalance: numLeaves exceeds maxLeaves");
+    DeviceGuard g(ctx->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const u32 cap = leafCapacity < ctx->maxLeaves ? leafCapacity : ctx->maxLeaves;
+    CS_TRY(enqueueRebalance(ctx, (const u64*)leaves, counts, numLeaves, bucketSize, kL, (u64*)newLeaves, cap, s));
+    CS_TRY(readCtrl(ctx, s));
+    const DeviceCtrl& c = ctx->hostCtrl->c;
+    *newNumLeaves = c.status == CS_OK ? c.numLeaves : 0;
+    *changed = c.status == CS_OK ? (c.converged ? 0u : 1u) : 0u;
+    return statusFromCtrl(ctx, "cs_rebalance");
+}
+
+cs_status cs_partitionLeaves(cs_context* ctx, const uint32_t* counts, uint32_t numLeaves, uint32_t numRanks,
+                             uint32_t* bounds, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_partitionLeaves: ctx is null");
+    if (!counts || !bounds) return fail(ctx, CS_ERR_INVALID_ARG, "cs_partitionLeaves: null pointer");
+    if (numLeaves == 0 || numRanks == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_partitionLeaves: numLeaves or numRanks is 0");
+    if (numLeaves > ctx->maxLeaves) return fail(ctx, CS_ERR_CAPACITY, "cs_partitionLeaves: numLeaves exceeds maxLeaves");
+    DeviceGuard g(ctx->device);
+    return enqueuePartition(ctx, counts, numLeaves, numRanks, bounds, (cudaStream_t)stream);
+}
+
+cs_status cs_nodeCountsFromLeaves(cs_context* ctx, const uint64_t* leaves, const uint32_t* leafCounts, uint32_t numLeaves,
+                                  const uint64_t* prefixes, uint32_t numNodes, uint32_t* nodeFirst, uint32_t* nodeCount,
+                                  void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_nodeCountsFromLeaves: ctx is null");
+    if (numNodes == 0) return CS_OK;
+    if (!leaves || !leafCounts || !prefixes || !nodeFirst || !nodeCount)
+        return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeCountsFromLeaves: null pointer");
+    if (numLeaves == 0) return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeCountsFromLeaves: numLeaves == 0");
+    if (numLeaves > ctx->maxLeaves) return fail(ctx, CS_ERR_CAPACITY, "cs_nodeCountsFromLeaves: numLeaves exceeds maxLeaves");
+    DeviceGuard g(ctx->device);
+    return enqueueNodeCountsFromLeaves(ctx, (const u64*)leaves, leafCounts, numLeaves, (const u64*)prefixes, numNodes,
+                                       nodeFirst, nodeCount, (cudaStream_t)stream);
+}
+
 cs_status cs_gatherParticles(cs_context* ctx, const double* x, const double* y, const double* z, const uint32_t* perm,
                              uint64_t n, double* xs, double* ys, double* zs, void* stream)
 {

@@ -253,6 +253,14 @@ cs_status enqueueNodeCounts(cs_context*, const u64* sortedKeys, u64 n, const u64
 // device-wide exclusive scan of u32 (decoupled look-back): out[i] = sum_{j<i} in[j], out[n] = total
 cs_status enqueueExclusiveScan(cs_context*, const u32* in, u32* out, u32 n, cudaStream_t);
 cs_status readCtrl(cs_context*, cudaStream_t);   // D2H of the control block + stream sync
+// the distributed build (cs_global.cu): f alone, g alone, SFC partition, node counts from leaf counts
+cs_status enqueueCountLeaves(cs_context*, const u64* sortedKeys, u64 n, const u64* leaves, u32 numLeaves, u32* counts,
+                             cudaStream_t);
+cs_status enqueueRebalance(cs_context*, const u64* leaves, const u32* counts, u32 numLeaves, u32 bucketSize, u32 maxLevel,
+                           u64* newLeaves, u32 cap, cudaStream_t);
+cs_status enqueuePartition(cs_context*, const u32* counts, u32 numLeaves, u32 numRanks, u32* bounds, cudaStream_t);
+cs_status enqueueNodeCountsFromLeaves(cs_context*, const u64* leaves, const u32* counts, u32 numLeaves, const u64* prefixes,
+                                      u32 numNodes, u32* nodeFirst, u32* nodeCount, cudaStream_t);
 // node properties on the linked tree (cs_props.cu)
 cs_status enqueueGather(cs_context*, const double* x, const double* y, const double* z, const u32* perm, u64 n,
                         double* xs, double* ys, double* zs, cudaStream_t);

@@ -533,6 +533,21 @@ cs_status leavesInit(cs_context* ctx)
     return CS_OK;
 }
 
+// f (Eq. 3) of a whole array K by the merge pass: ctx->leafK[0] = K (checked against Eq. 2: a violation sets
+// ctrl->status), ctx->leafOff[0][i] = lower_bound(P, K_i) for i = 0 .. nl.  The caller has cleared the control block.
+cs_status enqueueLocateLeaves(cs_context* ctx, const u64* P, u64 n, const u64* K, u32 nl, cudaStream_t s)
+{
+    const u32 persistentGrid = (u32)ctx->numSMs * 8;
+    const u32 locTiles = n ? divUp(n, kLocTile) : 1u;
+    u32 gs = divUp((u64)(nl > locTiles ? nl : locTiles) + 1, 256);
+    if (gs > persistentGrid) gs = persistentGrid;
+    leafSplitKernel<<<gs, 256, 0, s>>>(ctx->ctrl, P, (u32)n, K, nl, ctx->leafK[0], ctx->dirTotals);
+    CS_LAUNCH_CHECK(ctx, "leafSplitKernel");
+    leafLocateKernel<<<locTiles, kLocBlock, 0, s>>>(P, (u32)n, K, ctx->dirTotals, ctx->leafOff[0]);
+    CS_LAUNCH_CHECK(ctx, "leafLocateKernel");
+    return CS_OK;
+}
+
 cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const u64* prevLeaves, u32 prevNumLeaves,
                         u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, u32 maxLevel, cudaStream_t s)
 {
@@ -553,13 +568,7 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
     }
     if (prevLeaves) {
         // f of the previous array by one merge pass over P
-        const u32 locTiles = n ? divUp(n, kLocTile) : 1u;
-        u32 gs = divUp((u64)(prevNumLeaves > locTiles ? prevNumLeaves : locTiles) + 1, 256);
-        if (gs > persistentGrid) gs = persistentGrid;
-        leafSplitKernel<<<gs, 256, 0, s>>>(ctrl, P, (u32)n, prevLeaves, prevNumLeaves, ctx->leafK[0], ctx->dirTotals);
-        CS_LAUNCH_CHECK(ctx, "leafSplitKernel");
-        leafLocateKernel<<<locTiles, kLocBlock, 0, s>>>(P, (u32)n, prevLeaves, ctx->dirTotals, ctx->leafOff[0]);
-        CS_LAUNCH_CHECK(ctx, "leafLocateKernel");
+        CS_TRY(enqueueLocateLeaves(ctx, P, n, prevLeaves, prevNumLeaves, s));
     } else {
         leavesInitRootKernel<<<1, 32, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafOff[0], (u32)n);
         CS_LAUNCH_CHECK(ctx, "leavesInitRootKernel");

@@ -105,11 +105,32 @@ __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 }
 
 // ---- one radix pass ------------------------------------------------------------------------------
+#ifndef CS_SORT_HIST_ROWS
+#define CS_SORT_HIST_ROWS 1
+#endif
+constexpr int kHistStride = kSortWarps + 2;                 // halfwords per digit row
+static_assert(kSortWarps % 2 == 0 && (kHistStride / 2) % 2 == 1, "odd number of words per digit row");
+#if CS_SORT_HIST_ROWS
+constexpr int kHistWords = kRadix * kHistStride / 2;
+#define CS_WH(wh, d) (wh)[(d) * kHistStride]
+#else
+constexpr int kHistWords = kSortWarps * kRadix / 2;
+#define CS_WH(wh, d) (wh)[(d)]
+#endif
+
 template <typename KeyT>
 struct SortSmemT {
     KeyT keys[kSortTile];                          // tile in digit order
     u32 vals[kSortTile];
+#if CS_SORT_HIST_ROWS
+    // per-warp digit counts, then first tile-local slot of (warp, digit): one row per DIGIT (entry of warp w at
+    // [d * kHistStride + w]), rows kHistStride / 2 words apart, an odd number: a warp's look-ups by digit fall into
+    // random banks as before, and the thread that owns a digit reads all the warps' counts as kSortWarps / 2 words
+    // whose bank differs from lane to lane
+    unsigned short warpHist[kRadix * kHistStride];
+#else
     unsigned short warpHist[kSortWarps][kRadix];   // per-warp digit counts, then first tile-local slot of (warp, digit)
+#endif
     u32 globalBase[kRadix];                        // global slot of (digit d, tile-local slot i) = globalBase[d] + i
     u32 warpSums[kSortWarps + 1];
     u32 tile;
@@ -195,16 +216,20 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     u32 rankPk[(kSortItems + 1) / 2];                                        // two 16-bit ranks per register
 #pragma unroll
     for (int j = 0; j < (kSortItems + 1) / 2; ++j) rankPk[j] = 0;
+#if CS_SORT_HIST_ROWS
+    unsigned short* wh = sm.warpHist + warp;
+#else
     unsigned short* wh = sm.warpHist[warp];
+#endif
     const u32 lt = laneMaskLt();
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], SHIFT);
         const u32 peers = matchDigit(d);
         const u32 lower = __popc(peers & lt);
-        const u32 prev = wh[d];
+        const u32 prev = CS_WH(wh, d);
         __syncwarp();
-        if (lower == 0) wh[d] = (unsigned short)(prev + __popc(peers));
+        if (lower == 0) CS_WH(wh, d) = (unsigned short)(prev + __popc(peers));
         __syncwarp();
         rankPk[j >> 1] |= (prev + lower) << ((j & 1) * 16);
     }
@@ -224,8 +249,16 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     // ---- per digit (one thread each): tile count, tile-local start, first slot of every warp ------
     u32 count = 0;
     if (tid < kRadix) {
+#if CS_SORT_HIST_ROWS
+        const u32* row = reinterpret_cast<const u32*>(sm.warpHist) + tid * (kHistStride / 2);
+        u32 both = 0;                                          // two 16-bit sums side by side (a tile has < 2^16 keys)
+#pragma unroll
+        for (int j = 0; j < kSortWarps / 2; ++j) both += row[j];
+        count = (both & 0xFFFFu) + (both >> 16);
+#else
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) count += sm.warpHist[w][tid];
+#endif
         // publish this tile's count at once: the tiles behind it can start their look-back
         const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;   // pads are not elements
         lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, tile == 0 ? kLbPrefix : kLbAggregate, real));
@@ -234,12 +267,25 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     const u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
     if (tid < kRadix) {
         u32 run = start;
+#if CS_SORT_HIST_ROWS
+        u32* row = reinterpret_cast<u32*>(sm.warpHist) + tid * (kHistStride / 2);
+        u32 pk[kSortWarps / 2];
+#pragma unroll
+        for (int j = 0; j < kSortWarps / 2; ++j) pk[j] = row[j];
+#pragma unroll
+        for (int j = 0; j < kSortWarps / 2; ++j) {
+            const u32 lo = pk[j] & 0xFFFFu, hi = pk[j] >> 16;
+            row[j] = run | ((run + lo) << 16);
+            run += lo + hi;
+        }
+#else
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) {
             const u32 c = sm.warpHist[w][tid];
             sm.warpHist[w][tid] = (unsigned short)run;
             run += c;
         }
+#endif
     }
     __syncthreads();
 
@@ -248,7 +294,7 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], SHIFT);
         const u32 r = (rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
-        const u32 pos = wh[d] + r;
+        const u32 pos = CS_WH(wh, d) + r;
         sm.keys[pos] = key[j];
         if (j & 1) rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFFu) | (pos << 16);
         else rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFF0000u) | pos;
@@ -311,8 +357,8 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     SortSmemT<KeyT>& sm = *reinterpret_cast<SortSmemT<KeyT>*>(smemRaw);
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
-    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
-    for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
+    u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
+    for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
     const u32 tile = sm.tile;
     const u64 base = (u64)tile * kSortTile;
@@ -461,8 +507,8 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     __shared__ u32 sHeadMask[kHeadWords];
     const u32 tid = threadIdx.x;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
-    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
-    for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
+    u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
+    for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
     const u32 tile = sm.tile;
     if (tid < 64) {                                         // warps 0 and 1: where this tile starts and ends
@@ -504,12 +550,12 @@ __device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in
 {
     const u32 tid = threadIdx.x;
     const u32 tiles = (a.n + kSortTile - 1) / kSortTile;
-    u32* whWords = reinterpret_cast<u32*>(&sm.warpHist[0][0]);
+    u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
     constexpr int pass = SHIFT / kRadixBits;
     for (;;) {
         __syncthreads();                                   // the previous tile is written out
         if (tid == 0) sm.tile = atomicAdd(a.tickets + pass, 1u);
-        for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortBlock) whWords[i] = 0;
+        for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
         __syncthreads();
         const u32 tile = sm.tile;
         if (tile >= tiles) break;
