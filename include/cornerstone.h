@@ -261,6 +261,13 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
                          uint32_t maxRounds, const cs_octree_buffers* buffers, cs_octree_sizes* sizes,
                          void* stream);
 
+/* cs_setGraphLimit -- cs_buildOctree calls with at most maxParticles particles (default 2^22) are captured as ONE CUDA
+ *   graph when the same arguments (pointers, sizes, modes, stream) are seen twice in a row, and replayed while they
+ *   stay the same: small builds are bound by the cost of launching some 20 kernels, not by the device (a build of
+ *   2^16 particles takes about 0.2 ms enqueued kernel by kernel).  Results are identical.  0 switches graphs off.
+ *   Calls with cs_setProfiling enabled are never replayed (the stage timers need the separate launches). */
+cs_status cs_setGraphLimit(cs_context* ctx, uint64_t maxParticles);
+
 /* cs_buildOctreeHost -- the same path for HOST coordinate buffers (end-to-end form):
  *   copies x, y, z host -> device, runs cs_buildOctree into context-owned device buffers
  *   (the context must have been created with capacities covering n and the tree), and

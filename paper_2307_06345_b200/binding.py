@@ -18,7 +18,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcornerstone_b200.so")
+# CORNERSTONE_B200_LIB: another build of the same library (e.g. one compiled with other tile geometries)
+LIB_PATH = os.environ.get("CORNERSTONE_B200_LIB") or os.path.join(_HERE, "libcornerstone_b200.so")
 
 L = 21
 KEY_END = 1 << 63
@@ -85,6 +86,7 @@ def lib():
         "cs_setLeafMode": (C.c_int, [vp, C.c_int]),
         "cs_setSortMode": (C.c_int, [vp, C.c_int]),
         "cs_sortPasses": (C.c_int, [vp]),
+        "cs_setGraphLimit": (C.c_int, [vp, u64]),
         "cs_computeBox": (C.c_int, [vp, vp, vp, vp, u64, vp, vp]),
         "cs_computeKeys": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
         "cs_computeKeysHilbert": (C.c_int, [vp, vp, vp, vp, u64, vp, vp, vp]),
@@ -203,6 +205,10 @@ class Context:
     def setSortMode(self, mode: int):
         """SORT_AUTO (5 passes + fix-up of the low bits, plain passes behind it if needed) or SORT_PLAIN."""
         self.check(lib().cs_setSortMode(self.handle, int(mode)))
+
+    def setGraphLimit(self, max_particles: int):
+        """buildOctree calls with at most this many particles are replayed as one CUDA graph (0: never)."""
+        self.check(lib().cs_setGraphLimit(self.handle, int(max_particles)))
 
     def sortPasses(self) -> int:
         """Plain radix passes of the next sort (what the stage "sort_passes" times): 4, or 7 in SORT_PLAIN."""

@@ -1,4 +1,5 @@
 // extern "C" entry points of libcornerstone_b200.so (see include/cornerstone.h).
+#include <cstring>
 #include <new>
 
 #include "cs_internal.cuh"
@@ -27,6 +28,68 @@ cs_status checkParticles(cs_context* ctx, const char* fn, uint64_t n)
     if (n > ctx->maxParticles)
         return fail(ctx, CS_ERR_CAPACITY, "%s: n = %llu exceeds the context's maxParticles = %llu", fn,
                     (unsigned long long)n, (unsigned long long)ctx->maxParticles);
+    return CS_OK;
+}
+
+// the stages of cs_buildOctree back to back on `s`, ending with the copy of the control block to the host
+cs_status enqueueBuild(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n, uint32_t bucketSize,
+                       const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, const cs_octree_buffers* b,
+                       bool plain, cudaStream_t s)
+{
+    const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
+    CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
+    CS_TRY(enqueueSortReset(ctx, s));
+    // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
+    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plain, s));
+    CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
+                         (u64*)b->leaves, b->counts, leafCap, kL, s));
+    // link and node counts in one pass: the leaves' particle offsets are still in the workspace
+    CS_TRY(enqueueLink(ctx, (const u64*)b->leaves, &ctx->ctrl->numLeaves, 0, leafCap, (u64*)b->prefixes, b->levels,
+                       b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,
+                       ctx->leafOffFinal, b->nodeFirst, b->nodeCount, s));
+    return enqueueReadCtrl(ctx, s);
+}
+
+// Capture enqueueBuild as a CUDA graph on the context's own stream (the caller's may be the legacy default stream,
+// which cannot be captured) and instantiate it.  The look-back epochs of the captured kernels are relative to a device
+// word that the graph's first node loads from the pinned control block, so that every replay runs in fresh epochs.
+// If the driver refuses (capture or instantiation), graphs are switched off for this context and the caller enqueues
+// the stages directly.
+cs_status captureBuild(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n, uint32_t bucketSize,
+                       const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, const cs_octree_buffers* b,
+                       bool plain)
+{
+    if (ctx->buildGraph) {
+        cudaGraphExecDestroy(ctx->buildGraph);
+        ctx->buildGraph = nullptr;
+    }
+    cudaStream_t cs_ = ctx->captureStream;
+    if (cudaStreamBeginCapture(cs_, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->graphMaxParticles = 0;
+        return CS_OK;
+    }
+    const uint64_t launches0 = ctx->launches;
+    ctx->capturing = true;
+    ctx->captureEpochs = 0;
+    cudaError_t e = cudaMemcpyAsync(ctx->epochWords + 1, &ctx->hostCtrl->epochBase, sizeof(u32), cudaMemcpyHostToDevice, cs_);
+    cs_status st = e == cudaSuccess
+                       ? enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain, cs_)
+                       : CS_ERR_CUDA;
+    ctx->capturing = false;
+    cudaGraph_t graph = nullptr;
+    e = cudaStreamEndCapture(cs_, &graph);
+    ctx->buildGraphLaunches = ctx->launches - launches0;
+    ctx->launches = launches0;
+    ctx->buildGraphEpochs = ctx->captureEpochs;
+    if (st == CS_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&ctx->buildGraph, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (st != CS_OK || e != cudaSuccess || !ctx->buildGraph) {     // not capturable here: enqueue directly from now on
+        cudaGetLastError();
+        ctx->buildGraph = nullptr;
+        ctx->graphMaxParticles = 0;
+    }
     return CS_OK;
 }
 
@@ -186,6 +249,13 @@ cs_status cs_nodeCounts(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n,
                              leafOffsets, nodeToLeaf, nodeFirst, nodeCount, s);
 }
 
+cs_status cs_setGraphLimit(cs_context* ctx, uint64_t maxParticles)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setGraphLimit: ctx is null");
+    ctx->graphMaxParticles = maxParticles;
+    return CS_OK;
+}
+
 cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
                          uint32_t bucketSize, const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds,
                          const cs_octree_buffers* b, cs_octree_sizes* sizes, void* stream)
@@ -208,21 +278,40 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
         return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctree: prevNumLeaves exceeds the leaf capacity");
     DeviceGuard g(ctx->device);
     cudaStream_t s = (cudaStream_t)stream;
-    const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
-
-    CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
-    CS_TRY(enqueueSortReset(ctx, s));
-    // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
     const bool plain = sortDecidePlain(ctx);
-    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
-    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plain, s));
-    CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
-                         (u64*)b->leaves, b->counts, leafCap, kL, s));
-    // link and node counts in one pass: the leaves' particle offsets are still in the workspace
-    CS_TRY(enqueueLink(ctx, (const u64*)b->leaves, &ctx->ctrl->numLeaves, 0, leafCap, (u64*)b->prefixes, b->levels,
-                       b->childOffsets, b->parents, b->levelRange, b->leafToNode, b->nodeToLeaf, b->nodeCapacity,
-                       ctx->leafOffFinal, b->nodeFirst, b->nodeCount, s));
-    CS_TRY(readCtrl(ctx, s));
+    bool replayed = false;
+    if (!ctx->profiling && n <= ctx->graphMaxParticles) {
+        // small inputs are bound by launch overhead: the whole call is one CUDA graph, captured when first seen with
+        // these arguments and replayed while they stay the same (a time-stepping caller passes the same buffers)
+        BuildGraphKey key;
+        memset(&key, 0, sizeof(key));
+        key.x = x; key.y = y; key.z = z; key.n = n; key.bucket = bucketSize; key.prevNumLeaves = prevNumLeaves;
+        key.maxRounds = maxRounds; key.prevLeaves = prevLeaves; key.buffers = *b; key.plain = plain ? 1 : 0;
+        key.curve = ctx->curve; key.leafMode = ctx->leafMode; key.stream = s;
+        const bool known = ctx->buildGraph && memcmp(&key, &ctx->buildGraphKey, sizeof(key)) == 0;
+        if (!known) {
+            // capture on the second call in a row with the same arguments: a one-off call is cheaper enqueued directly
+            if (ctx->buildGraphSeen && memcmp(&key, &ctx->buildGraphCandidate, sizeof(key)) == 0) {
+                CS_TRY(captureBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain));
+                if (ctx->buildGraph) memcpy(&ctx->buildGraphKey, &key, sizeof(key));
+            } else {
+                memcpy(&ctx->buildGraphCandidate, &key, sizeof(key));
+                ctx->buildGraphSeen = true;
+            }
+        }
+        if (ctx->buildGraph && memcmp(&key, &ctx->buildGraphKey, sizeof(key)) == 0) {
+            const u32 first = reserveEpochs(ctx, ctx->buildGraphEpochs ? ctx->buildGraphEpochs : 1u, s);
+            ctx->hostCtrl->epochBase = first - 1u;
+            CS_CUDA(ctx, cudaGraphLaunch(ctx->buildGraph, s));
+            ctx->launches += ctx->buildGraphLaunches;
+            CS_CUDA(ctx, cudaStreamSynchronize(s));
+            replayed = true;
+        }
+    }
+    if (!replayed) {
+        CS_TRY(enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain, s));
+        CS_CUDA(ctx, cudaStreamSynchronize(s));
+    }
     if (ctx->hostCtrl->sortRedo) {                        // deep clustering: skip the short cut for a while
         ctx->autoPlainLeft = kPlainHold;
         ctx->hostCtrl->sortRedoHint = 0;

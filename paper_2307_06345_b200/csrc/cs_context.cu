@@ -30,7 +30,7 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what)
 // ---- workspace layout --------------------------------------------------------------------
 struct Layout {
     size_t keysAlt, permAlt, sortHist, sortLookback, boxPartials, boxCounter, leafK0, leafK1, leafOff0, leafOff1,
-        leafOffFinal, leafTasks, leafOpk, leafTileInfo, divLevel, tileLookback, dirFlags, dirTotals, dirBases, dirListSize, dirListKeys, dirListMeta, linkTileHist, hilbertTable, ctrl, total;
+        leafOffFinal, leafTasks, leafOpk, leafTileInfo, divLevel, tileLookback, dirFlags, dirTotals, dirBases, dirListSize, dirListKeys, dirListMeta, linkTileHist, hilbertTable, epochWords, ctrl, total;
 };
 
 static size_t alignUp(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -71,6 +71,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.dirListMeta = take(dirTiles * kDirectCompact * sizeof(u32));          // 0.5 B per particle
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
     L.hilbertTable = take(24 * 64 * sizeof(unsigned short));
+    L.epochWords = take(64);
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
     return L;
@@ -82,6 +83,11 @@ constexpr int kBoxGridMax = 148 * 8;
 // launches; only when the 30-bit epoch counter would wrap are they zeroed once (epoch 0 is never handed out).
 u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s)
 {
+    if (ctx->capturing) {                                   // relative to the base the replay supplies (cs_api.cu)
+        const u32 first = ctx->captureEpochs + 1;
+        ctx->captureEpochs += count;
+        return first;
+    }
     if (ctx->epoch + count >= (1u << 30)) {
         Layout L = makeLayout(ctx->maxParticles, ctx->maxLeaves, kBoxGridMax);
         cudaError_t e = cudaMemsetAsync(ctx->sortLookback, 0, L.boxPartials - L.sortLookback, s);
@@ -96,19 +102,27 @@ u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s)
 
 u32 nextEpoch(cs_context* ctx, cudaStream_t s) { return reserveEpochs(ctx, 1, s); }
 
-cs_status readCtrl(cs_context* ctx, cudaStream_t s)
+cs_status enqueueReadCtrl(cs_context* ctx, cudaStream_t s)
 {
     CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->c, ctx->ctrl, sizeof(DeviceCtrl), cudaMemcpyDeviceToHost, s));
     CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedo, ctx->sortTickets + kSortRedoSlot, sizeof(u32),
                                  cudaMemcpyDeviceToHost, s));
+    return CS_OK;
+}
+
+cs_status readCtrl(cs_context* ctx, cudaStream_t s)
+{
+    CS_TRY(enqueueReadCtrl(ctx, s));
     CS_CUDA(ctx, cudaStreamSynchronize(s));
     return CS_OK;
 }
 
 // ---- device-wide exclusive scan (g2's building block; decoupled look-back) -----------------
 __global__ void __launch_bounds__(kScanBlock) scanKernel(const u32* __restrict__ in, u32* __restrict__ out, u32 n,
-                                                         u32* ticket, u64* lookback, u32 epoch)
+                                                         u32* ticket, u64* lookback, u32 epoch,
+                                                         const u32* __restrict__ epochBase)
 {
+    epoch += *epochBase;
     __shared__ u32 sTile, sPrefix;
     __shared__ u32 warpSums[kScanBlock / 32 + 1];
     const u32 tiles = (n + kScanTile - 1) / kScanTile;
@@ -166,7 +180,7 @@ cs_status enqueueExclusiveScan(cs_context* ctx, const u32* in, u32* out, u32 n, 
     u32 epoch = nextEpoch(ctx, s);
     u32 tiles = divUp(n, kScanTile);
     u32 grid = tiles < (u32)ctx->numSMs * 8 ? tiles : (u32)ctx->numSMs * 8;
-    scanKernel<<<grid, kScanBlock, 0, s>>>(in, out, n, &ctx->ctrl->scanTicket, ctx->tileLookback, epoch);
+    scanKernel<<<grid, kScanBlock, 0, s>>>(in, out, n, &ctx->ctrl->scanTicket, ctx->tileLookback, epoch, epochBase(ctx));
     CS_LAUNCH_CHECK(ctx, "scanKernel");
     return CS_OK;
 }
@@ -206,6 +220,8 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slab, L.total);
     if (e == cudaSuccess) e = cudaMemset(ctx->slab + L.sortHist, 0, L.total - L.sortHist);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->hostCtrl, sizeof(HostCtrl));
+    if (e == cudaSuccess) memset(ctx->hostCtrl, 0, sizeof(HostCtrl));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->captureStream, cudaStreamNonBlocking);
     for (int i = 0; i < CS_NUM_STAGES && e == cudaSuccess; ++i) {
         e = cudaEventCreate(&ctx->evBegin[i]);
         if (e == cudaSuccess) e = cudaEventCreate(&ctx->evEnd[i]);
@@ -242,6 +258,7 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->dirListMeta = (u32*)(ctx->slab + L.dirListMeta);
     ctx->linkTileHist = (u32*)(ctx->slab + L.linkTileHist);
     ctx->ctrl = (DeviceCtrl*)(ctx->slab + L.ctrl);
+    ctx->epochWords = (u32*)(ctx->slab + L.epochWords);
     ctx->hilbertTable = (unsigned short*)(ctx->slab + L.hilbertTable);
     {
         unsigned short table[24 * 64];
@@ -272,6 +289,8 @@ void cs_destroy(cs_context* ctx)
     if (ctx->hostPathSlab) cudaFree(ctx->hostPathSlab);
     if (ctx->wideSlab) cudaFree(ctx->wideSlab);
     if (ctx->hostCtrl) cudaFreeHost(ctx->hostCtrl);
+    if (ctx->buildGraph) cudaGraphExecDestroy(ctx->buildGraph);
+    if (ctx->captureStream) cudaStreamDestroy(ctx->captureStream);
     for (int i = 0; i < CS_NUM_STAGES; ++i) {
         if (ctx->evBegin[i]) cudaEventDestroy(ctx->evBegin[i]);
         if (ctx->evEnd[i]) cudaEventDestroy(ctx->evEnd[i]);

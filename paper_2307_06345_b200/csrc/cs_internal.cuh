@@ -92,6 +92,19 @@ struct HostCtrl {                // pinned mirror read back once per call
     DeviceCtrl c;
     u32 sortRedo;                // the sort's fix-up gave up and the plain passes ran (cs_sort.cu)
     u32 sortRedoHint;            // the same flag, copied behind every default-plan sort without a synchronisation
+    u32 epochBase;               // replayed builds (CUDA graph): the look-back epoch before this replay, copied to the device by the graph's first node
+};
+
+// A whole cs_buildOctree call captured as a CUDA graph (small inputs are bound by launch overhead, not by the device):
+// valid while every argument and mode it was captured with stays the same.
+struct BuildGraphKey {
+    const void* x; const void* y; const void* z;
+    u64 n;
+    u32 bucket, prevNumLeaves, maxRounds;
+    const void* prevLeaves;
+    cs_octree_buffers buffers;
+    int plain, curve, leafMode;
+    cudaStream_t stream;
 };
 constexpr int kSortRedoSlot = 63;   // ctx->sortTickets[kSortRedoSlot]: that flag on the device
 
@@ -114,6 +127,17 @@ struct cs_context {
     cs::u32* sortTickets = nullptr;
     cs::u64* sortLookback = nullptr;   // [tiles][kRadix]
     cs::u32 epoch = 0;                 // look-back epoch, bumped per launch that uses a look-back array
+    cs::u32* epochWords = nullptr;     // device: [0] = 0 for ever, [1] = epoch base of the replayed graph (kernels add *base to their epoch argument)
+    bool capturing = false;            // a build is being captured: epochs are handed out relative to [1]
+    cs::u32 captureEpochs = 0;         // epochs the captured build uses
+    cudaStream_t captureStream = nullptr;
+    cudaGraphExec_t buildGraph = nullptr;
+    cs::BuildGraphKey buildGraphKey = {};
+    cs::BuildGraphKey buildGraphCandidate = {};   // arguments of the previous call (a graph is captured when they repeat)
+    bool buildGraphSeen = false;
+    cs::u32 buildGraphEpochs = 0;      // epochs one replay consumes
+    uint64_t buildGraphLaunches = 0;   // kernels one replay launches
+    uint64_t graphMaxParticles = 1ull << 22;   // builds of at most this many particles are captured and replayed
     int sortMode = CS_SORT_AUTO;       // cs_setSortMode
     int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after one needed the redo
     cs::u32 redoGrid = 0;              // CTAs of onesweepRedoKernel that are resident together (cooperative launch)
@@ -219,6 +243,7 @@ struct StageTimer {               // records CUDA events around a stage when pro
 
 inline u32 divUp(u64 a, u64 b) { return (u32)((a + b - 1) / b); }
 u32 nextEpoch(cs_context* ctx, cudaStream_t s);
+inline const u32* epochBase(const cs_context* ctx) { return ctx->epochWords + (ctx->capturing ? 1 : 0); }
 u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s);   // first of `count` consecutive look-back epochs
 
 // ---- stage enqueue functions (no synchronisation; sizes device-resident) ---------------
@@ -252,6 +277,7 @@ cs_status enqueueNodeCounts(cs_context*, const u64* sortedKeys, u64 n, const u64
                             u32* nodeFirst, u32* nodeCount, cudaStream_t);
 // device-wide exclusive scan of u32 (decoupled look-back): out[i] = sum_{j<i} in[j], out[n] = total
 cs_status enqueueExclusiveScan(cs_context*, const u32* in, u32* out, u32 n, cudaStream_t);
+cs_status enqueueReadCtrl(cs_context*, cudaStream_t);   // D2H of the control block
 cs_status readCtrl(cs_context*, cudaStream_t);   // D2H of the control block + stream sync
 // the distributed build (cs_global.cu): f alone, g alone, SFC partition, node counts from leaf counts
 cs_status enqueueCountLeaves(cs_context*, const u64* sortedKeys, u64 n, const u64* leaves, u32 numLeaves, u32* counts,

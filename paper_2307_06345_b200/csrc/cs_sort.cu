@@ -105,32 +105,20 @@ __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 }
 
 // ---- one radix pass ------------------------------------------------------------------------------
-#ifndef CS_SORT_HIST_ROWS
-#define CS_SORT_HIST_ROWS 1
+#ifndef CS_SORT_PREFETCH
+#define CS_SORT_PREFETCH 296
 #endif
-constexpr int kHistStride = kSortWarps + 2;                 // halfwords per digit row
-static_assert(kSortWarps % 2 == 0 && (kHistStride / 2) % 2 == 1, "odd number of words per digit row");
-#if CS_SORT_HIST_ROWS
-constexpr int kHistWords = kRadix * kHistStride / 2;
-#define CS_WH(wh, d) (wh)[(d) * kHistStride]
-#else
+__device__ __forceinline__ void bulkPrefetchL2(const void* p, u32 bytes)   // bytes: multiple of 16, p 16-byte aligned
+{
+    if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 constexpr int kHistWords = kSortWarps * kRadix / 2;
-#define CS_WH(wh, d) (wh)[(d)]
-#endif
 
 template <typename KeyT>
 struct SortSmemT {
     KeyT keys[kSortTile];                          // tile in digit order
     u32 vals[kSortTile];
-#if CS_SORT_HIST_ROWS
-    // per-warp digit counts, then first tile-local slot of (warp, digit): one row per DIGIT (entry of warp w at
-    // [d * kHistStride + w]), rows kHistStride / 2 words apart, an odd number: a warp's look-ups by digit fall into
-    // random banks as before, and the thread that owns a digit reads all the warps' counts as kSortWarps / 2 words
-    // whose bank differs from lane to lane
-    unsigned short warpHist[kRadix * kHistStride];
-#else
     unsigned short warpHist[kSortWarps][kRadix];   // per-warp digit counts, then first tile-local slot of (warp, digit)
-#endif
     u32 globalBase[kRadix];                        // global slot of (digit d, tile-local slot i) = globalBase[d] + i
     u32 warpSums[kSortWarps + 1];
     u32 tile;
@@ -216,20 +204,16 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     u32 rankPk[(kSortItems + 1) / 2];                                        // two 16-bit ranks per register
 #pragma unroll
     for (int j = 0; j < (kSortItems + 1) / 2; ++j) rankPk[j] = 0;
-#if CS_SORT_HIST_ROWS
-    unsigned short* wh = sm.warpHist + warp;
-#else
     unsigned short* wh = sm.warpHist[warp];
-#endif
     const u32 lt = laneMaskLt();
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], SHIFT);
         const u32 peers = matchDigit(d);
         const u32 lower = __popc(peers & lt);
-        const u32 prev = CS_WH(wh, d);
+        const u32 prev = wh[d];
         __syncwarp();
-        if (lower == 0) CS_WH(wh, d) = (unsigned short)(prev + __popc(peers));
+        if (lower == 0) wh[d] = (unsigned short)(prev + __popc(peers));
         __syncwarp();
         rankPk[j >> 1] |= (prev + lower) << ((j & 1) * 16);
     }
@@ -249,16 +233,8 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     // ---- per digit (one thread each): tile count, tile-local start, first slot of every warp ------
     u32 count = 0;
     if (tid < kRadix) {
-#if CS_SORT_HIST_ROWS
-        const u32* row = reinterpret_cast<const u32*>(sm.warpHist) + tid * (kHistStride / 2);
-        u32 both = 0;                                          // two 16-bit sums side by side (a tile has < 2^16 keys)
-#pragma unroll
-        for (int j = 0; j < kSortWarps / 2; ++j) both += row[j];
-        count = (both & 0xFFFFu) + (both >> 16);
-#else
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) count += sm.warpHist[w][tid];
-#endif
         // publish this tile's count at once: the tiles behind it can start their look-back
         const u32 real = (!FULL && tid == kRadix - 1) ? count - (kSortTile - valid) : count;   // pads are not elements
         lbStore(lookback + (size_t)tile * kRadix + tid, lbPack(epoch, tile == 0 ? kLbPrefix : kLbAggregate, real));
@@ -267,25 +243,12 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     const u32 start = blockExclusiveScan<kSortBlock>(count, sm.warpSums, &total);
     if (tid < kRadix) {
         u32 run = start;
-#if CS_SORT_HIST_ROWS
-        u32* row = reinterpret_cast<u32*>(sm.warpHist) + tid * (kHistStride / 2);
-        u32 pk[kSortWarps / 2];
-#pragma unroll
-        for (int j = 0; j < kSortWarps / 2; ++j) pk[j] = row[j];
-#pragma unroll
-        for (int j = 0; j < kSortWarps / 2; ++j) {
-            const u32 lo = pk[j] & 0xFFFFu, hi = pk[j] >> 16;
-            row[j] = run | ((run + lo) << 16);
-            run += lo + hi;
-        }
-#else
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) {
             const u32 c = sm.warpHist[w][tid];
             sm.warpHist[w][tid] = (unsigned short)run;
             run += c;
         }
-#endif
     }
     __syncthreads();
 
@@ -294,7 +257,7 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], SHIFT);
         const u32 r = (rankPk[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
-        const u32 pos = CS_WH(wh, d) + r;
+        const u32 pos = wh[d] + r;
         sm.keys[pos] = key[j];
         if (j & 1) rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFFu) | (pos << 16);
         else rankPk[j >> 1] = (rankPk[j >> 1] & 0xFFFF0000u) | pos;
@@ -351,12 +314,25 @@ template <int SHIFT, bool FIRST, typename KeyT>
 __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     onesweepKernel(const KeyT* __restrict__ keysIn, const u32* __restrict__ valsIn, KeyT* __restrict__ keysOut,
                    u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase /*scanned hist*/, u32* ticket,
-                   u64* lookback, u32 epoch)
+                   u64* lookback, u32 epoch, const u32* __restrict__ epochBase)
 {
+    epoch += *epochBase;
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmemT<KeyT>& sm = *reinterpret_cast<SortSmemT<KeyT>*>(smemRaw);
     const u32 tid = threadIdx.x;
-    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+    if (tid == 0) {
+        const u32 t = atomicAdd(ticket, 1u);
+        sm.tile = t;
+#if CS_SORT_PREFETCH
+        // the tile that a CTA will pick up one generation of resident CTAs from now: on its way into L2 already
+        const u64 pb = ((u64)t + CS_SORT_PREFETCH) * kSortTile;
+        if (pb < n) {
+            const u32 cnt = (u32)((n - pb) < (u64)kSortTile ? (n - pb) : (u64)kSortTile);
+            bulkPrefetchL2(keysIn + pb, (cnt * (u32)sizeof(KeyT)) & ~15u);
+            if (!FIRST) bulkPrefetchL2(valsIn + pb, (cnt * 4u) & ~15u);
+        }
+#endif
+    }
     u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
     for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
@@ -499,8 +475,9 @@ template <int SHIFT, int LOW>
 __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     onesweepLastKernel(const u64* __restrict__ keysIn, const u32* __restrict__ valsIn, u64* __restrict__ keysOut,
                        u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase, u32* ticket, u64* lookback,
-                       u32 epoch, u32* redo)
+                       u32 epoch, const u32* __restrict__ epochBase, u32* redo)
 {
+    epoch += *epochBase;
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
     __shared__ u32 sCut[2];
@@ -541,12 +518,13 @@ struct RedoArgs {
     u32* hist;                  // [kSortPasses][kRadix]: scanned for the digits >= kTopFirst, zero below
     u32* tickets;               // kSortPasses ticket counters
     u64* lookback;
-    u32 epoch0;                 // pass p uses look-back epoch epoch0 + p
+    u32 epoch0;                 // pass p uses look-back epoch epoch0 + *epochBase + p
+    const u32* epochBase;
     const u32* gate;
 };
 
 template <int SHIFT>
-__device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in)
+__device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in, u32 epoch0)
 {
     const u32 tid = threadIdx.x;
     const u32 tiles = (a.n + kSortTile - 1) / kSortTile;
@@ -563,10 +541,10 @@ __device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in
         const u32 valid = (u32)((a.n - base) < (u64)kSortTile ? (a.n - base) : (u64)kSortTile);
         if (valid == kSortTile)
             onesweepTile<SHIFT, false, true>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
-                                             a.hist + pass * kRadix, a.lookback, a.epoch0 + pass);
+                                             a.hist + pass * kRadix, a.lookback, epoch0 + pass);
         else
             onesweepTile<SHIFT, false, false>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
-                                              a.hist + pass * kRadix, a.lookback, a.epoch0 + pass);
+                                              a.hist + pass * kRadix, a.lookback, epoch0 + pass);
     }
 }
 
@@ -576,6 +554,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks) onesweepRedoKernel
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
     if (*reinterpret_cast<const volatile u32*>(a.gate) == 0) return;
     cg::grid_group grid = cg::this_grid();
+    const u32 epoch0 = a.epoch0 + *a.epochBase;
     const u32 tid = threadIdx.x;
     {   // digit counts of the passes the key kernel did not count (zero so far), then their exclusive scans
         u32* sh = reinterpret_cast<u32*>(smemRaw);
@@ -602,13 +581,13 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks) onesweepRedoKernel
         }
         grid.sync();
     }
-    redoPass<0>(sm, a, 0);  grid.sync();
-    redoPass<9>(sm, a, 1);  grid.sync();
-    redoPass<18>(sm, a, 0); grid.sync();
-    redoPass<27>(sm, a, 1); grid.sync();
-    redoPass<36>(sm, a, 0); grid.sync();
-    redoPass<45>(sm, a, 1); grid.sync();
-    redoPass<54>(sm, a, 0);
+    redoPass<0>(sm, a, 0, epoch0);  grid.sync();
+    redoPass<9>(sm, a, 1, epoch0);  grid.sync();
+    redoPass<18>(sm, a, 0, epoch0); grid.sync();
+    redoPass<27>(sm, a, 1, epoch0); grid.sync();
+    redoPass<36>(sm, a, 0, epoch0); grid.sync();
+    redoPass<45>(sm, a, 1, epoch0); grid.sync();
+    redoPass<54>(sm, a, 0, epoch0);
 }
 
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
@@ -636,7 +615,7 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
     const int in = pl.cur, out = in ^ 1;
     onesweepKernel<SHIFT, FIRST, u64><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
         pl.k[in], FIRST ? nullptr : pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
-        ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch);
+        ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, epochBase(ctx));
     CS_LAUNCH_CHECK(ctx, "onesweepKernel");
     pl.cur = out;
     return CS_OK;
@@ -746,7 +725,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         const int in = pl.cur, out = in ^ 1;
         onesweepLastKernel<54, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
             pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + 6 * kRadix, ctx->sortTickets + pl.ticketSlot++,
-            ctx->sortLookback, epoch, redo);
+            ctx->sortLookback, epoch, epochBase(ctx), redo);
         CS_LAUNCH_CHECK(ctx, "onesweepLastKernel");
     }
     // gated redo from the input of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
@@ -759,6 +738,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     a.tickets = ctx->sortTickets + pl.ticketSlot;
     a.lookback = ctx->sortLookback;
     a.epoch0 = reserveEpochs(ctx, kSortPasses, s);
+    a.epochBase = epochBase(ctx);
     a.gate = redo;
     const u32 grid = pl.tiles < ctx->redoGrid ? pl.tiles : ctx->redoGrid;
     void* args[] = {(void*)&a};
@@ -809,7 +789,7 @@ static cs_status launchPass32(cs_context* ctx, u32* const (&k)[2], u32* const (&
     const u32 epoch = nextEpoch(ctx, s);
     onesweepKernel<SHIFT, FIRST, u32><<<tiles, kSortBlock, sizeof(SortSmemT<u32>), s>>>(
         k[in], FIRST ? nullptr : v[in], k[in ^ 1], v[in ^ 1], n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
-        ctx->sortTickets + slot, ctx->sortLookback, epoch);
+        ctx->sortTickets + slot, ctx->sortLookback, epoch, epochBase(ctx));
     CS_LAUNCH_CHECK(ctx, "onesweepKernel<u32>");
     return CS_OK;
 }
