@@ -192,7 +192,7 @@ __device__ __forceinline__ void tileLoadKeys(KeyT (&key)[kSortItems], const KeyT
 
 // From the loaded keys to the tile staged in digit order in shared memory, with globalBase[] set
 // (ranking, per-digit prefixes, scatter of keys and values, look-back).  Ends with a barrier.
-template <int SHIFT, bool FIRST, bool FULL, typename KeyT>
+template <int SHIFT, bool FIRST, bool FULL, typename KeyT, bool COLD = false>
 __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSortItems], const u32* __restrict__ valsIn, u32 tile,
                                           u64 base, u32 valid, const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
 {
@@ -209,7 +209,8 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
 #pragma unroll
     for (int j = 0; j < kSortItems; ++j) {
         const u32 d = digitOf(key[j], SHIFT);
-        const u32 peers = matchDigit(d);
+        const u32 peers = COLD ? __match_any_sync(kFull, d) : matchDigit(d);   // COLD: the redo path, where ptxas runs out of
+                                                                                // predicates for the hand-written match
         const u32 lower = __popc(peers & lt);
         const u32 prev = wh[d];
         __syncwarp();
@@ -277,7 +278,6 @@ __device__ __forceinline__ void tileStage(SortSmemT<KeyT>& sm, KeyT (&key)[kSort
         sm.globalBase[tid] = digitBase[tid] + excl - start;
     }
     __syncthreads();
-
 }
 
 // write out: consecutive threads -> consecutive slots of a digit's run
@@ -297,7 +297,7 @@ __device__ __forceinline__ void tileWriteOut(const SortSmemT<KeyT>& sm, KeyT* __
     }
 }
 
-template <int SHIFT, bool FIRST, bool FULL, typename KeyT>
+template <int SHIFT, bool FIRST, bool FULL, typename KeyT, bool COLD = false>
 __device__ __forceinline__ void onesweepTile(SortSmemT<KeyT>& sm, const KeyT* __restrict__ keysIn, const u32* __restrict__ valsIn,
                                              KeyT* __restrict__ keysOut, u32* __restrict__ valsOut, u32 tile, u32 valid,
                                              const u32* __restrict__ digitBase, u64* lookback, u32 epoch)
@@ -305,7 +305,7 @@ __device__ __forceinline__ void onesweepTile(SortSmemT<KeyT>& sm, const KeyT* __
     KeyT key[kSortItems];
     const u64 base = (u64)tile * kSortTile;
     tileLoadKeys<FULL>(key, keysIn, base, valid);
-    tileStage<SHIFT, FIRST, FULL>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
+    tileStage<SHIFT, FIRST, FULL, KeyT, COLD>(sm, key, valsIn, tile, base, valid, digitBase, lookback, epoch);
     tileWriteOut<SHIFT, FULL>(sm, keysOut, valsOut, valid);
 }
 
@@ -391,12 +391,12 @@ __device__ __forceinline__ u32 groupStartBefore(const u64* __restrict__ keysIn, 
 // contiguous range of slots; "head" = first slot of a run.  First every thread marks the heads among its slots
 // into a bit mask in shared memory (headMask, bit i <-> slot i; the slots from `valid` on count as heads).  Then,
 // as in the plain write-out, consecutive lanes take consecutive slots, 32 slots (one mask word) per warp step.
-// A lane learns the part of its run inside the warp's 32 slots from the mask word and counts the members there
-// that must precede it from shuffled low words (d = 1 .. longest part - 1 steps for the whole warp; a word of
-// heads only goes straight out).  The (at most two) runs that continue beyond the 32 slots are completed by
-// their lanes from shared memory.  Slot of an element = run start + (members with smaller low bits) + (earlier
-// members with equal low bits); it is stored straight to its place in the output.  A run longer than
-// kFixupMaxRun + 1 raises *redo instead.
+// A lane finds its run [runStart, runEnd) from the mask words (nearest head at or below it, nearest head above it; a
+// word of heads only goes straight out) and counts the members that must precede it by reading the run's low words
+// from shared memory: slot of an element = run start + (members with smaller low bits) + (earlier members with equal
+// low bits); it is stored straight to its place in the output.  (Counting with shuffles inside the 32 slots plus
+// shared-memory loops for the parts outside measured 1.6 % slower.)  A run longer than kFixupMaxRun + 1 raises *redo
+// instead.
 constexpr int kHeadWords = kSortTile / 32 + 2 + (kFixupMaxRun + 64) / 32;   // + sentinels past the tile
 
 template <int SHIFT, int LOW>
@@ -428,38 +428,32 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headM
         const u32 dstBase = sm.globalBase[digitOf(keys[act ? i : cb], SHIFT)];
         u32 slot = i;
         if (H != kFull || !(headMask[(i >> 5) + 1] & 1u)) {  // not heads only, or the last slot's run goes on behind them
-            const u32 below = H & (kFull >> (31u - lane));   // heads at or below this lane
-            const u32 above = (H >> 1) >> lane;              // heads above it, bit 0 <-> lane + 1
-            const u32 rs = below ? 31u - (u32)__clz((int)below) : 0u;           // the run's part in these 32 slots: [rs, re)
-            const u32 re = above ? lane + (u32)__ffs((int)above) : 32u;
-            const u32 roomL = lane - rs, roomR = re - 1u - lane;
-            const u32 longest = __reduce_max_sync(kFull, act ? re - rs : 1u);
-            u32 before = 0;
-            for (u32 d = 1; d < longest; ++d) {
-                const u32 up = __shfl_up_sync(kFull, mine, d), dn = __shfl_down_sync(kFull, mine, d);
-                before += (d <= roomL && up <= mine) ? 1u : 0u;     // smaller or equal low bits to the left precede
-                before += (d <= roomR && dn < mine) ? 1u : 0u;      // strictly smaller ones to the right
-            }
-            u32 runStart = cb + rs, runEnd = cb + re;
-            if (act && !below) {                             // the run began before these 32 slots
-                u32 w = (cb - 1u) >> 5, bits = headMask[w], steps = 0;          // cb > 0: slot 0 is a head
+            // this lane's run [runStart, runEnd): the nearest head at or below it and the nearest head above it
+            const u32 below = H & (kFull >> (31u - lane));
+            const u32 above = (H >> 1) >> lane;              // bit 0 <-> lane + 1
+            u32 runStart = cb + 31u - (u32)__clz((int)below), runEnd = i + (u32)__ffs((int)above);
+            if (!below) {                                    // it began before these 32 slots (cb > 0: slot 0 is a head)
+                u32 w = (cb - 1u) >> 5, bits = headMask[w], steps = 0;
                 while (!bits && steps <= kFixupMaxRun / 32) { bits = headMask[--w]; ++steps; }
-                if (!bits) tooLong = true;
-                else {
-                    runStart = (w << 5) + 31u - (u32)__clz((int)bits);
-                    for (u32 m = runStart; m < cb; ++m) before += (low[2 * m] <= mine) ? 1u : 0u;
-                }
+                runStart = (w << 5) + 31u - (u32)__clz((int)bits);
+                if (!bits) runStart = 0, tooLong = act;
             }
-            if (act && !above) {                             // ... and / or continues behind them
-                u32 w = (cb >> 5) + 1u, bits = headMask[w], steps = 0;          // sentinel words end every run
+            if (!above) {                                    // it goes on behind them (sentinel words end every run)
+                u32 w = (cb >> 5) + 1u, bits = headMask[w], steps = 0;
                 while (!bits && steps <= kFixupMaxRun / 32) { bits = headMask[++w]; ++steps; }
-                if (!bits) tooLong = true;
-                else {
-                    runEnd = (w << 5) + (u32)__ffs((int)bits) - 1u;
-                    for (u32 m = cb + 32u; m < runEnd; ++m) before += (low[2 * m] < mine) ? 1u : 0u;
-                }
+                runEnd = (w << 5) + (u32)__ffs((int)bits) - 1u;
+                if (!bits) runEnd = runStart, tooLong = act;
             }
-            if (runEnd - runStart > kFixupMaxRun + 1u) tooLong = true;         // beyond the limit: the redo sorts it all
+            if (runEnd - runStart > kFixupMaxRun + 1u) {     // beyond the limit: the redo sorts it all
+                if (act) tooLong = true;
+                runEnd = runStart;
+            }
+            u32 before = 0;                                  // members that precede: smaller low bits, or equal and earlier
+            if (act)
+                for (u32 m = runStart; m < runEnd; ++m) {
+                    const u32 v = low[2 * m];
+                    before += (v < mine || (v == mine && m < i)) ? 1u : 0u;
+                }
             slot = runStart + before;
         }
         if (act && !tooLong) {
@@ -540,15 +534,15 @@ __device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in
         const u64 base = (u64)tile * kSortTile;
         const u32 valid = (u32)((a.n - base) < (u64)kSortTile ? (a.n - base) : (u64)kSortTile);
         if (valid == kSortTile)
-            onesweepTile<SHIFT, false, true>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
+            onesweepTile<SHIFT, false, true, u64, true>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
                                              a.hist + pass * kRadix, a.lookback, epoch0 + pass);
         else
-            onesweepTile<SHIFT, false, false>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
+            onesweepTile<SHIFT, false, false, u64, true>(sm, a.k[in], a.v[in], a.k[in ^ 1], a.v[in ^ 1], tile, valid,
                                               a.hist + pass * kRadix, a.lookback, epoch0 + pass);
     }
 }
 
-__global__ void __launch_bounds__(kSortBlock, kSortMinBlocks) onesweepRedoKernel(const RedoArgs a)
+__global__ void __launch_bounds__(kSortBlock, 1) onesweepRedoKernel(const RedoArgs a)
 {
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
