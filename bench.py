@@ -563,7 +563,7 @@ def run_ours(args):
                  "mass_centers": row(t_com, n * 24 + nn * (12 + 24 + 24)),  # sorted coordinates once + per-node arrays
                  "mac": row(t_mac, nn * (48 + 1)),
                  "mac_pass_fraction": float(mac.float().mean().item()), "nodes": nn,
-                 "note": "cs_gatherParticles, cs_nodeGeometry, cs_nodeMassCenters (22 launches), cs_macMinDistance; "
+                 "note": "cs_gatherParticles, cs_nodeGeometry, cs_nodeMassCenters (2 launches), cs_macMinDistance; "
                          "gather reads 8-byte words at random: 32-byte sectors make its DRAM traffic about 4x the useful bytes"}
         del xs, ys, zs, centers, half, com, mac
 

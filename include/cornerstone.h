@@ -409,7 +409,8 @@ cs_status cs_nodeGeometry(cs_context* ctx, const uint64_t* prefixes, uint32_t nu
  *   internal node's the sum over its 8 children in order of count_c * com_c over its count, an empty node takes
  *   its geometric centre.  xs, ys, zs: coordinates in SFC order (cs_gatherParticles); nodeFirst / nodeCount /
  *   childOffsets / levelRange: as written by cs_linkOctree + cs_nodeCounts or cs_buildOctree; centers: from
- *   cs_nodeGeometry.  One launch per level, deepest first; no host synchronisation. */
+ *   cs_nodeGeometry.  Two launches (the leaves of all levels; then the internal nodes level by level, deepest
+ *   first, behind grid barriers); no host synchronisation. */
 cs_status cs_nodeMassCenters(cs_context* ctx, const double* xs, const double* ys, const double* zs,
                              const uint32_t* nodeFirst, const uint32_t* nodeCount, const uint32_t* childOffsets,
                              const double* centers, const uint32_t* levelRange, uint32_t numNodes, double* com,

@@ -2,7 +2,11 @@
 // SFC order, the nodes' cells, centres of mass by an upward pass, the minimum-distance MAC of Eq. 12.
 // Readings A25-A27 of DESIGN.md fix the operation order; every floating-point operation below is an
 // explicitly rounded intrinsic (no FMA contraction), so the results equal the oracle's bit for bit.
+#include <cooperative_groups.h>
+
 #include "cs_device.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace cs {
 
@@ -59,35 +63,102 @@ __global__ void __launch_bounds__(kPropBlock)
     }
 }
 
-// ---- A26: centres of mass, one level per launch from the deepest to the root -----------------------------------
-// Leaves sum their particles in sorted order, internal nodes their 8 children in order: the oracle's order.
-__global__ void __launch_bounds__(kPropBlock)
-    massCentersLevelKernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
-                           const u32* __restrict__ nodeFirst, const u32* __restrict__ nodeCount,
-                           const u32* __restrict__ childOffsets, const double* __restrict__ centers,
-                           const u32* __restrict__ levelRange, int level, u32 n, double* __restrict__ com)
+// ---- A26: centres of mass by an upward pass ------------------------------------------------------------------------
+// Leaves sum their particles in sorted order, internal nodes their 8 children in order: the oracle's order.  Two
+// launches: the leaves of ALL levels at once (they depend on the particles only: 7/8 of the nodes and all of the
+// particle traffic), then the internal nodes level by level from the deepest to the root inside one cooperative
+// launch with a grid barrier between levels (the level sizes stay on the device).
+// four doubles of one 32-byte sector in one request (p 32-byte aligned; sm_100: 256-bit global loads)
+__device__ __forceinline__ void ldSector(const double* p, double (&v)[4])
 {
-    const u32 begin = levelRange[level], end = levelRange[level + 1];
-    const double* c[3] = {xs, ys, zs};
-    const u32 stride = gridDim.x * kPropBlock;
-    for (u32 i = begin + blockIdx.x * kPropBlock + threadIdx.x; i < end; i += stride) {
-        const u32 count = nodeCount[i], first = nodeFirst[i], co = childOffsets[i];
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];"
+                 : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3])
+                 : "l"(p));
+}
+
+__device__ __forceinline__ void leafCenter(const double* __restrict__ xs, const double* __restrict__ ys,
+                                           const double* __restrict__ zs, const double* __restrict__ centers, u32 first,
+                                           u32 count, u32 i, u32 n, bool sectors, double* __restrict__ com)
+{
+    if (count == 0) {
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            double r;
-            if (count == 0) r = centers[(size_t)d * n + i];
-            else {
-                double s = 0.0;
-                if (co == 0) {
-                    for (u32 j = first; j < first + count; ++j) s = __dadd_rn(s, c[d][j]);
-                } else {
-                    for (u32 k = 0; k < 8; ++k)
-                        s = __dadd_rn(s, __dmul_rn((double)nodeCount[co + k], com[(size_t)d * n + co + k]));
-                }
-                r = __ddiv_rn(s, (double)count);
-            }
-            com[(size_t)d * n + i] = r;
+        for (int d = 0; d < 3; ++d) com[(size_t)d * n + i] = centers[(size_t)d * n + i];
+        return;
+    }
+    // Neighbouring threads read ranges some 150 bytes apart, so every 8-byte load of a warp is its own L1 request; the
+    // middle of the range is therefore read 32 bytes (one sector, 4 coordinates) per request.  The additions stay in
+    // sorted order: three independent chains (x, y, z) that overlap.
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    u32 j = first;
+    const u32 end = first + count;
+    for (; j < end && (j & 3u); ++j) {
+        sx = __dadd_rn(sx, xs[j]);
+        sy = __dadd_rn(sy, ys[j]);
+        sz = __dadd_rn(sz, zs[j]);
+    }
+    for (; sectors && j + 4 <= end; j += 4) {
+        double a[4], b[4], c[4];
+        ldSector(xs + j, a);
+        ldSector(ys + j, b);
+        ldSector(zs + j, c);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            sx = __dadd_rn(sx, a[k]);
+            sy = __dadd_rn(sy, b[k]);
+            sz = __dadd_rn(sz, c[k]);
         }
+    }
+    for (; j < end; ++j) {
+        sx = __dadd_rn(sx, xs[j]);
+        sy = __dadd_rn(sy, ys[j]);
+        sz = __dadd_rn(sz, zs[j]);
+    }
+    const double c = (double)count;
+    com[i] = __ddiv_rn(sx, c);
+    com[(size_t)n + i] = __ddiv_rn(sy, c);
+    com[2 * (size_t)n + i] = __ddiv_rn(sz, c);
+}
+
+__global__ void __launch_bounds__(kPropBlock)
+    massCentersLeafKernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                          const u32* __restrict__ nodeFirst, const u32* __restrict__ nodeCount,
+                          const u32* __restrict__ childOffsets, const double* __restrict__ centers, u32 n,
+                          bool sectors /*xs, ys, zs are 32-byte aligned*/, double* __restrict__ com)
+{
+    const u32 stride = gridDim.x * kPropBlock;
+    for (u32 i = blockIdx.x * kPropBlock + threadIdx.x; i < n; i += stride)
+        if (childOffsets[i] == 0) leafCenter(xs, ys, zs, centers, nodeFirst[i], nodeCount[i], i, n, sectors, com);
+}
+
+__global__ void __launch_bounds__(kPropBlock)
+    massCentersUpKernel(const u32* __restrict__ nodeCount, const u32* __restrict__ childOffsets,
+                        const double* __restrict__ centers, const u32* __restrict__ levelRange, u32 n, double* com)
+{
+    cg::grid_group grid = cg::this_grid();
+    const u32 stride = gridDim.x * kPropBlock;
+    int deepest = kL;
+    while (deepest > 0 && levelRange[deepest] >= n) --deepest;         // levels past the deepest start at n (A19)
+    for (int level = deepest - 1; level >= 0; --level) {               // the deepest level holds leaves only
+        const u32 begin = levelRange[level], end = levelRange[level + 1];
+        for (u32 i = begin + blockIdx.x * kPropBlock + threadIdx.x; i < end; i += stride) {
+            const u32 co = childOffsets[i];
+            if (co == 0) continue;                                      // a leaf: done by the first launch
+            const u32 count = nodeCount[i];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double r;
+                if (count == 0) r = centers[(size_t)d * n + i];
+                else {
+                    double s = 0.0;
+#pragma unroll
+                    for (u32 k = 0; k < 8; ++k)
+                        s = __dadd_rn(s, __dmul_rn((double)nodeCount[co + k], __ldcg(com + (size_t)d * n + co + k)));
+                    r = __ddiv_rn(s, (double)count);
+                }
+                com[(size_t)d * n + i] = r;
+            }
+        }
+        if (level > 0) grid.sync();
     }
 }
 
@@ -146,13 +217,20 @@ cs_status enqueueMassCenters(cs_context* ctx, const double* xs, const double* ys
                              u32 n, double* com, cudaStream_t s)
 {
     if (n == 0) return CS_OK;
-    // the level sizes stay on the device: every level gets a launch sized for the widest level possible
-    const u32 grid = gridFor(ctx, n);
-    for (int level = kL; level >= 0; --level) {
-        massCentersLevelKernel<<<grid, kPropBlock, 0, s>>>(xs, ys, zs, nodeFirst, nodeCount, childOffsets, centers, levelRange,
-                                                           level, n, com);
-        CS_LAUNCH_CHECK(ctx, "massCentersLevelKernel");
-    }
+    const bool sectors = ((((uintptr_t)xs) | ((uintptr_t)ys) | ((uintptr_t)zs)) & 31u) == 0;
+    massCentersLeafKernel<<<gridFor(ctx, n), kPropBlock, 0, s>>>(xs, ys, zs, nodeFirst, nodeCount, childOffsets, centers, n,
+                                                                 sectors, com);
+    CS_LAUNCH_CHECK(ctx, "massCentersLeafKernel");
+    if (n == 1) return CS_OK;
+    int perSM = 0;
+    CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, massCentersUpKernel, kPropBlock, 0));
+    if (perSM < 1) return fail(ctx, CS_ERR_CUDA, "massCentersUpKernel does not fit on an SM");
+    u32 grid = divUp(n / 8 + 1, kPropBlock);                   // the widest level of internal nodes has < n / 8 of them
+    const u32 resident = (u32)perSM * (u32)ctx->numSMs;
+    if (grid > resident) grid = resident;
+    void* args[] = {(void*)&nodeCount, (void*)&childOffsets, (void*)&centers, (void*)&levelRange, (void*)&n, (void*)&com};
+    CS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)massCentersUpKernel, dim3(grid), dim3(kPropBlock), args, 0, s));
+    CS_LAUNCH_CHECK(ctx, "massCentersUpKernel");
     return CS_OK;
 }
 
