@@ -320,6 +320,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmemT<KeyT>& sm = *reinterpret_cast<SortSmemT<KeyT>*>(smemRaw);
     const u32 tid = threadIdx.x;
+    u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
     if (tid == 0) {
         const u32 t = atomicAdd(ticket, 1u);
         sm.tile = t;
@@ -333,7 +334,6 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
         }
 #endif
     }
-    u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
     for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
     const u32 tile = sm.tile;
