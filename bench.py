@@ -259,6 +259,22 @@ def run_sharded(args):
         barrier()
     ms = max_over_ranks(ms, world, "cuda")
     ms_per_step = ms / args.steps
+    # end to end: the rank's coordinates start in pinned HOST memory every step, the partition bounds and the sizes are
+    # read back to the host
+    e2e = None
+    if not args.no_e2e:
+        hx, hy, hz = (torch.from_numpy(a).pin_memory() for a in (x, y, z))
+        e2e_steps = max(1, min(args.steps, 3))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            dx.copy_(hx, non_blocking=True); dy.copy_(hy, non_blocking=True); dz.copy_(hz, non_blocking=True)
+            tree = builder.step(dx, dy, dz)
+            hb = tree["bounds"].cpu()
+        torch.cuda.synchronize()
+        dt = max_over_ranks((time.perf_counter() - t0) / e2e_steps, world, "cuda")
+        e2e = {"value": whole_job_value(n, world, dt * 1e3), "unit": UNIT, "h2d_bytes_per_step": 24 * n * world,
+               "d2h_bytes_per_step": 4 * (world + 1) * world, "ms_per_step": dt * 1e3, "steps": e2e_steps}
     if rank == 0:
         peak, peak_src = _peaks()
         passes = ctx.sortPasses()
@@ -281,7 +297,7 @@ def run_sharded(args):
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": (tr or {}).get("onesweep_dram_bytes_per_launch"), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": pass_bytes, "avg_launch_ms": pass_ms, "launches_per_step": passes},
-            "cpu_baseline": None, "e2e": None, "gpu_launches": int(launches),
+            "cpu_baseline": None, "e2e": e2e, "gpu_launches": int(launches),
             "stages_ms": {"sort": sort_ms, "sort_passes": passes_ms}, "clocks": clocks.summary(),
         }
         print(json.dumps(line), flush=True)
