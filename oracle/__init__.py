@@ -33,6 +33,7 @@ def lib():
         _lib.orc_link.restype = C.c_int64
         _lib.orc_node_counts.restype = None
         _lib.orc_node_geometry.restype = None
+        _lib.orc_node_geometry_hilbert.restype = None
         _lib.orc_centers_of_mass.restype = None
         _lib.orc_mac_min_distance.restype = None
         _lib.orc_set_L.restype = C.c_int
@@ -259,13 +260,15 @@ def full_build(x, y, z, bucket_size, curve="morton"):
     return out
 
 
-def node_geometry(prefixes, box6):
-    """O8: (centers[3, n], halfSizes[3, n]) of the nodes' cells in the bounding box."""
+def node_geometry(prefixes, box6, curve="morton"):
+    """O8 / O8h: (centers[3, n], halfSizes[3, n]) of the nodes' cells in the bounding box; the prefixes are
+    placeholder-bit keys on the Morton or on the Hilbert curve (reading A28)."""
     prefixes, box6 = _u64(prefixes), _f64(box6)
     n = prefixes.size
     centers = np.empty((3, n), dtype=np.float64)
     half = np.empty((3, n), dtype=np.float64)
-    lib().orc_node_geometry(_p(prefixes), C.c_uint32(n), _p(box6), _p(centers), _p(half))
+    fn = lib().orc_node_geometry if curve == "morton" else lib().orc_node_geometry_hilbert
+    fn(_p(prefixes), C.c_uint32(n), _p(box6), _p(centers), _p(half))
     return centers, half
 
 

@@ -16,7 +16,7 @@
 // passages are the "A<n>" items of DESIGN.md ("Readings of the paper").
 // Parity pins: tests/test_oracle_*.py (every function here is pinned).  O8-O10 (node properties, the
 // first row past the hot path) are pinned in tests/test_oracle_props.py; O2h (Hilbert keys), the
-// L = 10 setting, O11 (one round of the distributed build) and O12 (SFC domain decomposition) in
+// O8h (node cells on the Hilbert curve), L = 10, O11 (one round of the distributed build) and O12 (SFC decomposition) in
 // tests/test_oracle_next.py.  PARITY UNPINNED: which 3D Hilbert curve the paper's own code walks --
 // the paper names none (its reference [11] lists millions); O2h's pins fix the properties the paper
 // relies on (bijection, face-continuity, octant by octant), not that choice (reading A28).
@@ -538,6 +538,42 @@ void orc_node_geometry(const uint64_t* prefixes, uint32_t n, const double* box6,
             const double h = e / cells;
             centers[(size_t)d * n + i] = lo + ((double)g[d] + 0.5) * h;
             halfSizes[(size_t)d * n + i] = 0.5 * h;
+        }
+    }
+}
+
+// -------------------------------------------------------------------------------------
+// O8h  node geometry for Hilbert keys (reading A28): the node's cell is found by walking the curve of O2h
+// backwards, digit by digit from the most significant: in orientation (e, d) the w-th sub-cube of the
+// curve is the octant l = T_(e,d)^-1(gc(w)) = rotl(gc(w), d+1) xor e (the inverse of l' = T_(e,d)(l),
+// w = gc^-1(l')), with l = 4 xbit + 2 ybit + zbit; (e, d) are updated as in O2h.  The arithmetic on the
+// cell is O8's (A25).
+// -------------------------------------------------------------------------------------
+void orc_node_geometry_hilbert(const uint64_t* prefixes, uint32_t n, const double* box6, double* centers,
+                               double* halfSizes)
+{
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint64_t p = prefixes[i];
+        int bits = 0;
+        while ((p >> bits) > 1) ++bits;
+        const int level = bits / 3;
+        uint64_t g[3] = {0, 0, 0};
+        unsigned e = 0, d = 0;
+        for (int l = 1; l <= level; ++l) {
+            const unsigned w = (unsigned)((p >> (3 * (level - l))) & 7u);
+            const unsigned oct = rotl3(gc3(w), d + 1) ^ e;
+            g[0] = (g[0] << 1) | ((oct >> 2) & 1u);
+            g[1] = (g[1] << 1) | ((oct >> 1) & 1u);
+            g[2] = (g[2] << 1) | (oct & 1u);
+            e = e ^ rotl3(entry3(w), d + 1);
+            d = (d + dir3(w) + 1) % 3;
+        }
+        const double cells = (double)(1ull << level);
+        for (int k = 0; k < 3; ++k) {
+            const double lo = box6[2 * k], ext = box6[2 * k + 1] - box6[2 * k];
+            const double h = ext / cells;
+            centers[(size_t)k * n + i] = lo + ((double)g[k] + 0.5) * h;
+            halfSizes[(size_t)k * n + i] = 0.5 * h;
         }
     }
 }

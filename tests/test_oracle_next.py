@@ -115,6 +115,48 @@ def test_hilbert_tree_counts_match_brute_force_cube_membership():
 
 # ---- L = 10: 30-bit keys ------------------------------------------------------------------------------
 
+def test_hilbert_node_cells_invert_the_key_encoding():
+    """O8h walks the curve backwards.  Pin: for random cells of the 2^m grid, the cell decoded from the placeholder-bit
+    key (1 followed by the m Hilbert digits of the cell, O2h) is that cell again; with the box [0, 2^m]^3 its centre is
+    (g + 0.5) and its half size 0.5 exactly."""
+    rng = np.random.default_rng(11)
+    for m in (1, 2, 3, 5, 8, 13, 21):
+        g = rng.integers(0, 1 << m, (3, 4000), dtype=np.uint32)
+        h = oracle.hilbert_from_grid(g[0], g[1], g[2], m)
+        prefixes = h | (np.uint64(1) << np.uint64(3 * m))
+        box = np.array([0.0, float(1 << m)] * 3)
+        c, half = oracle.node_geometry(prefixes, box, curve="hilbert")
+        for d in range(3):
+            assert np.array_equal(c[d], g[d].astype(np.float64) + 0.5), (m, d)
+        assert np.all(half == 0.5)
+    c, half = oracle.node_geometry(np.array([1], dtype=np.uint64), np.array([-1.0, 3.0, 0.0, 2.0, 5.0, 6.0]), curve="hilbert")
+    assert c[:, 0].tolist() == [1.0, 1.0, 5.5] and half[:, 0].tolist() == [2.0, 1.0, 0.5]          # the root is the box
+
+
+def test_hilbert_node_cells_contain_their_particles_and_children_tile_parents():
+    """Every particle lies in the cell of the leaf that holds it, and the 8 children of an internal node are the 8
+    octants of its cell (in the curve's order, not in Morton order): the geometry belongs to the tree of Hilbert keys."""
+    x, y, z = W.plummer(20_000, W.BASE_SEED + 77)
+    r = oracle.full_build(x, y, z, 16, curve="hilbert")
+    c, h = oracle.node_geometry(r["prefixes"], r["box"], curve="hilbert")
+    xs = [a[r["perm"]] for a in (x, y, z)]
+    leaf_nodes = r["leafToNode"]
+    node_of_particle = np.repeat(leaf_nodes, r["counts"])
+    for d in range(3):
+        lo, hi = c[d] - h[d], c[d] + h[d]
+        eps = 1e-9 * (r["box"][2 * d + 1] - r["box"][2 * d])
+        assert np.all(xs[d] >= lo[node_of_particle] - eps) and np.all(xs[d] <= hi[node_of_particle] + eps), d
+    internal = np.nonzero(r["childOffsets"])[0]
+    for i in internal[:: max(1, internal.size // 300)]:
+        kids = r["childOffsets"][i] + np.arange(8)
+        octants = set()
+        for k in kids:
+            assert np.allclose(h[:, k], 0.5 * h[:, i], rtol=1e-12)
+            octants.add(tuple(bool(c[d, k] > c[d, i]) for d in range(3)))
+            assert np.all(np.abs(c[:, k] - c[:, i]) <= 0.5000001 * h[:, i])
+        assert len(octants) == 8
+
+
 def test_keys_with_10_levels_are_the_top_10_digits_of_the_21_level_keys():
     """floor(t 2^10) = floor(floor(t 2^21) / 2^11) for every t >= 0 (scaling by a power of two is exact), and the clamps
     agree, so the 30-bit key is the 63-bit key shifted right by 33 bits -- for Morton and for Hilbert keys."""
