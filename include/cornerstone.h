@@ -111,7 +111,7 @@ cs_status cs_computeKeys(cs_context* ctx, const double* x, const double* y, cons
  *   The paper gives no encoding; reading A28 takes the curve of the Butz algorithm in Hamilton's
  *   formulation: octants of a cube in reflected-Gray-code order, sub-cube w entered at corner e(w) and left
  *   along axis d(w).  Cells of consecutive keys share a face.  Arguments and errors as cs_computeKeys.
- *   (cs_nodeGeometry decodes Morton prefixes only.) */
+ *   (Node cells of such a tree: cs_nodeGeometryHilbert.) */
 cs_status cs_computeKeysHilbert(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
                                 const double* box6, uint64_t* keys, void* stream);
 
@@ -403,6 +403,13 @@ cs_status cs_gatherParticles(cs_context* ctx, const double* x, const double* y, 
  *   binary64 rounding per operation.  box6: dev, as written by cs_computeBox. */
 cs_status cs_nodeGeometry(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
                           double* centers, double* halfSizes, void* stream);
+
+/* cs_nodeGeometryHilbert -- the same for a tree built on Hilbert keys (cs_computeKeysHilbert / cs_setCurve; DESIGN.md
+ *   reading A28): the digits of NK are positions along the curve, and the cell is found by walking the curve backwards
+ *   from the root (in orientation (e, d) the w-th sub-cube is the octant rotl(gc(w), d + 1) xor e).  Same arithmetic on
+ *   the cell, same arguments. */
+cs_status cs_nodeGeometryHilbert(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
+                                 double* centers, double* halfSizes, void* stream);
 
 /* cs_nodeMassCenters -- centres of mass (unit masses) by an upward pass over the links: a leaf's
  *   is the sum of its particles' sorted coordinates xs[first .. first + count) in that order over count, an

@@ -110,6 +110,7 @@ def lib():
         "cs_nodeCountsFromLeaves": (C.c_int, [vp, vp, vp, u32, vp, u32, vp, vp, vp]),
         "cs_gatherParticles": (C.c_int, [vp, vp, vp, vp, vp, u64, vp, vp, vp, vp]),
         "cs_nodeGeometry": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
+        "cs_nodeGeometryHilbert": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
         "cs_nodeMassCenters": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, u32, vp, vp]),
         "cs_macMinDistance": (C.c_int, [vp, vp, vp, u32, C.POINTER(C.c_double), C.c_double, vp, vp]),
     }
@@ -520,12 +521,13 @@ def gatherParticles(ctx: Context, x, y, z, perm):
     return tuple(out)
 
 
-def nodeGeometry(ctx: Context, prefixes, box6):
-    """(centers[3, n], halfSizes[3, n]) float64 tensors."""
+def nodeGeometry(ctx: Context, prefixes, box6, curve: int = CURVE_MORTON):
+    """(centers[3, n], halfSizes[3, n]) float64 tensors; curve = the curve the tree's keys lie on."""
     n = prefixes.numel()
     centers = torch.empty((3, n), dtype=torch.float64, device=ctx.device)
     half = torch.empty((3, n), dtype=torch.float64, device=ctx.device)
-    ctx.check(lib().cs_nodeGeometry(ctx.handle, _ptr(prefixes), n, _ptr(box6), _ptr(centers), _ptr(half), _stream()))
+    fn = lib().cs_nodeGeometryHilbert if curve == CURVE_HILBERT else lib().cs_nodeGeometry
+    ctx.check(fn(ctx.handle, _ptr(prefixes), n, _ptr(box6), _ptr(centers), _ptr(half), _stream()))
     return centers, half
 
 

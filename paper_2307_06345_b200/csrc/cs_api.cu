@@ -462,14 +462,27 @@ cs_status cs_gatherParticles(cs_context* ctx, const double* x, const double* y, 
     return enqueueGather(ctx, x, y, z, perm, n, xs, ys, zs, (cudaStream_t)stream);
 }
 
+static cs_status nodeGeometryCall(cs_context* ctx, const char* fn, const uint64_t* prefixes, uint32_t numNodes,
+                                  const double* box6, int curve, double* centers, double* halfSizes, void* stream)
+{
+    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "%s: ctx is null", fn);
+    if (numNodes == 0) return CS_OK;
+    if (!prefixes || !box6 || !centers || !halfSizes) return fail(ctx, CS_ERR_INVALID_ARG, "%s: null pointer", fn);
+    DeviceGuard g(ctx->device);
+    return enqueueNodeGeometry(ctx, (const u64*)prefixes, numNodes, box6, curve, centers, halfSizes, (cudaStream_t)stream);
+}
+
 cs_status cs_nodeGeometry(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
                           double* centers, double* halfSizes, void* stream)
 {
-    if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_nodeGeometry: ctx is null");
-    if (numNodes == 0) return CS_OK;
-    if (!prefixes || !box6 || !centers || !halfSizes) return fail(ctx, CS_ERR_INVALID_ARG, "cs_nodeGeometry: null pointer");
-    DeviceGuard g(ctx->device);
-    return enqueueNodeGeometry(ctx, (const u64*)prefixes, numNodes, box6, centers, halfSizes, (cudaStream_t)stream);
+    return nodeGeometryCall(ctx, "cs_nodeGeometry", prefixes, numNodes, box6, CS_CURVE_MORTON, centers, halfSizes, stream);
+}
+
+cs_status cs_nodeGeometryHilbert(cs_context* ctx, const uint64_t* prefixes, uint32_t numNodes, const double* box6,
+                                 double* centers, double* halfSizes, void* stream)
+{
+    return nodeGeometryCall(ctx, "cs_nodeGeometryHilbert", prefixes, numNodes, box6, CS_CURVE_HILBERT, centers, halfSizes,
+                            stream);
 }
 
 cs_status cs_nodeMassCenters(cs_context* ctx, const double* xs, const double* ys, const double* zs,

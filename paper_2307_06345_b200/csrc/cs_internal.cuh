@@ -144,6 +144,7 @@ struct cs_context {
 
     // keys
     unsigned short* hilbertTable = nullptr;   // [24][64] two-level transitions of the Hilbert curve (cs_particles.cu)
+    unsigned char* hilbertInverse = nullptr;  // [24][8] one-level inverse transitions (node geometry, cs_props.cu)
     int curve = CS_CURVE_MORTON;              // cs_setCurve: the curve cs_buildOctree computes keys on
 
     // box
@@ -253,6 +254,7 @@ cs_status enqueueBox(cs_context*, const double* x, const double* y, const double
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
                       u64* keys, int histFrom, int curve, cudaStream_t, u32* keys32 = nullptr /*30-bit keys instead*/);
 void hilbertBuildTable(unsigned short* table /*[24 * 64], host*/);
+void hilbertBuildInverse(unsigned char* inv /*[24 * 8], host*/);
 cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
 cs_status leavesDirectInit(cs_context*);
 cs_status leavesInit(cs_context*);
@@ -290,7 +292,7 @@ cs_status enqueueNodeCountsFromLeaves(cs_context*, const u64* leaves, const u32*
 // node properties on the linked tree (cs_props.cu)
 cs_status enqueueGather(cs_context*, const double* x, const double* y, const double* z, const u32* perm, u64 n,
                         double* xs, double* ys, double* zs, cudaStream_t);
-cs_status enqueueNodeGeometry(cs_context*, const u64* prefixes, u32 n, const double* box6, double* centers,
+cs_status enqueueNodeGeometry(cs_context*, const u64* prefixes, u32 n, const double* box6, int curve, double* centers,
                               double* halfSizes, cudaStream_t);
 cs_status enqueueMassCenters(cs_context*, const double* xs, const double* ys, const double* zs, const u32* nodeFirst,
                              const u32* nodeCount, const u32* childOffsets, const double* centers, const u32* levelRange,

@@ -280,6 +280,18 @@ void hilbertBuildTable(unsigned short* table /*[24 * 64]*/)
         }
 }
 
+// One-level inverse transitions for the node geometry (cs_props.cu): inv[state][Hilbert digit w] = octant l | next
+// state << 3 (24 x 8 bytes), stored behind the two-level table.
+void hilbertBuildInverse(unsigned char* inv /*[24 * 8]*/)
+{
+    for (u32 s = 0; s < (u32)kHilbertStates; ++s)
+        for (u32 l = 0; l < 8; ++l) {
+            u32 w, next;
+            hilbertStep(s, l, w, next);
+            inv[s * 8 + w] = (unsigned char)(l | (next << 3));
+        }
+}
+
 __device__ __forceinline__ u64 hilbertFromMorton(u64 m, const unsigned short* __restrict__ tab)
 {
     u32 ent = tab[kHilbertStart * 64 + (u32)(m >> 60)];               // (0, first digit)

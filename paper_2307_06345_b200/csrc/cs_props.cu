@@ -42,16 +42,37 @@ __device__ __forceinline__ u32 compact3(u64 v)
     return (u32)v;
 }
 
+// HILBERT (reading A28): the prefix holds Hilbert digits; the curve is walked backwards from the root, one table
+// look-up per level: inv[state][w] = octant (4x + 2y + z) | next state << 3, start state (e = 0, d = 0) = 0.
+template <bool HILBERT>
 __global__ void __launch_bounds__(kPropBlock)
     nodeGeometryKernel(const u64* __restrict__ prefixes, u32 n, const double* __restrict__ box6,
-                       double* __restrict__ centers, double* __restrict__ halfSizes)
+                       const unsigned char* __restrict__ inv, double* __restrict__ centers, double* __restrict__ halfSizes)
 {
+    __shared__ unsigned char sInv[HILBERT ? 24 * 8 : 1];
+    if (HILBERT) {
+        for (int i = threadIdx.x; i < 24 * 8; i += kPropBlock) sInv[i] = inv[i];
+        __syncthreads();
+    }
     const u32 stride = gridDim.x * kPropBlock;
     for (u32 i = blockIdx.x * kPropBlock + threadIdx.x; i < n; i += stride) {
         const u64 p = prefixes[i];
         const int level = (63 - __clzll((long long)p)) / 3;
         const u64 digits = p ^ (1ull << (3 * level));
-        const u32 g[3] = {compact3(digits >> 2), compact3(digits >> 1), compact3(digits)};   // digit = 4x + 2y + z (A3)
+        u32 g[3];
+        if (HILBERT) {
+            u32 state = 0;
+            g[0] = g[1] = g[2] = 0;
+            for (int l = level - 1; l >= 0; --l) {
+                const u32 ent = sInv[state * 8 + ((u32)(digits >> (3 * l)) & 7u)];
+                state = ent >> 3;
+                g[0] = (g[0] << 1) | ((ent >> 2) & 1u);
+                g[1] = (g[1] << 1) | ((ent >> 1) & 1u);
+                g[2] = (g[2] << 1) | (ent & 1u);
+            }
+        } else {
+            g[0] = compact3(digits >> 2); g[1] = compact3(digits >> 1); g[2] = compact3(digits);   // digit = 4x + 2y + z (A3)
+        }
         const double cells = (double)(1ull << level);
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -203,11 +224,14 @@ cs_status enqueueGather(cs_context* ctx, const double* x, const double* y, const
     return CS_OK;
 }
 
-cs_status enqueueNodeGeometry(cs_context* ctx, const u64* prefixes, u32 n, const double* box6, double* centers,
+cs_status enqueueNodeGeometry(cs_context* ctx, const u64* prefixes, u32 n, const double* box6, int curve, double* centers,
                               double* halfSizes, cudaStream_t s)
 {
     if (n == 0) return CS_OK;
-    nodeGeometryKernel<<<gridFor(ctx, n), kPropBlock, 0, s>>>(prefixes, n, box6, centers, halfSizes);
+    if (curve == CS_CURVE_HILBERT)
+        nodeGeometryKernel<true><<<gridFor(ctx, n), kPropBlock, 0, s>>>(prefixes, n, box6, ctx->hilbertInverse, centers, halfSizes);
+    else
+        nodeGeometryKernel<false><<<gridFor(ctx, n), kPropBlock, 0, s>>>(prefixes, n, box6, nullptr, centers, halfSizes);
     CS_LAUNCH_CHECK(ctx, "nodeGeometryKernel");
     return CS_OK;
 }

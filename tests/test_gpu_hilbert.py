@@ -84,3 +84,31 @@ def test_full_build_on_hilbert_keys(cs, cfg_i, n, bucket):
     assert mort["numLeaves"] == got["numLeaves"] and mort["numNodes"] == got["numNodes"]
     assert np.array_equal(cs.u32(mort["levelRange"]), cs.u32(got["levelRange"]))
     ctx.close()
+
+
+def test_node_properties_of_a_hilbert_tree(cs):
+    """cs_nodeGeometryHilbert against O8h, and the rest of the node properties (centres of mass, MAC) on a tree of
+    Hilbert keys: cells of deep and shallow nodes, empty leaves (they take their cell's centre)."""
+    n, bucket = 150_001, 16
+    x, y, z = W.blobs(n, W.BASE_SEED + 91, nblobs=12)
+    ref = oracle.full_build(x, y, z, bucket, curve="hilbert")
+    ctx = cs.Context(max_particles=n, max_leaves=n)
+    ctx.setCurve(cs.CURVE_HILBERT)
+    dx, dy, dz = dev(x), dev(y), dev(z)
+    tree = cs.buildOctree(ctx, dx, dy, dz, bucket)
+    assert np.array_equal(cs.u64(tree["prefixes"]), ref["prefixes"])
+    centers, half = cs.nodeGeometry(ctx, tree["prefixes"], tree["box6"], curve=cs.CURVE_HILBERT)
+    rc, rh = oracle.node_geometry(ref["prefixes"], ref["box"], curve="hilbert")
+    assert np.array_equal(centers.cpu().numpy().view(np.uint64), rc.view(np.uint64))
+    assert np.array_equal(half.cpu().numpy().view(np.uint64), rh.view(np.uint64))
+    mc, _ = cs.nodeGeometry(ctx, tree["prefixes"], tree["box6"])           # read as Morton digits: other cells
+    assert not np.array_equal(mc.cpu().numpy(), rc)
+    xs, ys, zs = cs.gatherParticles(ctx, dx, dy, dz, tree["perm"])
+    com = cs.nodeMassCenters(ctx, xs, ys, zs, tree, centers)
+    rcom = oracle.centers_of_mass(x[ref["perm"]], y[ref["perm"]], z[ref["perm"]], ref["nodeFirst"], ref["nodeCount"],
+                                  ref["childOffsets"], rc)
+    assert np.array_equal(com.cpu().numpy().view(np.uint64), rcom.view(np.uint64))
+    focus = [0.1, 0.2, 0.3, 0.4, 0.5, 0.6]
+    mac = cs.macMinDistance(ctx, centers, half, focus, 0.6)
+    assert np.array_equal(mac.cpu().numpy(), oracle.mac_min_distance(rc, rh, np.array(focus), 0.6))
+    ctx.close()
