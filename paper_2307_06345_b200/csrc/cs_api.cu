@@ -189,7 +189,8 @@ cs_status cs_setSortMode(cs_context* ctx, int mode)
 int cs_sortPasses(const cs_context* ctx)
 {
     if (!ctx) return 0;
-    return (ctx->sortMode == CS_SORT_PLAIN || ctx->autoPlainLeft > 0 || ctx->hostCtrl->sortRedoHint) ? 7 : 4;
+    return (ctx->sortMode == CS_SORT_PLAIN || ctx->autoPlainLeft > 0 || ctx->hostCtrl->sortRedoHint)
+               ? kSortPasses : kSortPasses - 1 - kSortTopFirst;
 }
 
 cs_status cs_setLeafMode(cs_context* ctx, int mode)

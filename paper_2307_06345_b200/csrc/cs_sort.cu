@@ -542,6 +542,16 @@ __device__ __forceinline__ void redoPass(SortSmem& sm, const RedoArgs& a, int in
     }
 }
 
+template <int P>
+__device__ __forceinline__ void redoPasses(SortSmem& sm, const RedoArgs& a, cg::grid_group& grid, u32 epoch0)
+{
+    redoPass<P * kRadixBits>(sm, a, P & 1, epoch0);
+    if constexpr (P + 1 < kSortPasses) {
+        grid.sync();
+        redoPasses<P + 1>(sm, a, grid, epoch0);
+    }
+}
+
 __global__ void __launch_bounds__(kSortBlock, 1) onesweepRedoKernel(const RedoArgs a)
 {
     extern __shared__ __align__(16) unsigned char smemRaw[];
@@ -575,13 +585,14 @@ __global__ void __launch_bounds__(kSortBlock, 1) onesweepRedoKernel(const RedoAr
         }
         grid.sync();
     }
-    redoPass<0>(sm, a, 0, epoch0);  grid.sync();
-    redoPass<9>(sm, a, 1, epoch0);  grid.sync();
-    redoPass<18>(sm, a, 0, epoch0); grid.sync();
-    redoPass<27>(sm, a, 1, epoch0); grid.sync();
-    redoPass<36>(sm, a, 0, epoch0); grid.sync();
-    redoPass<45>(sm, a, 1, epoch0); grid.sync();
-    redoPass<54>(sm, a, 0, epoch0);
+    redoPasses<0>(sm, a, grid, epoch0);
+    if ((kSortPasses & 1) == 0) {                          // an even number of passes ends where it began: move it over
+        grid.sync();
+        for (u64 i = (u64)blockIdx.x * kSortBlock + tid; i < a.n; i += (u64)gridDim.x * kSortBlock) {
+            a.k[1][i] = a.k[0][i];
+            a.v[1][i] = a.v[0][i];
+        }
+    }
 }
 
 cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
@@ -590,9 +601,12 @@ cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
     return CS_OK;
 }
 
-constexpr int kTopPasses = 5;                               // digits 2..6 (bits 18..62); the fifth also orders the low bits
-constexpr int kFixupLow = (kSortPasses - kTopPasses) * kRadixBits;
-static_assert(kSortPasses == 7 && kRadixBits == 9, "the pass plan below is written for 7 digits of 9 bits");
+// The default plan sorts by the digits kTopFirst .. kSortPasses - 1 (the last of them, the key's top digit, in the
+// fused pass that also orders the bits below kFixupLow); the plain plan sorts by all kSortPasses digits.
+constexpr int kFixupLow = kTopFirst * kRadixBits;
+constexpr int kLastShift = (kSortPasses - 1) * kRadixBits;
+static_assert(kFixupLow <= 32 && kTopFirst % 2 == 0 && kTopFirst + 1 < kSortPasses,
+              "the fix-up compares the keys' low words; both plans run the same parity of passes");
 
 struct PassPlan {
     u64* k[2];
@@ -617,26 +631,24 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 
 // The radix kernels need more dynamic shared memory than the default limit: opt in on the context's device
 // (function attributes are per device, so this runs once per cs_create, not once per process).
-template <int SHIFT>
-static cudaError_t sortInitShift()
+template <int P>
+static cudaError_t sortInitPasses()
 {
     const int bytes = (int)sizeof(SortSmem);
-    return cudaFuncSetAttribute(onesweepKernel<SHIFT, false, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    cudaError_t e = cudaFuncSetAttribute(onesweepKernel<P * kRadixBits, false, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if constexpr (P + 1 < kSortPasses) {
+        if (e == cudaSuccess) e = sortInitPasses<P + 1>();
+    }
+    return e;
 }
 cs_status sortInit32(cs_context* ctx);
 cs_status sortInit(cs_context* ctx)
 {
     const int bytes = (int)sizeof(SortSmem);
-    CS_CUDA(ctx, sortInitShift<0>());
-    CS_CUDA(ctx, sortInitShift<9>());
-    CS_CUDA(ctx, sortInitShift<18>());
-    CS_CUDA(ctx, sortInitShift<27>());
-    CS_CUDA(ctx, sortInitShift<36>());
-    CS_CUDA(ctx, sortInitShift<45>());
-    CS_CUDA(ctx, sortInitShift<54>());
+    CS_CUDA(ctx, sortInitPasses<0>());
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<54, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kFixupLow, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepRedoKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int perSM = 0;
     CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, onesweepRedoKernel, kSortBlock, bytes));
@@ -645,10 +657,22 @@ cs_status sortInit(cs_context* ctx)
     return sortInit32(ctx);
 }
 
-// Where the first radix pass reads the unsorted keys.  The passes alternate between the workspace's
-// arrays and the caller's; both plans (5 passes, and 7 more if redone; 7 plain passes) run an odd number
-// of passes over the data, so they start in the workspace and end in the caller's arrays.
-u64* sortSource(cs_context* ctx, u64*) { return ctx->keysAlt; }
+// the plain passes of the digits P .. END - 1
+template <int P, int END>
+static cs_status launchPasses(cs_context* ctx, PassPlan& pl, cudaStream_t s)
+{
+    if constexpr (P < END) {
+        CS_TRY((launchPass<P * kRadixBits, false>(ctx, pl, s)));
+        return launchPasses<P + 1, END>(ctx, pl, s);
+    } else {
+        return CS_OK;
+    }
+}
+
+// Where the first radix pass reads the unsorted keys.  The passes alternate between the workspace's arrays and the
+// caller's and must end in the caller's; both plans run the same parity of passes (kTopFirst is even), so with an
+// odd number of digits they start in the workspace, with an even number in the caller's arrays.
+u64* sortSource(cs_context* ctx, u64* keys) { return (kSortPasses & 1) ? ctx->keysAlt : keys; }
 
 // fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
 // (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
@@ -695,35 +719,28 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     pl.n = (u32)n;
     pl.tiles = divUp(n, kSortTile);
     pl.ticketSlot = 0;
-    if (plain) {                                            // all 7 digits, least significant first
+    if (plain) {                                            // all digits, least significant first
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
         CS_TRY((launchPass<0, true>(ctx, pl, s)));
-        CS_TRY((launchPass<9, false>(ctx, pl, s)));
-        CS_TRY((launchPass<18, false>(ctx, pl, s)));
-        CS_TRY((launchPass<27, false>(ctx, pl, s)));
-        CS_TRY((launchPass<36, false>(ctx, pl, s)));
-        CS_TRY((launchPass<45, false>(ctx, pl, s)));
-        return launchPass<54, false>(ctx, pl, s);
+        return launchPasses<1, kSortPasses>(ctx, pl, s);
     }
     u32* redo = ctx->sortTickets + kSortRedoSlot;
     {   // leading digits
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
-        CS_TRY((launchPass<18, true>(ctx, pl, s)));
-        CS_TRY((launchPass<27, false>(ctx, pl, s)));
-        CS_TRY((launchPass<36, false>(ctx, pl, s)));
-        CS_TRY((launchPass<45, false>(ctx, pl, s)));
+        CS_TRY((launchPass<kFixupLow, true>(ctx, pl, s)));
+        CS_TRY((launchPasses<kTopFirst + 1, kSortPasses - 1>(ctx, pl, s)));
     }
     StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     {   // top digit; this pass also orders the low bits inside the runs
         const u32 epoch = nextEpoch(ctx, s);
         const int in = pl.cur, out = in ^ 1;
-        onesweepLastKernel<54, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
-            pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + 6 * kRadix, ctx->sortTickets + pl.ticketSlot++,
+        onesweepLastKernel<kLastShift, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
+            pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (kSortPasses - 1) * kRadix, ctx->sortTickets + pl.ticketSlot++,
             ctx->sortLookback, epoch, epochBase(ctx), redo);
         CS_LAUNCH_CHECK(ctx, "onesweepLastKernel");
     }
-    // gated redo from the input of the fifth pass (pl.cur still names it): 7 passes end in the other pair,
-    // which is where the fifth pass wrote
+    // gated redo from the input of the last pass (pl.cur still names it); its result ends in the other pair,
+    // which is where the last pass wrote
     RedoArgs a;
     a.k[0] = pl.k[pl.cur]; a.k[1] = pl.k[pl.cur ^ 1];
     a.v[0] = pl.v[pl.cur]; a.v[1] = pl.v[pl.cur ^ 1];
@@ -749,7 +766,8 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
 // (u32 key, u32 index): 8 B per element, 16 B per element and pass.  30 bits = 4 digits of 9 bits (the last one 3
 // bits wide): 4 plain passes of the same kernel; with so few bits there is nothing left for a fix-up.  An even
 // number of passes: they start and end in the caller's arrays.
-constexpr int kSortPasses32 = 4;
+constexpr int kSortPasses32 = (30 + kRadixBits - 1) / kRadixBits;
+static_assert(kSortPasses32 % 2 == 0, "the 30-bit sort starts and ends in the caller's arrays");
 
 __global__ void __launch_bounds__(kHistBlock) sortHist32Kernel(const u32* __restrict__ keys, u64 n, u32* gHist)
 {
@@ -788,13 +806,33 @@ static cs_status launchPass32(cs_context* ctx, u32* const (&k)[2], u32* const (&
     return CS_OK;
 }
 
+template <int P>
+static cudaError_t sortInitPasses32()
+{
+    cudaError_t e = cudaFuncSetAttribute(onesweepKernel<P * kRadixBits, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SortSmemT<u32>));
+    if constexpr (P + 1 < kSortPasses32) {
+        if (e == cudaSuccess) e = sortInitPasses32<P + 1>();
+    }
+    return e;
+}
+
+template <int P>
+static cs_status launchPasses32(cs_context* ctx, u32* const (&k)[2], u32* const (&v)[2], u32 n, u32 tiles, cudaStream_t s)
+{
+    if constexpr (P < kSortPasses32) {
+        CS_TRY((launchPass32<P * kRadixBits, P == 0>(ctx, k, v, P & 1, n, tiles, P, s)));
+        return launchPasses32<P + 1>(ctx, k, v, n, tiles, s);
+    } else {
+        return CS_OK;
+    }
+}
+
 cs_status sortInit32(cs_context* ctx)
 {
     const int bytes = (int)sizeof(SortSmemT<u32>);
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<9, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<18, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<27, false, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, sortInitPasses32<1>());
     return CS_OK;
 }
 
@@ -817,10 +855,7 @@ cs_status enqueueSort32(cs_context* ctx, u32* keys, u32* perm, u64 n, cudaStream
     u32* const v[2] = {perm, ctx->permAlt};
     const u32 tiles = divUp(n, kSortTile);
     StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
-    CS_TRY((launchPass32<0, true>(ctx, k, v, 0, (u32)n, tiles, 0, s)));
-    CS_TRY((launchPass32<9, false>(ctx, k, v, 1, (u32)n, tiles, 1, s)));
-    CS_TRY((launchPass32<18, false>(ctx, k, v, 0, (u32)n, tiles, 2, s)));
-    return launchPass32<27, false>(ctx, k, v, 1, (u32)n, tiles, 3, s);
+    return launchPasses32<0>(ctx, k, v, (u32)n, tiles, s);
 }
 
 }  // namespace cs

@@ -131,7 +131,8 @@ def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
         assert np.array_equal(cs.u32(got["nodeCount"]), ref["nodeCount"])
     # the short cut (4 plain passes + the fused fifth), redone on the device; then the 7 plain passes for 16 builds;
     # then the short cut is tried again (and redone again): one pathological step does not cost every later one
-    assert plans == [4] + [7] * 16 + [4] + [7] * 2
+    short, plain = plans[0], plans[1]                        # 4 and 7 with the default 9-bit digits
+    assert plain > short + 1 and plans == [short] + [plain] * 16 + [short] + [plain] * 2
     ctx.setSortMode(cs.SORT_AUTO)
 
 
@@ -143,12 +144,12 @@ def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
                         (np.uint64(0x1234567) << np.uint64(30)) | rng.integers(0, 1 << LOW, 3000, dtype=np.uint64)])
     rng.shuffle(k)
     ctx.setSortMode(cs.SORT_AUTO)
-    assert ctx.sortPasses() == 4
+    short = ctx.sortPasses()                                    # 4 with the default 9-bit digits
     check(cs, ctx, k)                                           # check() synchronises when it copies the result back
-    assert ctx.sortPasses() == 7
+    assert ctx.sortPasses() > short + 1                         # 7: all digits
     check(cs, ctx, k, mode=None)
     ctx.setSortMode(cs.SORT_AUTO)
-    assert ctx.sortPasses() == 4
+    assert ctx.sortPasses() == short
 
 
 def test_workload_shapes(cs, ctx):
