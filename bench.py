@@ -293,7 +293,7 @@ def run_sharded(args):
                                       "replicated (PAPER.md:198-204); start array = rank 0's local tree, broadcast",
                        "partition_bounds": bounds if len(bounds) <= 17 else None,
                        "l2": "inputs larger than L2 (1.5 GiB of coordinates per step and GPU at N=2^26)"},
-            "roofline": {"bound": "hbm", "kernel": "onesweepKernel (one 9-bit radix pass over u64 key + u32 index)",
+            "roofline": {"bound": "hbm", "kernel": "onesweepKernel (one radix pass over u64 key + u32 index, 9-bit digits)",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": (tr or {}).get("onesweep_dram_bytes_per_launch"), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": pass_bytes, "avg_launch_ms": pass_ms, "launches_per_step": passes},
@@ -408,7 +408,7 @@ def run_ours(args):
     pass_bytes = sort_pass_bytes_per_particle(passes) * n
     achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
     tr = _traffic()
-    roofline = {"bound": "hbm", "kernel": "onesweepKernel (one 9-bit radix pass over u64 key + u32 index)",
+    roofline = {"bound": "hbm", "kernel": "onesweepKernel (one radix pass over u64 key + u32 index, 9-bit digits)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": (tr or {}).get("onesweep_dram_bytes_per_launch"), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "avg_launch_ms": pass_ms, "launches_per_step": passes,
@@ -640,7 +640,19 @@ def main():
     if args.impl == "reference":
         run_reference(args)
     elif args.mode == "sharded" or (args.mode == "auto" and world > 1):
-        run_sharded(args)
+        try:
+            run_sharded(args)
+        except Exception as e:                       # never leave the driver without a line: say so and run the replicas
+            import traceback
+            traceback.print_exc()
+            sys.stderr.write(f"bench.py: the sharded mode failed ({e!r}); running --mode replicas instead\n")
+            try:
+                import torch.distributed as dist
+                if dist.is_initialized():
+                    dist.destroy_process_group()
+            except Exception:
+                pass
+            run_ours(args)
     else:
         run_ours(args)
 
