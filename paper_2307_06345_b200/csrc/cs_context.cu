@@ -70,7 +70,7 @@ static Layout makeLayout(uint64_t maxParticles, uint32_t maxLeaves, int boxGrid)
     L.dirListKeys = take(dirTiles * kDirectCompact * sizeof(ulonglong2));   // 2 B per particle
     L.dirListMeta = take(dirTiles * kDirectCompact * sizeof(u32));          // 0.5 B per particle
     L.linkTileHist = take(linkTiles * kLinkBins * sizeof(u32));            // plain counts, never look-back words
-    L.hilbertTable = take(24 * 64 * sizeof(unsigned short) + 24 * 8);      // + the one-level inverse table
+    L.hilbertTable = take(24 * 512 * sizeof(unsigned short) + 24 * 8);      // + the one-level inverse table
     L.epochWords = take(64);
     L.ctrl = take(sizeof(DeviceCtrl));
     L.total = o;
@@ -261,12 +261,12 @@ cs_status cs_create(cs_context** out, int device, uint64_t maxParticles, uint32_
     ctx->epochWords = (u32*)(ctx->slab + L.epochWords);
     ctx->hilbertTable = (unsigned short*)(ctx->slab + L.hilbertTable);
     {
-        unsigned short table[24 * 64];
+        unsigned short table[24 * 512];
         hilbertBuildTable(table);
         e = cudaMemcpy(ctx->hilbertTable, table, sizeof(table), cudaMemcpyHostToDevice);
         unsigned char inv[24 * 8];
         hilbertBuildInverse(inv);
-        ctx->hilbertInverse = reinterpret_cast<unsigned char*>(ctx->hilbertTable + 24 * 64);
+        ctx->hilbertInverse = reinterpret_cast<unsigned char*>(ctx->hilbertTable + 24 * 512);
         if (e == cudaSuccess) e = cudaMemcpy(ctx->hilbertInverse, inv, sizeof(inv), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             cs_status stc = cudaFail(nullptr, e, "cs_create (Hilbert table)");

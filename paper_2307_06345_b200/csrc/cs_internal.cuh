@@ -143,7 +143,7 @@ struct cs_context {
     cs::u32 redoGrid = 0;              // CTAs of onesweepRedoKernel that are resident together (cooperative launch)
 
     // keys
-    unsigned short* hilbertTable = nullptr;   // [24][64] two-level transitions of the Hilbert curve (cs_particles.cu)
+    unsigned short* hilbertTable = nullptr;   // [24][512] three-level transitions of the Hilbert curve (cs_particles.cu)
     unsigned char* hilbertInverse = nullptr;  // [24][8] one-level inverse transitions (node geometry, cs_props.cu)
     int curve = CS_CURVE_MORTON;              // cs_setCurve: the curve cs_buildOctree computes keys on
 
@@ -253,7 +253,7 @@ cs_status enqueueBox(cs_context*, const double* x, const double* y, const double
 // histFrom: also accumulate the digit histograms of the radix sort, digits histFrom..6, into ctx->sortHist (-1: none)
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
                       u64* keys, int histFrom, int curve, cudaStream_t, u32* keys32 = nullptr /*30-bit keys instead*/);
-void hilbertBuildTable(unsigned short* table /*[24 * 64], host*/);
+void hilbertBuildTable(unsigned short* table /*[24 * 512], host*/);
 void hilbertBuildInverse(unsigned char* inv /*[24 * 8], host*/);
 cs_status sortInit(cs_context*);            // per-device kernel attributes, called by cs_create
 cs_status leavesDirectInit(cs_context*);

@@ -757,8 +757,8 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
                                              sizeof(SortSmem), s));
     CS_LAUNCH_CHECK(ctx, "onesweepRedoKernel");
     // a hint for callers that never read the control block (cs_sortKeys): the outcome reaches the host with the
-    // stream, and the next sort on this context looks at it
-    CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedoHint, redo, sizeof(u32), cudaMemcpyDeviceToHost, s));
+    // stream, and the next sort on this context looks at it (cs_buildOctree reads the flag with the control block)
+    if (!fused) CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedoHint, redo, sizeof(u32), cudaMemcpyDeviceToHost, s));
     return CS_OK;
 }
 
