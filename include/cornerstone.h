@@ -273,7 +273,9 @@ cs_status cs_setGraphLimit(cs_context* ctx, uint64_t maxParticles);
  *   (the context must have been created with capacities covering n and the tree), and
  *   copies the tree back into the caller's HOST arrays.  `host` has the layout of
  *   cs_octree_buffers but every pointer is host memory; NULL members are not copied back.
- *   Pinned (page-locked) host memory gives the full PCIe rate; pageable memory works.
+ *   Pinned (page-locked) host memory gives the full PCIe rate; pageable memory works.  Inputs above the graph limit
+ *   (cs_setGraphLimit) are uploaded in 8 pieces on a second stream and the bounding box is reduced piece by piece under
+ *   the upload; everything after the box needs all of it, so the rest of the build follows the upload.
  */
 cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n,
                              uint32_t bucketSize, const cs_octree_buffers* host, cs_octree_sizes* sizes,

@@ -37,7 +37,7 @@ cs_status enqueueBuild(cs_context* ctx, const double* x, const double* y, const 
                        bool plain, cudaStream_t s)
 {
     const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
-    CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
+    if (!ctx->boxReady) CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
     // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
     CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
@@ -340,19 +340,47 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
     auto up = [](size_t v) { return (v + 255) / 256 * 256; };
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = up(o + bytes); return at; };
-    const size_t oX = take(np * 8), oY = take(np * 8), oZ = take(np * 8), oBox = take(64), oKeys = take(np * 8),
+    const size_t oX = take(np * 8), oY = take(np * 8), oZ = take(np * 8), oBox = take(64 + 8 * 64), oKeys = take(np * 8),
                  oPerm = take(np * 4), oLeaves = take((nlc + 1) * 8), oCounts = take(nlc * 4), oPre = take(nnc * 8),
                  oLev = take(nnc * 4), oCO = take(nnc * 4), oPar = take(nnc * 4), oLR = take(256),
                  oL2N = take(nlc * 4), oN2L = take(nnc * 4), oNF = take(nnc * 4), oNC = take(nnc * 4);
     if (!ctx->hostPathSlab) {
         CS_CUDA(ctx, cudaMalloc((void**)&ctx->hostPathSlab, o));
         ctx->hostPathBytes = o;
+        CS_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copyStream, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : ctx->copyEvents) CS_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
     char* d = ctx->hostPathSlab;
     double* dx = (double*)(d + oX); double* dy = (double*)(d + oY); double* dz = (double*)(d + oZ);
-    CS_CUDA(ctx, cudaMemcpyAsync(dx, x, n * 8, cudaMemcpyHostToDevice, s));
-    CS_CUDA(ctx, cudaMemcpyAsync(dy, y, n * 8, cudaMemcpyHostToDevice, s));
-    CS_CUDA(ctx, cudaMemcpyAsync(dz, z, n * 8, cudaMemcpyHostToDevice, s));
+    double* chunkBoxes = (double*)(d + oBox) + 8;            // 8 doubles per chunk, behind box6
+    // Large inputs: the upload runs on a second stream in kChunks pieces, and the box of every piece is reduced on
+    // `stream` as soon as it has arrived (exact min / max: the fold of the pieces' boxes is the box of the set), so the
+    // box stage hides under the upload.  Everything after it needs the whole box.
+    constexpr int kChunks = 8;
+    const bool chunked = n > ctx->graphMaxParticles && n >= (1u << 20);
+    if (chunked) {
+        const uint64_t per = ((n + kChunks - 1) / kChunks + 511) / 512 * 512;
+        CS_CUDA(ctx, cudaEventRecord(ctx->copyEvents[kChunks], s));          // the staging buffers are free once `stream` got here
+        CS_CUDA(ctx, cudaStreamWaitEvent(ctx->copyStream, ctx->copyEvents[kChunks], 0));
+        int used = 0;
+        for (int c = 0; c < kChunks; ++c) {
+            const uint64_t a = (uint64_t)c * per;
+            if (a >= n) break;
+            const uint64_t cnt = n - a < per ? n - a : per;
+            CS_CUDA(ctx, cudaMemcpyAsync(dx + a, x + a, cnt * 8, cudaMemcpyHostToDevice, ctx->copyStream));
+            CS_CUDA(ctx, cudaMemcpyAsync(dy + a, y + a, cnt * 8, cudaMemcpyHostToDevice, ctx->copyStream));
+            CS_CUDA(ctx, cudaMemcpyAsync(dz + a, z + a, cnt * 8, cudaMemcpyHostToDevice, ctx->copyStream));
+            CS_CUDA(ctx, cudaEventRecord(ctx->copyEvents[c], ctx->copyStream));
+            CS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->copyEvents[c], 0));
+            CS_TRY(enqueueBox(ctx, dx + a, dy + a, dz + a, cnt, chunkBoxes + 8 * c, s));
+            ++used;
+        }
+        CS_TRY(enqueueBoxFold(ctx, chunkBoxes, used, (double*)(d + oBox), s));
+    } else {
+        CS_CUDA(ctx, cudaMemcpyAsync(dx, x, n * 8, cudaMemcpyHostToDevice, s));
+        CS_CUDA(ctx, cudaMemcpyAsync(dy, y, n * 8, cudaMemcpyHostToDevice, s));
+        CS_CUDA(ctx, cudaMemcpyAsync(dz, z, n * 8, cudaMemcpyHostToDevice, s));
+    }
     cs_octree_buffers b{};
     b.box6 = (double*)(d + oBox); b.keys = (uint64_t*)(d + oKeys); b.perm = (uint32_t*)(d + oPerm);
     b.leaves = (uint64_t*)(d + oLeaves); b.counts = (uint32_t*)(d + oCounts); b.prefixes = (uint64_t*)(d + oPre);
@@ -360,7 +388,9 @@ cs_status cs_buildOctreeHost(cs_context* ctx, const double* x, const double* y, 
     b.levelRange = (uint32_t*)(d + oLR); b.leafToNode = (uint32_t*)(d + oL2N); b.nodeToLeaf = (uint32_t*)(d + oN2L);
     b.nodeFirst = (uint32_t*)(d + oNF); b.nodeCount = (uint32_t*)(d + oNC);
     b.leafCapacity = ctx->maxLeaves; b.nodeCapacity = ctx->maxNodes;
+    ctx->boxReady = chunked;
     cs_status st = cs_buildOctree(ctx, dx, dy, dz, n, bucketSize, nullptr, 0, 0, &b, sizes, stream);
+    ctx->boxReady = false;
     if (st != CS_OK) return st;
     const size_t nl = sizes->numLeaves, nn = sizes->numNodes;
     if ((h->leaves || h->counts || h->leafToNode) && nl > h->leafCapacity)

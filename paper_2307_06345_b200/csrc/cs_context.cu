@@ -295,6 +295,9 @@ void cs_destroy(cs_context* ctx)
     if (ctx->hostCtrl) cudaFreeHost(ctx->hostCtrl);
     if (ctx->buildGraph) cudaGraphExecDestroy(ctx->buildGraph);
     if (ctx->captureStream) cudaStreamDestroy(ctx->captureStream);
+    if (ctx->copyStream) cudaStreamDestroy(ctx->copyStream);
+    for (cudaEvent_t e : ctx->copyEvents)
+        if (e) cudaEventDestroy(e);
     for (int i = 0; i < CS_NUM_STAGES; ++i) {
         if (ctx->evBegin[i]) cudaEventDestroy(ctx->evBegin[i]);
         if (ctx->evEnd[i]) cudaEventDestroy(ctx->evEnd[i]);

@@ -182,6 +182,9 @@ struct cs_context {
     // buffers for cs_buildOctreeHost (allocated lazily)
     char* hostPathSlab = nullptr;
     size_t hostPathBytes = 0;
+    cudaStream_t copyStream = nullptr;   // the upload runs here, chunk by chunk, while the box of earlier chunks is reduced
+    cudaEvent_t copyEvents[9] = {};
+    bool boxReady = false;               // cs_buildOctreeHost: buffers->box6 is already filled, the build skips the box stage
 
     // profiling
     bool profiling = false;
@@ -250,6 +253,7 @@ u32 reserveEpochs(cs_context* ctx, u32 count, cudaStream_t s);   // first of `co
 // ---- stage enqueue functions (no synchronisation; sizes device-resident) ---------------
 cs_status enqueueBox(cs_context*, const double* x, const double* y, const double* z, u64 n, double* box6,
                      cudaStream_t);
+cs_status enqueueBoxFold(cs_context*, const double* chunkBoxes, int chunks, double* box6, cudaStream_t);
 // histFrom: also accumulate the digit histograms of the radix sort, digits histFrom..6, into ctx->sortHist (-1: none)
 cs_status enqueueKeys(cs_context*, const double* x, const double* y, const double* z, u64 n, const double* box6,
                       u64* keys, int histFrom, int curve, cudaStream_t, u32* keys32 = nullptr /*30-bit keys instead*/);

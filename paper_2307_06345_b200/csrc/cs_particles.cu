@@ -158,6 +158,23 @@ cs_status enqueueBox(cs_context* ctx, const double* x, const double* y, const do
     return CS_OK;
 }
 
+// box of the whole set from the boxes of its chunks (cs_buildOctreeHost reduces chunk by chunk under the upload)
+__global__ void boxFoldKernel(const double* __restrict__ chunkBoxes, int chunks, double* __restrict__ box6)
+{
+    const int q = threadIdx.x;
+    if (q >= 6) return;
+    double v = chunkBoxes[q];
+    for (int c = 1; c < chunks; ++c) v = (q & 1) ? fmax(v, chunkBoxes[8 * c + q]) : fmin(v, chunkBoxes[8 * c + q]);
+    box6[q] = v;
+}
+
+cs_status enqueueBoxFold(cs_context* ctx, const double* chunkBoxes, int chunks, double* box6, cudaStream_t s)
+{
+    boxFoldKernel<<<1, 32, 0, s>>>(chunkBoxes, chunks, box6);
+    CS_LAUNCH_CHECK(ctx, "boxFoldKernel");
+    return CS_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // H2: Morton keys.  g = clamp(floor(((c - lo) / e) * 2^21), 0, 2^21 - 1) with explicitly
 // rounded intrinsics (__dsub_rn, __ddiv_rn, __dmul_rn are never contracted into FMAs), then

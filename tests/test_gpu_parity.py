@@ -302,6 +302,34 @@ def test_host_path_matches(cs, ctx):
     assert np.array_equal(hb.t["levelRange"].numpy().view(np.uint32), ref["levelRange"])
 
 
+def test_host_path_with_chunked_upload(cs):
+    """Above the graph limit cs_buildOctreeHost uploads in 8 pieces on a second stream and reduces the box piece by
+    piece under the upload: the tree must be the oracle's, call after call (the staging buffers are reused), for a size
+    whose last piece is ragged and for particles whose extremes lie in different pieces."""
+    n = (1 << 22) + 12345
+    x, y, z = W.plummer(n, 77)
+    x[n - 1] = x.max() + 3.0                                  # extremes in the last and in the first piece
+    y[0] = y.min() - 2.0
+    ref = oracle.full_build(x, y, z, 64)
+    ctx = cs.Context(max_particles=n, max_leaves=n // 4)
+    hb = cs.HostBuffers(n, ctx.max_leaves, want=("box6", "keys", "perm", "leaves", "counts", "prefixes", "childOffsets",
+                                                  "nodeFirst", "nodeCount"))
+    hx, hy, hz = (torch.from_numpy(a).pin_memory() for a in (x, y, z))
+    for it in range(3):
+        sz = cs.buildOctreeHost(ctx, hx, hy, hz, 64, hb)
+        nl, nn = sz["numLeaves"], sz["numNodes"]
+        assert nl == ref["leaves"].size - 1 and nn == ref["numNodes"]
+        assert np.array_equal(hb.t["box6"].numpy().view(np.uint64), ref["box"].view(np.uint64)), it
+        assert np.array_equal(hb.t["keys"].numpy().view(np.uint64), ref["sortedKeys"]), it
+        assert np.array_equal(hb.t["perm"].numpy().view(np.uint32), ref["perm"]), it
+        assert np.array_equal(hb.t["leaves"].numpy().view(np.uint64)[:nl + 1], ref["leaves"]), it
+        assert np.array_equal(hb.t["counts"].numpy().view(np.uint32)[:nl], ref["counts"]), it
+        assert np.array_equal(hb.t["prefixes"].numpy().view(np.uint64)[:nn], ref["prefixes"]), it
+        for k in ("childOffsets", "nodeFirst", "nodeCount"):
+            assert np.array_equal(hb.t[k].numpy().view(np.uint32)[:nn], ref[k]), k
+    ctx.close()
+
+
 def test_two_contexts_and_a_side_stream(cs):
     """Contexts share nothing: two of them used alternately, one on a non-default stream, give the oracle's trees."""
     xa, ya, za = W.blobs(150001, 41, nblobs=20)
