@@ -407,15 +407,20 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headM
     const u64* keys = sm.keys;
     const u32* low = reinterpret_cast<const u32*>(sm.keys);
     // ---- head bits: consecutive threads <-> consecutive slots, one ballot per 32 slots -----------------
+    bool someRun = false;                                    // a slot that is not a head: a run of two or more elements
 #pragma unroll
     for (int k = 0; k < kSortItems; ++k) {
         const u32 i = tid + k * kSortBlock;
         const bool head = i == 0 || i >= valid || ((keys[i - (i ? 1 : 0)] ^ keys[i]) >> LOW) != 0;
         const u32 H = __ballot_sync(kFull, head);
         if (lane == 0) headMask[i >> 5] = H;
+        someRun |= H != kFull;
     }
     if (tid < kHeadWords - kSortTile / 32) headMask[kSortTile / 32 + tid] = kFull;
-    __syncthreads();
+    if (!__syncthreads_or(someRun)) {                        // every element is alone in its run (most tiles of most inputs):
+        tileWriteOut<SHIFT, false>(sm, keysOut, valsOut, valid);   // the stable split has put it in place already
+        return;
+    }
     bool tooLong = false;
 #pragma unroll 1
     for (int k = 0; k < kSortItems; ++k) {
