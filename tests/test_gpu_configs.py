@@ -1,7 +1,7 @@
 """GPU parity on BASELINE.json's configurations, through cs_buildOctree with pre-allocated
 buffers (the launch configuration bench.py times).  Bit-exact against the oracle.
 
-c1, c2 run in test_gpu_parity.py.  c3 (2^24, buckets 16 and 64), c4 (2^26, the headline) and c5
+c1, c2 run in test_gpu_parity.py.  c3 (2^24, buckets 16 and 64), c4 (2^26, the headline; also on Hilbert keys) and c5
 (2^28) run here at full size, every output array compared with the oracle's.  c5's 10 incremental
 rebuilds run at 2^22 by default and, at 2^28, the full build + the first rebuild; all 10 rebuilds at
 2^28 when CS_TEST_FULL_C5=1 (≈ 30 GB of host memory, about a quarter of an hour of oracle time).
@@ -70,6 +70,13 @@ def test_config4_blobs_64m_headline(cs):
     assert got["converged"]
     # duplicates exist at this density: stability is really exercised
     assert int((ref["sortedKeys"][1:] == ref["sortedKeys"][:-1]).sum()) > 0
+    del ref
+    # the same particles on the Hilbert curve, every array again
+    refh = oracle.full_build(x, y, z, 64, curve="hilbert")
+    ctx.setCurve(cs.CURVE_HILBERT)
+    got = cs.buildOctree(ctx, dev(x), dev(y), dev(z), 64, buffers=bufs)
+    ctx.setCurve(cs.CURVE_MORTON)
+    check_against_oracle(cs, got, refh, "c4 on Hilbert keys")
     ctx.close()
 
 
