@@ -482,7 +482,21 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
     __shared__ u32 sCut[2];
     __shared__ u32 sHeadMask[kHeadWords];
     const u32 tid = threadIdx.x;
-    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
+    if (tid == 0) {
+        const u32 t = atomicAdd(ticket, 1u);
+        sm.tile = t;
+#if CS_SORT_PREFETCH
+        // as in the plain pass: the nominal range of the tile one generation of CTAs ahead (its cuts lie at most
+        // kFixupMaxRun elements before the nominal ones), on its way into L2
+        const u64 nom = ((u64)t + CS_SORT_PREFETCH) * kLastTile;
+        if (nom < n) {
+            const u64 pb = (nom - kFixupMaxRun) & ~3ull;            // 32-byte aligned for keys, 16-byte for values
+            const u32 cnt = (u32)((n - pb) < (u64)kSortTile ? (n - pb) : (u64)kSortTile);
+            bulkPrefetchL2(keysIn + pb, (cnt * 8u) & ~15u);
+            bulkPrefetchL2(valsIn + pb, (cnt * 4u) & ~15u);
+        }
+#endif
+    }
     u32* whWords = reinterpret_cast<u32*>(sm.warpHist);
     for (int i = tid; i < kHistWords; i += kSortBlock) whWords[i] = 0;
     __syncthreads();
