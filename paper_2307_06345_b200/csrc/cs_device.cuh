@@ -58,6 +58,13 @@ __device__ __forceinline__ void stStreamU2(u64* p, u64 a, u64 b)
     asm volatile("st.global.L1::no_allocate.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
 
+// Ask the copy engine to bring [p, p + bytes) into L2 (bytes: a multiple of 16, p 16-byte aligned): issued by one thread
+// for the tile that a CTA will pick up one generation of resident CTAs later, so that its first loads hit L2.
+__device__ __forceinline__ void bulkPrefetchL2(const void* p, u32 bytes)
+{
+    if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // ---- decoupled look-back words -----------------------------------------------------------
 // One 64-bit word per (tile, counter): [63:34] epoch, [33:32] status, [31:0] value.  Value and
 // flag travel in one 8-byte store, so no fence is needed between them.  The epoch makes

@@ -198,6 +198,9 @@ __device__ __forceinline__ u32 subtreeEnd(const u64* __restrict__ K, u32 j, u32 
     return lo;
 }
 
+#ifndef CS_LINK_PREFETCH
+#define CS_LINK_PREFETCH 592                    // 4 CTAs per SM x 148 SMs
+#endif
 #ifndef CS_LINK_MINBLOCKS
 #define CS_LINK_MINBLOCKS 4
 #endif
@@ -242,6 +245,14 @@ __global__ void __launch_bounds__(kLinkBlock, CS_LINK_MINBLOCKS)
     const u32 lt = laneMaskLt();
     for (u32 tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
         __syncthreads();
+#if CS_LINK_PREFETCH
+        if (tid == 0 && (u64)(tile + CS_LINK_PREFETCH) * kLinkTile < nl) {   // the tile one generation of CTAs ahead
+            const u64 pb = (u64)(tile + CS_LINK_PREFETCH) * kLinkTile;
+            const u32 cnt = (u32)((u64)nl - pb < (u64)kLinkTile ? (u64)nl - pb : (u64)kLinkTile);
+            bulkPrefetchL2(K + pb, (cnt * 8u) & ~15u);
+            if (out.leafOffsets) bulkPrefetchL2(out.leafOffsets + pb, (cnt * 4u) & ~15u);
+        }
+#endif
         for (int i = tid; i < kLinkWarps * kLinkBins; i += kLinkBlock) (&sWarp[0][0])[i] = 0;
         if (tid < kLinkBins) sBase[tid] = tilePrefix[(size_t)tile * kLinkBins + tid];
         __syncthreads();

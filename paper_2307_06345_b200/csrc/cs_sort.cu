@@ -108,10 +108,6 @@ __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 #ifndef CS_SORT_PREFETCH
 #define CS_SORT_PREFETCH 296
 #endif
-__device__ __forceinline__ void bulkPrefetchL2(const void* p, u32 bytes)   // bytes: multiple of 16, p 16-byte aligned
-{
-    if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
 constexpr int kHistWords = kSortWarps * kRadix / 2;
 
 template <typename KeyT>
