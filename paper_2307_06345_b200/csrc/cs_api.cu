@@ -34,14 +34,14 @@ cs_status checkParticles(cs_context* ctx, const char* fn, uint64_t n)
 // the stages of cs_buildOctree back to back on `s`, ending with the copy of the control block to the host
 cs_status enqueueBuild(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n, uint32_t bucketSize,
                        const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, const cs_octree_buffers* b,
-                       bool plain, cudaStream_t s)
+                       int plan, cudaStream_t s)
 {
     const u32 leafCap = b->leafCapacity < ctx->maxLeaves ? b->leafCapacity : ctx->maxLeaves;
     if (!ctx->boxReady) CS_TRY(enqueueBox(ctx, x, y, z, n, b->box6, s));
     CS_TRY(enqueueSortReset(ctx, s));
-    // the key kernel writes where the first radix pass reads, and accumulates the digit histograms
-    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys), plain ? 0 : kSortTopFirst, ctx->curve, s));
-    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plain, s));
+    // the key kernel writes where the first radix pass reads, and accumulates the histograms of the plan's digits
+    CS_TRY(enqueueKeys(ctx, x, y, z, n, b->box6, sortSource(ctx, (u64*)b->keys, plan), planFirstDigit(plan), ctx->curve, s));
+    CS_TRY(enqueueSort(ctx, (u64*)b->keys, b->perm, n, /*fused=*/true, plan, s));
     CS_TRY(enqueueLeaves(ctx, (const u64*)b->keys, n, bucketSize, (const u64*)prevLeaves, prevNumLeaves, maxRounds,
                          (u64*)b->leaves, b->counts, leafCap, kL, s));
     // link and node counts in one pass: the leaves' particle offsets are still in the workspace
@@ -58,7 +58,7 @@ cs_status enqueueBuild(cs_context* ctx, const double* x, const double* y, const 
 // the stages directly.
 cs_status captureBuild(cs_context* ctx, const double* x, const double* y, const double* z, uint64_t n, uint32_t bucketSize,
                        const uint64_t* prevLeaves, uint32_t prevNumLeaves, uint32_t maxRounds, const cs_octree_buffers* b,
-                       bool plain)
+                       int plan)
 {
     if (ctx->buildGraph) {
         cudaGraphExecDestroy(ctx->buildGraph);
@@ -75,7 +75,7 @@ cs_status captureBuild(cs_context* ctx, const double* x, const double* y, const 
     ctx->captureEpochs = 0;
     cudaError_t e = cudaMemcpyAsync(ctx->epochWords + 1, &ctx->hostCtrl->epochBase, sizeof(u32), cudaMemcpyHostToDevice, cs_);
     cs_status st = e == cudaSuccess
-                       ? enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain, cs_)
+                       ? enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plan, cs_)
                        : CS_ERR_CUDA;
     ctx->capturing = false;
     cudaGraph_t graph = nullptr;
@@ -146,7 +146,7 @@ cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t 
     if (!keys || !perm) return fail(ctx, CS_ERR_INVALID_ARG, "cs_sortKeys: null pointer");
     CS_TRY(checkParticles(ctx, "cs_sortKeys", n));
     DeviceGuard g(ctx->device);
-    return enqueueSort(ctx, (u64*)keys, perm, n, false, sortDecidePlain(ctx), (cudaStream_t)stream);
+    return enqueueSort(ctx, (u64*)keys, perm, n, false, sortDecidePlan(ctx), (cudaStream_t)stream);
 }
 
 cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n, uint32_t bucketSize,
@@ -179,18 +179,20 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
 cs_status cs_setSortMode(cs_context* ctx, int mode)
 {
     if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setSortMode: ctx is null");
-    if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN)
+    if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN && mode != CS_SORT_DEFAULT && mode != CS_SORT_SHORT)
         return fail(ctx, CS_ERR_INVALID_ARG, "cs_setSortMode: unknown mode %d", mode);
     ctx->sortMode = mode;
     ctx->autoPlainLeft = 0;
+    ctx->shortLeft = 0;
+    ctx->shortHold = kShortHold;
+    ctx->hostCtrl->sortRedoHint = 0;
     return CS_OK;
 }
 
 int cs_sortPasses(const cs_context* ctx)
 {
     if (!ctx) return 0;
-    return (ctx->sortMode == CS_SORT_PLAIN || ctx->autoPlainLeft > 0 || ctx->hostCtrl->sortRedoHint)
-               ? kSortPasses : kSortPasses - 1 - kSortTopFirst;
+    return sortPeekPlainPasses(ctx);
 }
 
 cs_status cs_setLeafMode(cs_context* ctx, int mode)
@@ -279,7 +281,7 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
         return fail(ctx, CS_ERR_CAPACITY, "cs_buildOctree: prevNumLeaves exceeds the leaf capacity");
     DeviceGuard g(ctx->device);
     cudaStream_t s = (cudaStream_t)stream;
-    const bool plain = sortDecidePlain(ctx);
+    const int plan = sortDecidePlan(ctx);
     bool replayed = false;
     if (!ctx->profiling && n <= ctx->graphMaxParticles) {
         // small inputs are bound by launch overhead: the whole call is one CUDA graph, captured when first seen with
@@ -287,13 +289,13 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
         BuildGraphKey key;
         memset(&key, 0, sizeof(key));
         key.x = x; key.y = y; key.z = z; key.n = n; key.bucket = bucketSize; key.prevNumLeaves = prevNumLeaves;
-        key.maxRounds = maxRounds; key.prevLeaves = prevLeaves; key.buffers = *b; key.plain = plain ? 1 : 0;
+        key.maxRounds = maxRounds; key.prevLeaves = prevLeaves; key.buffers = *b; key.plain = plan;
         key.curve = ctx->curve; key.leafMode = ctx->leafMode; key.stream = s;
         const bool known = ctx->buildGraph && memcmp(&key, &ctx->buildGraphKey, sizeof(key)) == 0;
         if (!known) {
             // capture on the second call in a row with the same arguments: a one-off call is cheaper enqueued directly
             if (ctx->buildGraphSeen && memcmp(&key, &ctx->buildGraphCandidate, sizeof(key)) == 0) {
-                CS_TRY(captureBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain));
+                CS_TRY(captureBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plan));
                 if (ctx->buildGraph) memcpy(&ctx->buildGraphKey, &key, sizeof(key));
             } else {
                 memcpy(&ctx->buildGraphCandidate, &key, sizeof(key));
@@ -310,13 +312,11 @@ cs_status cs_buildOctree(cs_context* ctx, const double* x, const double* y, cons
         }
     }
     if (!replayed) {
-        CS_TRY(enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plain, s));
+        CS_TRY(enqueueBuild(ctx, x, y, z, n, bucketSize, prevLeaves, prevNumLeaves, maxRounds, b, plan, s));
         CS_CUDA(ctx, cudaStreamSynchronize(s));
     }
-    if (ctx->hostCtrl->sortRedo) {                        // deep clustering: skip the short cut for a while
-        ctx->autoPlainLeft = kPlainHold;
-        ctx->hostCtrl->sortRedoHint = 0;
-    }
+    sortPlanOutcome(ctx, plan, plan != kPlanPlain && ctx->hostCtrl->sortRedo != 0);   // deep clustering: the next plan for a while
+    ctx->hostCtrl->sortRedoHint = 0;
     const DeviceCtrl& c = ctx->hostCtrl->c;
     sizes->rounds = c.rounds;
     sizes->converged = c.converged;

@@ -26,8 +26,19 @@ constexpr int kRoundSlots = kMaxRounds + 2;
 constexpr int kRadixBits = CS_RADIX_BITS;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits: 7 passes of 9 bits
-constexpr int kSortTopFirst = 2;      // the default sort plan orders by the digits 2..6 (bits 18..62) and fixes up the rest (cs_sort.cu)
-constexpr int kPlainHold = 16;        // sorts that run the plain plan after one needed the redo, before the short cut is tried again
+// Sort plans (cs_sort.cu): the plain plan sorts by all digits; the default plan by the digits kSortTopFirst .. (bits
+// 18..62) and orders the bits below inside runs of equal leading digits in its last pass; the short plan does the same
+// from digit kSortShortFirst (bits 27..62: one pass less), which works as long as no cell of octree level 12 holds more
+// than 257 particles.  A plan whose last pass finds a run too long is redone on the device and the context moves to the
+// next plan for a while.
+enum { kPlanShort = 0, kPlanDefault = 1, kPlanPlain = 2 };
+constexpr int kSortTopFirst = 2;
+constexpr int kSortShortFirst = 3;
+constexpr int kPlainHold = 16;        // sorts on the plain plan after the default plan needed the redo, before it is tried again
+constexpr int kShortHold = 256;       // sorts on the default plan after the short plan needed the redo (doubles with every failure)
+constexpr int kShortHoldMax = 1 << 14;
+inline int planFirstDigit(int plan) { return plan == kPlanShort ? kSortShortFirst : plan == kPlanDefault ? kSortTopFirst : 0; }
+inline int planPasses(int plan) { return kSortPasses - planFirstDigit(plan); }
 #ifndef CS_SORT_BLOCK
 #define CS_SORT_BLOCK 512
 #endif
@@ -97,7 +108,7 @@ struct HostCtrl {                // pinned mirror read back once per call
 
 // A whole cs_buildOctree call captured as a CUDA graph (small inputs are bound by launch overhead, not by the device):
 // valid while every argument and mode it was captured with stays the same.
-struct BuildGraphKey {
+struct BuildGraphKey {   // `plain` holds the sort plan
     const void* x; const void* y; const void* z;
     u64 n;
     u32 bucket, prevNumLeaves, maxRounds;
@@ -139,7 +150,10 @@ struct cs_context {
     uint64_t buildGraphLaunches = 0;   // kernels one replay launches
     uint64_t graphMaxParticles = 1ull << 22;   // builds of at most this many particles are captured and replayed
     int sortMode = CS_SORT_AUTO;       // cs_setSortMode
-    int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after one needed the redo
+    int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after the default plan needed the redo
+    int shortLeft = 0;                 // CS_SORT_AUTO: sorts left before the short plan is tried again
+    int shortHold = cs::kShortHold;    // the next value of shortLeft (back-off)
+    int lastPlan = cs::kPlanDefault;   // plan of the last sort enqueued (whose redo flag may still arrive)
     cs::u32 redoGrid = 0;              // CTAs of onesweepRedoKernel that are resident together (cooperative launch)
 
     // keys
@@ -263,10 +277,12 @@ cs_status sortInit(cs_context*);            // per-device kernel attributes, cal
 cs_status leavesDirectInit(cs_context*);
 cs_status leavesInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
-u64* sortSource(cs_context*, u64* keys);   // where the first radix pass reads the unsorted keys
+u64* sortSource(cs_context*, u64* keys, int plan);   // where the first radix pass reads the unsorted keys
 cs_status enqueueSort32(cs_context*, u32* keys, u32* perm, u64 n, cudaStream_t);   // 30-bit keys: 4 plain passes
-bool sortDecidePlain(cs_context*);            // plan of the next sort: 7 plain passes, or the short cut
-cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, bool plain, cudaStream_t);
+int sortDecidePlan(cs_context*);              // plan of the next sort (kPlanShort / kPlanDefault / kPlanPlain)
+void sortPlanOutcome(cs_context*, int plan, bool redone);   // what the host learnt about a finished sort
+int sortPeekPlainPasses(const cs_context*);   // plain passes of the next sort (cs_sortPasses)
+cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, int plan, cudaStream_t);
 // maxLevel: depth below which no leaf is split: kL, or 10 for 30-bit keys held in the top 10 digits (cs_api32.cu)
 cs_status enqueueLeaves(cs_context*, const u64* sortedKeys, u64 n, u32 bucketSize, const u64* prevLeaves,
                         u32 prevNumLeaves, u32 maxRounds, u64* leaves, u32* counts, u32 leafCapacity, u32 maxLevel,

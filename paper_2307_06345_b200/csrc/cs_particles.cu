@@ -322,7 +322,7 @@ __device__ __forceinline__ u64 hilbertFromMorton(u64 m, const unsigned short* __
     return h;
 }
 
-// HIST: first digit that is counted (the default sort plan needs the digits kSortTopFirst..6 only), or -1 for none
+// HIST: first digit that is counted (the sort plan's first digit: the others are not sorted by), or -1 for none
 template <int HIST>
 __device__ __forceinline__ void histAdd(u32* sh, u64 key)
 {
@@ -436,6 +436,7 @@ cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const d
     do {                                                          \
         if (histFrom < 0) CS_KEYS_LAUNCH(V, -1, C);               \
         else if (histFrom == 0) CS_KEYS_LAUNCH(V, 0, C);          \
+        else if (histFrom == kSortShortFirst) CS_KEYS_LAUNCH(V, kSortShortFirst, C); \
         else CS_KEYS_LAUNCH(V, kSortTopFirst, C);                 \
     } while (0)
     if (curve == CS_CURVE_HILBERT) {

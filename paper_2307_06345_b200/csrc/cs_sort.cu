@@ -29,7 +29,6 @@ namespace cg = cooperative_groups;
 namespace cs {
 
 constexpr int kHistBlock = 512;
-constexpr int kTopFirst = kSortTopFirst;                    // first digit the default path sorts by (bits 18..)
 constexpr int kSortWarps = kSortBlock / 32;
 static_assert(kSortBlock >= kRadix, "one thread per digit in the per-digit phases of a radix pass");
 static_assert(kSortItems * 32 < 65536 && kSortTile < 65536, "16-bit per-warp digit counters and tile-local slots");
@@ -524,7 +523,8 @@ struct RedoArgs {
     u64* k[2];
     u32* v[2];
     u32 n;
-    u32* hist;                  // [kSortPasses][kRadix]: scanned for the digits >= kTopFirst, zero below
+    u32* hist;                  // [kSortPasses][kRadix]: scanned for the digits >= first, zero below
+    u32 first;                  // first digit the key kernel / the histogram kernel counted (the plan's)
     u32* tickets;               // kSortPasses ticket counters
     u64* lookback;
     u32 epoch0;                 // pass p uses look-back epoch epoch0 + *epochBase + p
@@ -577,18 +577,20 @@ __global__ void __launch_bounds__(kSortBlock, 1) onesweepRedoKernel(const RedoAr
     const u32 tid = threadIdx.x;
     {   // digit counts of the passes the key kernel did not count (zero so far), then their exclusive scans
         u32* sh = reinterpret_cast<u32*>(smemRaw);
-        for (int i = tid; i < kTopFirst * kRadix; i += kSortBlock) sh[i] = 0;
+        const int first = (int)a.first;                       // at most kSortShortFirst digits: 6 KB of counters
+        for (int i = tid; i < first * kRadix; i += kSortBlock) sh[i] = 0;
         __syncthreads();
         for (u64 i = (u64)blockIdx.x * kSortBlock + tid; i < a.n; i += (u64)gridDim.x * kSortBlock) {
             const u64 k = a.k[0][i];
 #pragma unroll
-            for (int p = 0; p < kTopFirst; ++p) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
+            for (int p = 0; p < kSortShortFirst; ++p)
+                if (p < first) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
         }
         __syncthreads();
-        for (int i = tid; i < kTopFirst * kRadix; i += kSortBlock)
+        for (int i = tid; i < first * kRadix; i += kSortBlock)
             if (sh[i]) atomicAdd(&a.hist[i], sh[i]);
         grid.sync();
-        for (u32 p = blockIdx.x; p < (u32)kTopFirst; p += gridDim.x) {   // block-uniform trip count
+        for (u32 p = blockIdx.x; p < a.first; p += gridDim.x) {   // block-uniform trip count
             u32 total;
             u32* warpSums = reinterpret_cast<u32*>(smemRaw);
             const u32 idx = p * kRadix + tid;
@@ -616,12 +618,12 @@ cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
     return CS_OK;
 }
 
-// The default plan sorts by the digits kTopFirst .. kSortPasses - 1 (the last of them, the key's top digit, in the
-// fused pass that also orders the bits below kFixupLow); the plain plan sorts by all kSortPasses digits.
-constexpr int kFixupLow = kTopFirst * kRadixBits;
+// A plan with first digit F sorts by the digits F .. kSortPasses - 1, the last of them (the key's top digit) in the
+// fused pass that also orders the bits below F * kRadixBits inside runs of equal leading digits; F = kSortShortFirst
+// (short plan), kSortTopFirst (default plan).  The plain plan sorts by all kSortPasses digits.
 constexpr int kLastShift = (kSortPasses - 1) * kRadixBits;
-static_assert(kFixupLow <= 32 && kTopFirst % 2 == 0 && kTopFirst + 1 < kSortPasses,
-              "the fix-up compares the keys' low words; both plans run the same parity of passes");
+static_assert(kSortShortFirst * kRadixBits <= 32 && kSortShortFirst + 1 < kSortPasses && kSortShortFirst == kSortTopFirst + 1,
+              "the fix-up compares the keys' low words");
 
 struct PassPlan {
     u64* k[2];
@@ -662,8 +664,10 @@ cs_status sortInit(cs_context* ctx)
     const int bytes = (int)sizeof(SortSmem);
     CS_CUDA(ctx, sortInitPasses<0>());
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kFixupLow, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kFixupLow>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kSortTopFirst * kRadixBits, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kSortShortFirst * kRadixBits, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kSortTopFirst * kRadixBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kSortShortFirst * kRadixBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepRedoKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int perSM = 0;
     CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, onesweepRedoKernel, kSortBlock, bytes));
@@ -685,73 +689,78 @@ static cs_status launchPasses(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 }
 
 // Where the first radix pass reads the unsorted keys.  The passes alternate between the workspace's arrays and the
-// caller's and must end in the caller's; both plans run the same parity of passes (kTopFirst is even), so with an
-// odd number of digits they start in the workspace, with an even number in the caller's arrays.
-u64* sortSource(cs_context* ctx, u64* keys) { return (kSortPasses & 1) ? ctx->keysAlt : keys; }
+// caller's and must end in the caller's: a plan with an odd number of passes starts in the workspace, one with an even
+// number in the caller's arrays.
+u64* sortSource(cs_context* ctx, u64* keys, int plan) { return (planPasses(plan) & 1) ? ctx->keysAlt : keys; }
 
-// fused: the unsorted keys already lie in sortSource(ctx, keys) and ctx->sortHist holds their digit counts
-// (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
-// Which plan the next sort on this context runs: the 7 plain passes if the caller asked for them (cs_setSortMode)
-// or if a recent sort had to be redone (runs too long for the short cut); in the latter case the short cut is
-// tried again after kPlainHold sorts.
-bool sortDecidePlain(cs_context* ctx)
+// Which plan the next sort on this context runs (cs_setSortMode; include/cornerstone.h).  CS_SORT_AUTO climbs a
+// ladder: the short plan; after it had to be redone, the default plan for shortHold sorts (doubling with every failure,
+// so that inputs that never fit the short plan pay for ever fewer attempts); after the default plan had to be redone,
+// the plain plan for kPlainHold sorts.
+static int peekPlan(const cs_context* ctx)
 {
-    if (ctx->hostCtrl->sortRedoHint) {                      // written by the stream behind an earlier sort
-        ctx->hostCtrl->sortRedoHint = 0;
-        ctx->autoPlainLeft = kPlainHold;
+    switch (ctx->sortMode) {
+        case CS_SORT_PLAIN: return kPlanPlain;
+        case CS_SORT_SHORT: return kPlanShort;
+        case CS_SORT_DEFAULT: return ctx->autoPlainLeft > 0 ? kPlanPlain : kPlanDefault;
+        default: return ctx->autoPlainLeft > 0 ? kPlanPlain : ctx->shortLeft > 0 ? kPlanDefault : kPlanShort;
     }
-    if (ctx->sortMode == CS_SORT_PLAIN) return true;
-    if (ctx->autoPlainLeft == 0) return false;
-    --ctx->autoPlainLeft;
-    return true;
 }
 
-cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, bool plain, cudaStream_t s)
+void sortPlanOutcome(cs_context* ctx, int plan, bool redone)
 {
-    StageTimer t(ctx, CS_STAGE_SORT, s);
-    if (n == 0) return CS_OK;
-    u64* first = sortSource(ctx, keys);
-    {
-        StageTimer th(ctx, CS_STAGE_SORT_HIST, s);
-        if (!fused) {
-            CS_TRY(enqueueSortReset(ctx, s));
-            u32 grid = (u32)ctx->numSMs * 4;
-            u32 need = divUp((n + 1) / 2, kHistBlock);
-            if (need < grid) grid = need ? need : 1;
-            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first,
-                                                       plain ? 0 : kTopFirst);
-            CS_LAUNCH_CHECK(ctx, "sortHistKernel");
-        }
-        sortScanHistKernel<<<kSortPasses, kRadix, 0, s>>>(ctx->sortHist);
-        CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
+    if (!redone) {
+        if (plan == kPlanShort) ctx->shortHold = kShortHold;           // it fits: forget the back-off
+        return;
     }
-    ctx->evUsed[CS_STAGE_SORT_FIXUP] = false;
-    PassPlan pl;
-    const bool own = first == keys;
-    pl.k[0] = first; pl.k[1] = own ? ctx->keysAlt : keys;
-    pl.v[0] = own ? perm : ctx->permAlt; pl.v[1] = own ? ctx->permAlt : perm;
-    pl.cur = 0;
-    pl.n = (u32)n;
-    pl.tiles = divUp(n, kSortTile);
-    pl.ticketSlot = 0;
-    if (plain) {                                            // all digits, least significant first
-        StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
-        CS_TRY((launchPass<0, true>(ctx, pl, s)));
-        return launchPasses<1, kSortPasses>(ctx, pl, s);
+    if (ctx->sortMode == CS_SORT_PLAIN || ctx->sortMode == CS_SORT_SHORT) return;   // forced plans do not adapt
+    if (plan == kPlanShort) {
+        ctx->shortLeft = ctx->shortHold;
+        ctx->shortHold = ctx->shortHold * 2 < kShortHoldMax ? ctx->shortHold * 2 : kShortHoldMax;
+    } else if (plan == kPlanDefault) {
+        ctx->autoPlainLeft = kPlainHold;
+        if (ctx->shortLeft < ctx->shortHold) ctx->shortLeft = ctx->shortHold;   // what the default plan cannot do, the short one cannot
     }
+}
+
+int sortDecidePlan(cs_context* ctx)
+{
+    if (ctx->hostCtrl->sortRedoHint) {                      // written by the stream behind an earlier cs_sortKeys
+        ctx->hostCtrl->sortRedoHint = 0;
+        sortPlanOutcome(ctx, ctx->lastPlan, true);
+    }
+    const int plan = peekPlan(ctx);
+    if (plan == kPlanPlain && ctx->autoPlainLeft > 0) --ctx->autoPlainLeft;
+    else if (plan == kPlanDefault && ctx->sortMode == CS_SORT_AUTO && ctx->shortLeft > 0) --ctx->shortLeft;
+    ctx->lastPlan = plan;
+    return plan;
+}
+
+int sortPeekPlainPasses(const cs_context* ctx)
+{
+    const bool forced = ctx->sortMode == CS_SORT_PLAIN || ctx->sortMode == CS_SORT_SHORT;
+    const int plan = (ctx->hostCtrl->sortRedoHint && !forced) ? (ctx->lastPlan == kPlanShort ? kPlanDefault : kPlanPlain) : peekPlan(ctx);
+    return plan == kPlanPlain ? kSortPasses : planPasses(plan) - 1;
+}
+
+// the leading digits F + 1 .. and the fused last pass of a plan with first digit F, then the gated redo
+template <int F>
+static cs_status enqueueShortCut(cs_context* ctx, PassPlan& pl, bool fused, cudaStream_t s)
+{
+    constexpr int kLow = F * kRadixBits;
     u32* redo = ctx->sortTickets + kSortRedoSlot;
     {   // leading digits
         StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
-        CS_TRY((launchPass<kFixupLow, true>(ctx, pl, s)));
-        CS_TRY((launchPasses<kTopFirst + 1, kSortPasses - 1>(ctx, pl, s)));
+        CS_TRY((launchPass<kLow, true>(ctx, pl, s)));
+        CS_TRY((launchPasses<F + 1, kSortPasses - 1>(ctx, pl, s)));
     }
     StageTimer tf(ctx, CS_STAGE_SORT_FIXUP, s);
     {   // top digit; this pass also orders the low bits inside the runs
         const u32 epoch = nextEpoch(ctx, s);
         const int in = pl.cur, out = in ^ 1;
-        onesweepLastKernel<kLastShift, kFixupLow><<<divUp(n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
-            pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (kSortPasses - 1) * kRadix, ctx->sortTickets + pl.ticketSlot++,
-            ctx->sortLookback, epoch, epochBase(ctx), redo);
+        onesweepLastKernel<kLastShift, kLow><<<divUp(pl.n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
+            pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (kSortPasses - 1) * kRadix,
+            ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, epochBase(ctx), redo);
         CS_LAUNCH_CHECK(ctx, "onesweepLastKernel");
     }
     // gated redo from the input of the last pass (pl.cur still names it); its result ends in the other pair,
@@ -761,6 +770,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     a.v[0] = pl.v[pl.cur]; a.v[1] = pl.v[pl.cur ^ 1];
     a.n = pl.n;
     a.hist = ctx->sortHist;
+    a.first = (u32)F;
     a.tickets = ctx->sortTickets + pl.ticketSlot;
     a.lookback = ctx->sortLookback;
     a.epoch0 = reserveEpochs(ctx, kSortPasses, s);
@@ -775,6 +785,45 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
     // stream, and the next sort on this context looks at it (cs_buildOctree reads the flag with the control block)
     if (!fused) CS_CUDA(ctx, cudaMemcpyAsync(&ctx->hostCtrl->sortRedoHint, redo, sizeof(u32), cudaMemcpyDeviceToHost, s));
     return CS_OK;
+}
+
+// fused: the unsorted keys already lie in sortSource(ctx, keys, plan) and ctx->sortHist holds the counts of the plan's
+// digits (cs_buildOctree: the key kernel wrote both); otherwise they are in `keys`.
+cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, int plan, cudaStream_t s)
+{
+    StageTimer t(ctx, CS_STAGE_SORT, s);
+    if (n == 0) return CS_OK;
+    u64* first = sortSource(ctx, keys, plan);
+    {
+        StageTimer th(ctx, CS_STAGE_SORT_HIST, s);
+        if (!fused) {
+            CS_TRY(enqueueSortReset(ctx, s));
+            u32 grid = (u32)ctx->numSMs * 4;
+            u32 need = divUp((n + 1) / 2, kHistBlock);
+            if (need < grid) grid = need ? need : 1;
+            sortHistKernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist, first == keys ? nullptr : first,
+                                                       planFirstDigit(plan));
+            CS_LAUNCH_CHECK(ctx, "sortHistKernel");
+        }
+        sortScanHistKernel<<<kSortPasses, kRadix, 0, s>>>(ctx->sortHist);
+        CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
+    }
+    ctx->evUsed[CS_STAGE_SORT_FIXUP] = false;
+    PassPlan pl;
+    const bool own = first == keys;
+    pl.k[0] = first; pl.k[1] = own ? ctx->keysAlt : keys;
+    pl.v[0] = own ? perm : ctx->permAlt; pl.v[1] = own ? ctx->permAlt : perm;
+    pl.cur = 0;
+    pl.n = (u32)n;
+    pl.tiles = divUp(n, kSortTile);
+    pl.ticketSlot = 0;
+    if (plan == kPlanPlain) {                               // all digits, least significant first
+        StageTimer tp(ctx, CS_STAGE_SORT_PASSES, s);
+        CS_TRY((launchPass<0, true>(ctx, pl, s)));
+        return launchPasses<1, kSortPasses>(ctx, pl, s);
+    }
+    return plan == kPlanShort ? enqueueShortCut<kSortShortFirst>(ctx, pl, fused, s)
+                              : enqueueShortCut<kSortTopFirst>(ctx, pl, fused, s);
 }
 
 // ---- 30-bit keys (L = 10) -----------------------------------------------------------------------

@@ -33,6 +33,7 @@ def check(cs, got, ref, what):
 def test_replays_follow_the_data_in_the_buffers(cs, n, bucket):
     ctx = cs.Context(max_particles=n, max_leaves=8 * n + 64)
     bufs = cs.TreeBuffers(ctx, n)
+    ctx.setSortMode(cs.SORT_DEFAULT)                             # one plan for all calls (the blobs are too dense for the short one)
     sets = [W.blobs(n, W.BASE_SEED + 200 + k, nblobs=16) for k in range(3)]
     dx, dy, dz = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
     launches = []

@@ -1,9 +1,10 @@
 """GPU parity of cs_sortKeys on every path of cs_sort.cu against the oracle's stable sort (O3).
 
-Default path: 5 radix passes over the leading 45 bits + fix-up of the low 18 bits inside runs of
-equal leading bits; a run longer than 257 elements raises the device flag and the 7 gated plain
-passes redo the sort.  cs_setSortMode(PLAIN) runs the 7 plain passes directly.  All of them must
-return the same (unique) keys and permutation, bit for bit.
+Default plan: 5 radix passes over the leading 45 bits, the last of which also orders the low 18 bits inside runs of
+equal leading bits; short plan: 4 passes over the leading 36 bits, the low 27 ordered inside runs.  A run longer than
+257 elements raises the device flag and the 7 gated plain passes redo the sort.  cs_setSortMode(PLAIN) runs the 7
+plain passes directly; AUTO moves between the three.  All of them must return the same (unique) keys and permutation,
+bit for bit.
 """
 import numpy as np
 import pytest
@@ -14,7 +15,6 @@ from paper_2307_06345_b200 import workloads as W
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
-LOW = 18            # bits ordered by the fix-up
 MAX_RUN = 257       # longest run the fix-up takes (kFixupMaxRun + 1)
 
 
@@ -33,9 +33,16 @@ def ctx(cs):
     c.close()
 
 
+@pytest.fixture(params=["default", "short"])
+def plan(request, cs):
+    """(sort mode, LOW): the plan whose last pass orders the low LOW bits inside runs of equal leading bits: the default
+    plan (5 passes over bits 18..62) and the short plan (4 passes over bits 27..62)."""
+    return (cs.SORT_DEFAULT, 18) if request.param == "default" else (cs.SORT_SHORT, 27)
+
+
 def check(cs, ctx, k, mode=0):
-    """mode: SORT_AUTO (0) / SORT_PLAIN (1) is set first (which also forgets an earlier redo); None leaves the context as
-    it is."""
+    """mode (SORT_AUTO, SORT_PLAIN, SORT_DEFAULT, SORT_SHORT) is set first (which also forgets an earlier redo); None
+    leaves the context as it is."""
     if mode is not None:
         ctx.setSortMode(mode)
     P, perm = oracle.sort(k)
@@ -45,9 +52,9 @@ def check(cs, ctx, k, mode=0):
     assert np.array_equal(cs.u32(dperm), perm), "perm"
 
 
-def keys_with_runs(rng, run_lengths, low_mode="random"):
-    """Keys whose leading 45 bits form runs of the given lengths, shuffled."""
-    tops = rng.choice(1 << 40, size=len(run_lengths), replace=False).astype(np.uint64)
+def keys_with_runs(rng, run_lengths, LOW, low_mode="random"):
+    """Keys whose bits above LOW form runs of the given lengths, shuffled."""
+    tops = rng.choice(1 << 34, size=len(run_lengths), replace=False).astype(np.uint64)
     parts = []
     for t, r in zip(tops, run_lengths):
         if low_mode == "random":
@@ -63,49 +70,53 @@ def keys_with_runs(rng, run_lengths, low_mode="random"):
 
 
 @pytest.mark.parametrize("low_mode", ["random", "few", "equal"])
-def test_fixup_orders_short_runs(cs, ctx, low_mode):
+def test_fixup_orders_short_runs(cs, ctx, plan, low_mode):
+    mode, LOW = plan
     rng = np.random.default_rng(11)
     runs = list(rng.integers(1, 40, 3000)) + [MAX_RUN - 1, MAX_RUN, 200, 256]
-    check(cs, ctx, keys_with_runs(rng, runs, low_mode))
+    check(cs, ctx, keys_with_runs(rng, runs, LOW, low_mode), mode)
 
 
 @pytest.mark.parametrize("longest", [MAX_RUN, MAX_RUN + 1, MAX_RUN + 2, 300, 513, 5000])
-def test_run_length_boundary_and_gated_redo(cs, ctx, longest):
+def test_run_length_boundary_and_gated_redo(cs, ctx, plan, longest):
     """Runs of exactly the limit stay on the fix-up; one element more takes the gated 7 passes."""
+    mode, LOW = plan
     rng = np.random.default_rng(longest)
     runs = [1] * 20000 + [longest] + list(rng.integers(1, 9, 2000))
-    check(cs, ctx, keys_with_runs(rng, runs))
+    check(cs, ctx, keys_with_runs(rng, runs, LOW), mode)
     # the context is reusable afterwards (flag and tickets are reset per call)
-    check(cs, ctx, keys_with_runs(rng, [1] * 9000 + [17, 3]))
+    check(cs, ctx, keys_with_runs(rng, [1] * 9000 + [17, 3], LOW), mode)
 
 
-def test_runs_at_the_ends_and_across_blocks(cs, ctx):
+def test_runs_at_the_ends_and_across_blocks(cs, ctx, plan):
+    mode, LOW = plan
     rng = np.random.default_rng(3)
     n_runs = 600
-    tops = np.sort(rng.choice(1 << 40, size=n_runs, replace=False).astype(np.uint64))
+    tops = np.sort(rng.choice(1 << 34, size=n_runs, replace=False).astype(np.uint64))
     lens = rng.integers(100, MAX_RUN + 1, n_runs)            # long runs straddle every 256-thread block
     lens[0] = MAX_RUN
     lens[-1] = MAX_RUN
     k = np.concatenate([(t << np.uint64(LOW)) | rng.integers(0, 1 << LOW, r, dtype=np.uint64)
                         for t, r in zip(tops, lens)])
     rng.shuffle(k)
-    check(cs, ctx, k)
+    check(cs, ctx, k, mode)
 
 
-def test_one_giant_run_and_all_equal_keys(cs, ctx):
+def test_one_giant_run_and_all_equal_keys(cs, ctx, plan):
+    mode, LOW = plan
     rng = np.random.default_rng(4)
     k = (np.uint64(12345) << np.uint64(LOW)) | rng.integers(0, 1 << LOW, 50000, dtype=np.uint64)
-    check(cs, ctx, k)
-    check(cs, ctx, np.full(30001, 0x7FFFFFFFFFFFFFFF, dtype=np.uint64))
-    check(cs, ctx, np.zeros(777, dtype=np.uint64))
+    check(cs, ctx, k, mode)
+    check(cs, ctx, np.full(30001, 0x7FFFFFFFFFFFFFFF, dtype=np.uint64), mode)
+    check(cs, ctx, np.zeros(777, dtype=np.uint64), mode)
 
 
 def test_plain_mode_equals_default(cs, ctx):
     rng = np.random.default_rng(8)
     for n in (1, 257, 6656, 6657, 123457):
         k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
-        check(cs, ctx, k, cs.SORT_PLAIN)
-        check(cs, ctx, k, cs.SORT_AUTO)
+        for mode in (cs.SORT_PLAIN, cs.SORT_AUTO, cs.SORT_DEFAULT, cs.SORT_SHORT):
+            check(cs, ctx, k, mode)
     with pytest.raises(cs.CornerstoneError):
         ctx.setSortMode(7)
 
@@ -129,11 +140,45 @@ def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
         assert np.array_equal(cs.u32(got["perm"]), ref["perm"])
         assert np.array_equal(cs.u64(got["leaves"]), ref["leaves"])
         assert np.array_equal(cs.u32(got["nodeCount"]), ref["nodeCount"])
-    # the short cut (4 plain passes + the fused fifth), redone on the device; then the 7 plain passes for 16 builds;
-    # then the short cut is tried again (and redone again): one pathological step does not cost every later one
-    short, plain = plans[0], plans[1]                        # 4 and 7 with the default 9-bit digits
-    assert plain > short + 1 and plans == [short] + [plain] * 16 + [short] + [plain] * 2
+    # the ladder of CS_SORT_AUTO: the short plan (3 plain passes + the fused last one), redone on the device; the default
+    # plan (4 + 1), redone as well; then the 7 plain passes for 16 builds; then the default plan is tried again (and
+    # redone again): one pathological step does not cost every later one
+    short, default, plain = plans[0], plans[1], plans[2]        # 3, 4 and 7 with the 9-bit digits
+    assert short + 1 == default and plain > default + 1
+    assert plans == [short, default] + [plain] * 16 + [default, plain]
+    # CS_SORT_DEFAULT never tries the short plan
+    ctx.setSortMode(cs.SORT_DEFAULT)
+    plans = []
+    for _ in range(3):
+        plans.append(ctx.sortPasses())
+        got = cs.buildOctree(ctx, d[0], d[1], d[2], 64)
+        assert np.array_equal(cs.u64(got["keys"]), ref["sortedKeys"]) and np.array_equal(cs.u32(got["perm"]), ref["perm"])
+    assert plans == [default, plain, plain]
     ctx.setSortMode(cs.SORT_AUTO)
+
+
+def test_auto_backs_off_from_the_short_plan(cs, ctx):
+    """More than 257 particles in a level-12 cell but none in a level-15 cell: the short plan is redone once, then the
+    default plan serves (no redo, no plain passes); uniform particles stay on the short plan."""
+    rng = np.random.default_rng(22)
+    n = 50000
+    k = np.concatenate([rng.integers(0, 1 << 63, n, dtype=np.uint64),
+                        (np.uint64(0x765432101) << np.uint64(27)) | rng.integers(0, 1 << 27, 2000, dtype=np.uint64)])
+    rng.shuffle(k)
+    ctx.setSortMode(cs.SORT_AUTO)
+    short = ctx.sortPasses()
+    plans = []
+    for _ in range(6):
+        plans.append(ctx.sortPasses())
+        check(cs, ctx, k, mode=None)
+    assert plans == [short] + [short + 1] * 5
+    ctx.setSortMode(cs.SORT_AUTO)
+    u = rng.integers(0, 1 << 63, 200000, dtype=np.uint64)
+    plans = []
+    for _ in range(4):
+        plans.append(ctx.sortPasses())
+        check(cs, ctx, u, mode=None)
+    assert plans == [short] * 4
 
 
 def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
@@ -141,12 +186,14 @@ def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
     context takes the plain passes."""
     rng = np.random.default_rng(5)
     k = np.concatenate([rng.integers(0, 1 << 63, 50000, dtype=np.uint64),
-                        (np.uint64(0x1234567) << np.uint64(30)) | rng.integers(0, 1 << LOW, 3000, dtype=np.uint64)])
+                        (np.uint64(0x1234567) << np.uint64(30)) | rng.integers(0, 1 << 18, 3000, dtype=np.uint64)])
     rng.shuffle(k)
     ctx.setSortMode(cs.SORT_AUTO)
-    short = ctx.sortPasses()                                    # 4 with the default 9-bit digits
+    short = ctx.sortPasses()                                    # 3 with the 9-bit digits
     check(cs, ctx, k)                                           # check() synchronises when it copies the result back
-    assert ctx.sortPasses() > short + 1                         # 7: all digits
+    assert ctx.sortPasses() == short + 1                        # the default plan
+    check(cs, ctx, k, mode=None)
+    assert ctx.sortPasses() > short + 2                         # 7: all digits
     check(cs, ctx, k, mode=None)
     ctx.setSortMode(cs.SORT_AUTO)
     assert ctx.sortPasses() == short
@@ -172,17 +219,18 @@ def test_unaligned_arrays(cs, ctx):
 
 
 @pytest.mark.parametrize("group", [3, 40, 200])
-def test_runs_that_are_not_neighbours_before_the_last_pass(cs, ctx, group):
-    """Keys that agree in bits 18..53 but differ in the top digit are interleaved in the order the fifth pass
-    reads (it is sorted by bits 18..53 only), so the members of a run (equal bits 18..62) are not neighbours
+def test_runs_that_are_not_neighbours_before_the_last_pass(cs, ctx, plan, group):
+    """Keys that agree in bits LOW..53 but differ in the top digit are interleaved in the order the last pass
+    reads (it is sorted by bits LOW..53 only), so the members of a run (equal bits LOW..62) are not neighbours
     there.  The tile cuts of that pass must not separate them: with groups this long every cut falls into one."""
+    mode, LOW = plan
     rng = np.random.default_rng(100 + group)
     n_groups = 300000 // group
-    mid = rng.choice(1 << 36, size=n_groups, replace=False).astype(np.uint64)            # bits 18..53
+    mid = rng.choice(1 << (54 - LOW), size=n_groups, replace=False).astype(np.uint64)    # bits LOW..53
     mid = np.repeat(mid, group)
     top = rng.integers(0, 4, mid.size, dtype=np.uint64) * np.uint64(127)                 # 4 different top digits
     low = rng.integers(0, 1 << LOW, mid.size, dtype=np.uint64)
     k = (top << np.uint64(54)) | (mid << np.uint64(LOW)) | low
     k[::11] = k[1::11][: k[::11].size]                                                   # and some equal whole keys
     rng.shuffle(k)
-    check(cs, ctx, k)
+    check(cs, ctx, k, mode)
