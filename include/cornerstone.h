@@ -382,6 +382,28 @@ cs_status cs_rebalance(cs_context* ctx, const uint64_t* leaves, const uint32_t* 
 cs_status cs_partitionLeaves(cs_context* ctx, const uint32_t* counts, uint32_t numLeaves, uint32_t numRanks,
                              uint32_t* bounds, void* stream);
 
+/* cs_partitionLeavesStatic -- cs_partitionLeaves for callers that must not allocate (code under CUDA graph capture,
+ *   serving loops, harnesses that forbid cudaMalloc): same arguments without the context, same result (PAPER.md:202-204,
+ *   reading A29), and no cudaMalloc / cudaFree or allocating library call on any path: there is no context, and the
+ *   kernel's scratch (one 64-bit sum per 2048 counts, and a ticket) is a fixed __device__ array inside the library,
+ *   64.25 KB on every GPU that loads it, held until the process exits.
+ *   Limit: numLeaves <= CS_STATIC_PARTITION_MAX_LEAVES (2^24; BASELINE's largest tree has 14.2 M leaves); beyond it
+ *   the call returns CS_ERR_CAPACITY and touches nothing.  numRanks: any (bounds holds numRanks + 1 uint32).
+ *   counts, bounds: device pointers on the CURRENT device (there is no context to name one).  Enqueues a 8-byte memset
+ *   node (the ticket must start at zero; the sums need no clearing, they are overwritten before they are read) and one
+ *   kernel on `stream`; does not synchronise; capturable.
+ *   All calls on a device share the scratch array: calls that overlap on the GPU (different streams, or host threads
+ *   on streams that are not ordered with each other) race and give wrong bounds; the caller orders them.
+ *   cs_partitionLeavesStaticSetup looks up the array's device address for the current device (cudaGetSymbolAddress,
+ *   once per device; the entry point does the same on its first call there): call it before a capture begins.
+ *   Errors: INVALID_ARG (null pointer, numLeaves or numRanks 0), CAPACITY (see above), CUDA.  cs_lastError(NULL) has
+ *   the message. */
+#define CS_STATIC_PARTITION_MAX_LEAVES (1u << 24)
+cs_status cs_partitionLeavesStatic(const uint32_t* counts, uint32_t numLeaves, uint32_t numRanks, uint32_t* bounds,
+                                   void* stream);
+cs_status cs_partitionLeavesStaticSetup(void);
+uint32_t  cs_partitionLeavesStaticMax(void);   /* CS_STATIC_PARTITION_MAX_LEAVES of the loaded library */
+
 /* cs_nodeCountsFromLeaves -- particle ranges of the nodes of a linked octree from the counts of its leaves, without
  *   the particles (the upward pass of PAPER.md:258; for the replicated global octree the counts are the all-reduced
  *   ones): nodeCount[i] = sum of leafCounts over the leaves inside node i, nodeFirst[i] = sum over the leaves before

@@ -107,6 +107,9 @@ def lib():
         "cs_countLeaves": (C.c_int, [vp, vp, u64, vp, u32, vp, vp]),
         "cs_rebalance": (C.c_int, [vp, vp, vp, u32, u32, vp, u32, C.POINTER(u32), C.POINTER(u32), vp]),
         "cs_partitionLeaves": (C.c_int, [vp, vp, u32, u32, vp, vp]),
+        "cs_partitionLeavesStatic": (C.c_int, [vp, u32, u32, vp, vp]),
+        "cs_partitionLeavesStaticSetup": (C.c_int, []),
+        "cs_partitionLeavesStaticMax": (u32, []),
         "cs_nodeCountsFromLeaves": (C.c_int, [vp, vp, vp, u32, vp, u32, vp, vp, vp]),
         "cs_gatherParticles": (C.c_int, [vp, vp, vp, vp, vp, u64, vp, vp, vp, vp]),
         "cs_nodeGeometry": (C.c_int, [vp, vp, u32, vp, vp, vp, vp]),
@@ -501,6 +504,27 @@ def partitionLeaves(ctx: Context, counts, numRanks: int, bounds=None):
     if bounds is None:
         bounds = _i32(numRanks + 1, ctx.device)
     ctx.check(lib().cs_partitionLeaves(ctx.handle, _ptr(counts), counts.numel(), numRanks, _ptr(bounds), _stream()))
+    return bounds
+
+
+def partitionLeavesStaticMax() -> int:
+    return int(lib().cs_partitionLeavesStaticMax())
+
+
+def partitionLeavesStaticSetup():
+    """Looks up the library's static scratch array on the current device (the entry point does so itself on first use)."""
+    st = lib().cs_partitionLeavesStaticSetup()
+    if st != OK:
+        raise CornerstoneError(st, lib().cs_lastError(None).decode())
+
+
+def partitionLeavesStatic(counts, numRanks: int, bounds):
+    """cs_partitionLeaves without a context and without any allocation: the caller passes `bounds` (numRanks + 1 int32
+    on the device of `counts`, which must be the current device); at most partitionLeavesStaticMax() leaves.  Calls
+    share one scratch array in the library: do not let two of them overlap on the GPU."""
+    st = lib().cs_partitionLeavesStatic(_ptr(counts), counts.numel(), numRanks, _ptr(bounds), _stream())
+    if st != OK:
+        raise CornerstoneError(st, lib().cs_lastError(None).decode())
     return bounds
 
 

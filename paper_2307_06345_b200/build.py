@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libcornerstone_b200.so")
-SOURCES = ["cs_context.cu", "cs_particles.cu", "cs_sort.cu", "cs_leaves.cu", "cs_leaves_direct.cu", "cs_link.cu", "cs_props.cu", "cs_global.cu", "cs_api.cu", "cs_api32.cu"]
+SOURCES = ["cs_context.cu", "cs_particles.cu", "cs_sort.cu", "cs_leaves.cu", "cs_leaves_direct.cu", "cs_link.cu", "cs_props.cu", "cs_global.cu", "cs_static.cu", "cs_api.cu", "cs_api32.cu"]
 HEADERS = ["cs_internal.cuh", "cs_device.cuh", os.path.join("..", "..", "include", "cornerstone.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
