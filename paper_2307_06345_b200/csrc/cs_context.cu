@@ -122,6 +122,7 @@ __global__ void __launch_bounds__(kScanBlock) scanKernel(const u32* __restrict__
                                                          u32* ticket, u64* lookback, u32 epoch,
                                                          const u32* __restrict__ epochBase)
 {
+    chainEnter();
     epoch += *epochBase;
     __shared__ u32 sTile, sPrefix;
     __shared__ u32 warpSums[kScanBlock / 32 + 1];
@@ -180,7 +181,7 @@ cs_status enqueueExclusiveScan(cs_context* ctx, const u32* in, u32* out, u32 n, 
     u32 epoch = nextEpoch(ctx, s);
     u32 tiles = divUp(n, kScanTile);
     u32 grid = tiles < (u32)ctx->numSMs * 8 ? tiles : (u32)ctx->numSMs * 8;
-    scanKernel<<<grid, kScanBlock, 0, s>>>(in, out, n, &ctx->ctrl->scanTicket, ctx->tileLookback, epoch, epochBase(ctx));
+    launchChained(scanKernel, dim3(grid), dim3(kScanBlock), 0, s, in, out, n, &ctx->ctrl->scanTicket, ctx->tileLookback, epoch, epochBase(ctx));
     CS_LAUNCH_CHECK(ctx, "scanKernel");
     return CS_OK;
 }

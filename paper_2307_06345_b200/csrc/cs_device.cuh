@@ -65,6 +65,17 @@ __device__ __forceinline__ void bulkPrefetchL2(const void* p, u32 bytes)
     if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// Programmatic dependent launch.  A kernel launched with launchChained() (cs_internal.cuh) may be scheduled while the
+// kernel before it on the stream still runs.  chainEnter() is the first statement of such a kernel: it lets the CTAs of
+// the kernel BEHIND this one take the slots this grid leaves free (they then wait in their own chainEnter), and waits
+// until the kernel before this one has finished and its writes are visible.  No global memory is touched before it.
+// Launched without the attribute, both instructions do nothing.
+__device__ __forceinline__ void chainEnter()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // ---- decoupled look-back words -----------------------------------------------------------
 // One 64-bit word per (tile, counter): [63:34] epoch, [33:32] status, [31:0] value.  Value and
 // flag travel in one 8-byte store, so no fence is needed between them.  The epoch makes

@@ -232,6 +232,30 @@ cs_status cudaFail(cs_context* ctx, cudaError_t e, const char* what);
         if (e__ != cudaSuccess) return ::cs::cudaFail((ctx), e__, name);       \
     } while (0)
 
+// Launch `kernel` so that it may be scheduled before the kernel in front of it on the stream has finished (programmatic
+// dependent launch: the launch latency and the prologue of one kernel hide behind the tail of the one before; what a
+// small build is made of).  ONLY for kernels whose first statement is chainEnter() (cs_device.cuh): that is where they
+// wait for the data of their predecessors.  Works under stream capture (a programmatic edge of the graph); behind a
+// memset, copy or event node, or a kernel without chainEnter(), it is an ordinary launch.
+#ifndef CS_CHAIN
+#define CS_CHAIN 1
+#endif
+template <typename... KArgs, typename... Args>
+inline void launchChained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = CS_CHAIN ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);     // errors: cudaGetLastError in CS_LAUNCH_CHECK
+}
+
 struct DeviceGuard {              // makes `dev` current for the scope and restores the caller's device
     int prev = -1;
     cudaError_t err = cudaSuccess;

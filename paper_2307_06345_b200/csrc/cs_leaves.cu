@@ -450,6 +450,7 @@ __device__ __forceinline__ void leavesEmitBody(const u64* K, const u32* off, u32
 __global__ void __launch_bounds__(256) leavesEmitKernel(const DeviceCtrl* ctrl, const u64* K0, const u32* off0, u64* leaves,
                                                         u32* counts, u32* offFinal)
 {
+    chainEnter();
     const u32 st = ctrl->status;
     if (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) return;   // outputs untouched
     leavesEmitBody(K0, off0, ctrl->nl[ctrl->rounds], leaves, counts, offFinal);
@@ -562,7 +563,7 @@ cs_status enqueueLeaves(cs_context* ctx, const u64* P, u64 n, u32 bucket, const 
         CS_TRY(enqueueLeavesDirect(ctx, P, n, bucket, cap, maxLevel, s));
         u32 g = divUp((u64)cap + 1, 256);
         if (g > persistentGrid) g = persistentGrid;
-        leavesEmitKernel<<<g, 256, 0, s>>>(ctrl, ctx->leafK[0], ctx->leafOff[0], leaves, counts, ctx->leafOffFinal);
+        launchChained(leavesEmitKernel, dim3(g), dim3(256), 0, s, ctrl, ctx->leafK[0], ctx->leafOff[0], leaves, counts, ctx->leafOffFinal);
         CS_LAUNCH_CHECK(ctx, "leavesEmitKernel");
         return CS_OK;
     }

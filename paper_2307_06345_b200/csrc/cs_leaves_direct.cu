@@ -255,6 +255,7 @@ __global__ void __launch_bounds__(kDirBlock, CS_DIR_MINBLOCKS)
                        unsigned char* __restrict__ flags, u32* __restrict__ totals, u32* __restrict__ listSize,
                        ulonglong2* __restrict__ listKeys, u32* __restrict__ listMeta)
 {
+    chainEnter();
     extern __shared__ __align__(16) unsigned char dsm[];
     __shared__ u32 sTotal, sMaxLevel;
     __shared__ u32 warpSums[kDirBlock / 32 + 1];
@@ -338,6 +339,7 @@ __global__ void __launch_bounds__(kEmitBlock)
                            const u32* __restrict__ listSize, const ulonglong2* __restrict__ listKeys,
                            const u32* __restrict__ listMeta, u64* __restrict__ K, u32* __restrict__ off, u32 cap)
 {
+    chainEnter();
     __shared__ unsigned short list[kDirTile];
     __shared__ u32 warpSums[kEmitBlock / 32 + 1];
     const u32 tid = threadIdx.x;
@@ -454,11 +456,11 @@ cs_status enqueueLeavesDirect(cs_context* ctx, const u64* P, u64 n, u32 bucket, 
     const u32 tiles = (u32)(n / kDirTile) + 1;            // positions 0 .. n inclusive
     // the bucket sizes of BASELINE.json's configurations get kernels with the bucket size folded in
     auto* kernel = bucket == 64 ? leavesLevelsKernel<64> : bucket == 16 ? leavesLevelsKernel<16> : leavesLevelsKernel<0>;
-    kernel<<<tiles, kDirBlock, L.total, s>>>(ctrl, P, (u32)n, bucket, maxLevel - 1, ctx->divLevel, ctx->dirFlags, ctx->dirTotals,
+    launchChained(kernel, dim3(tiles), dim3(kDirBlock), L.total, s, ctrl, P, (u32)n, bucket, maxLevel - 1, ctx->divLevel, ctx->dirFlags, ctx->dirTotals,
                                              ctx->dirListSize, ctx->dirListKeys, ctx->dirListMeta);
     CS_LAUNCH_CHECK(ctx, "leavesLevelsKernel");
     CS_TRY(enqueueExclusiveScan(ctx, ctx->dirTotals, ctx->dirBases, tiles, s));
-    leavesEmitDirectKernel<<<tiles, kEmitBlock, 0, s>>>(ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
+    launchChained(leavesEmitDirectKernel, dim3(tiles), dim3(kEmitBlock), 0, s, ctrl, P, (u32)n, ctx->divLevel, ctx->dirFlags, ctx->dirBases, tiles,
                                                        ctx->dirListSize, ctx->dirListKeys, ctx->dirListMeta,
                                                        ctx->leafK[0], ctx->leafOff[0], cap);
     CS_LAUNCH_CHECK(ctx, "leavesEmitDirectKernel");

@@ -104,6 +104,7 @@ __global__ void __launch_bounds__(kLinkBlock)
     linkCountKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves,
                     u32* __restrict__ tileHist)
 {
+    chainEnter();
     __shared__ u32 sWarp[kLinkWarps][kLinkBins];
     __shared__ u32 sStop;
     const u32 tid = threadIdx.x, lane = laneId(), warp = tid >> 5;
@@ -139,6 +140,7 @@ constexpr int kColItems = 4;
 __global__ void __launch_bounds__(256)
     linkScanKernel(DeviceCtrl* ctrl, const u32* dNumLeaves, u32 hNumLeaves, u32* __restrict__ tileHist)
 {
+    chainEnter();
     __shared__ u32 warpSums[256 / 32 + 1];
     const u32 st = ctrl->status;
     if (st == CS_ERR_CAPACITY || st == CS_ERR_NOT_CORNERSTONE) return;
@@ -208,6 +210,7 @@ __global__ void __launch_bounds__(kLinkBlock, CS_LINK_MINBLOCKS)
     linkEmitKernel(DeviceCtrl* ctrl, const u64* __restrict__ K, const u32* dNumLeaves, u32 hNumLeaves, LinkOut out,
                    const u32* __restrict__ tilePrefix)
 {
+    chainEnter();
     __shared__ u32 sLO[kLevels + 2];                  // level offsets
     __shared__ u32 sWarp[kLinkWarps][kLinkBins];      // per-warp counts -> running exclusive prefix
     __shared__ u32 sBase[kLinkBins];                  // tile's exclusive prefix per bin
@@ -332,13 +335,13 @@ cs_status enqueueLink(cs_context* ctx, const u64* leaves, const u32* dNumLeaves,
     u32 grid = divUp((u64)leafBound, kLinkTile);
     if (grid > gridCap) grid = gridCap;
     if (grid == 0) grid = 1;
-    linkCountKernel<<<grid, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, tileHist);
+    launchChained(linkCountKernel, dim3(grid), dim3(kLinkBlock), 0, s, ctrl, leaves, dNumLeaves, hNumLeaves, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkCountKernel");
-    linkScanKernel<<<kLinkBins, 256, 0, s>>>(ctrl, dNumLeaves, hNumLeaves, tileHist);
+    launchChained(linkScanKernel, dim3(kLinkBins), dim3(256), 0, s, ctrl, dNumLeaves, hNumLeaves, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkScanKernel");
     LinkOut out{prefixes, levels, childOffsets, parents, levelRange, leafToNode, nodeToLeaf, nodeCapacity,
                 leafOffsets, leafOffsets ? nodeFirst : nullptr, nodeCount};
-    linkEmitKernel<<<grid, kLinkBlock, 0, s>>>(ctrl, leaves, dNumLeaves, hNumLeaves, out, tileHist);
+    launchChained(linkEmitKernel, dim3(grid), dim3(kLinkBlock), 0, s, ctrl, leaves, dNumLeaves, hNumLeaves, out, tileHist);
     CS_LAUNCH_CHECK(ctx, "linkEmitKernel");
     return CS_OK;
 }

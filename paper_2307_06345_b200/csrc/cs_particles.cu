@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(kBoxBlock) boxKernel(const double* __restrict_
                                                        const double* __restrict__ z, u64 n, double* partials,
                                                        u32* counter, double* box6)
 {
+    chainEnter();
     MinMax3 m;
     mmInit(m);
     const double* c[3] = {x, y, z};
@@ -152,8 +153,8 @@ cs_status enqueueBox(cs_context* ctx, const double* x, const double* y, const do
     u32 grid = (u32)ctx->numSMs * kBoxBlocksPerSM;
     u32 need = divUp(work, kBoxBlock);
     if (need < grid) grid = need ? need : 1;
-    if (vec) boxKernel<true><<<grid, kBoxBlock, 0, s>>>(x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
-    else boxKernel<false><<<grid, kBoxBlock, 0, s>>>(x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
+    if (vec) launchChained(boxKernel<true>, dim3(grid), dim3(kBoxBlock), 0, s, x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
+    else launchChained(boxKernel<false>, dim3(grid), dim3(kBoxBlock), 0, s, x, y, z, n, ctx->boxPartials, ctx->boxCounter, box6);
     CS_LAUNCH_CHECK(ctx, "boxKernel");
     return CS_OK;
 }
@@ -340,6 +341,7 @@ __global__ void __launch_bounds__(kKeysBlock, CS_KEYS_MINBLOCKS) keysKernel(cons
                                                          u32* gHist, const unsigned short* __restrict__ hilbertTable,
                                                          u32* __restrict__ keys32)
 {
+    chainEnter();
     constexpr int kHistWords = HIST >= 0 ? (kSortPasses - HIST) * kRadix : 1;
     __shared__ u32 sh[kHistWords];
     __shared__ unsigned short sTab[HILBERT ? kHilbertStates * kHilbertEntries : 1];
@@ -431,7 +433,7 @@ cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const d
     if (need < grid) grid = need ? need : 1;
     u32* h = ctx->sortHist;
     const unsigned short* tab = ctx->hilbertTable;
-#define CS_KEYS_LAUNCH(V, H, C) keysKernel<V, H, C><<<grid, kKeysBlock, 0, s>>>(x, y, z, n, box6, keys, h, tab, keys32)
+#define CS_KEYS_LAUNCH(V, H, C) launchChained(keysKernel<V, H, C>, dim3(grid), dim3(kKeysBlock), 0, s, x, y, z, n, box6, keys, h, tab, keys32)
 #define CS_KEYS_HIST(V, C)                                        \
     do {                                                          \
         if (histFrom < 0) CS_KEYS_LAUNCH(V, -1, C);               \

@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(kHistBlock) sortHistKernel(const u64* __restri
 // exclusive scan of each pass's digit counts, in place (one CTA per pass)
 __global__ void __launch_bounds__(kRadix) sortScanHistKernel(u32* gHist)
 {
+    chainEnter();
     __shared__ u32 warpSums[kRadix / 32 + 1];
     const u32 i = blockIdx.x * kRadix + threadIdx.x;
     u32 total;
@@ -311,6 +312,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
                    u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase /*scanned hist*/, u32* ticket,
                    u64* lookback, u32 epoch, const u32* __restrict__ epochBase)
 {
+    chainEnter();
     epoch += *epochBase;
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmemT<KeyT>& sm = *reinterpret_cast<SortSmemT<KeyT>*>(smemRaw);
@@ -471,6 +473,7 @@ __global__ void __launch_bounds__(kSortBlock, kSortMinBlocks)
                        u32* __restrict__ valsOut, u32 n, const u32* __restrict__ digitBase, u32* ticket, u64* lookback,
                        u32 epoch, const u32* __restrict__ epochBase, u32* redo)
 {
+    chainEnter();
     epoch += *epochBase;
     extern __shared__ __align__(16) unsigned char smemRaw[];
     SortSmem& sm = *reinterpret_cast<SortSmem*>(smemRaw);
@@ -638,7 +641,7 @@ static cs_status launchPass(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 {
     const u32 epoch = nextEpoch(ctx, s);
     const int in = pl.cur, out = in ^ 1;
-    onesweepKernel<SHIFT, FIRST, u64><<<pl.tiles, kSortBlock, sizeof(SortSmem), s>>>(
+    launchChained(onesweepKernel<SHIFT, FIRST, u64>, dim3(pl.tiles), dim3(kSortBlock), sizeof(SortSmem), s, 
         pl.k[in], FIRST ? nullptr : pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (SHIFT / kRadixBits) * kRadix,
         ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, epochBase(ctx));
     CS_LAUNCH_CHECK(ctx, "onesweepKernel");
@@ -758,7 +761,7 @@ static cs_status enqueueShortCut(cs_context* ctx, PassPlan& pl, bool fused, cuda
     {   // top digit; this pass also orders the low bits inside the runs
         const u32 epoch = nextEpoch(ctx, s);
         const int in = pl.cur, out = in ^ 1;
-        onesweepLastKernel<kLastShift, kLow><<<divUp(pl.n, kLastTile), kSortBlock, sizeof(SortSmem), s>>>(
+        launchChained(onesweepLastKernel<kLastShift, kLow>, dim3(divUp(pl.n, kLastTile)), dim3(kSortBlock), sizeof(SortSmem), s, 
             pl.k[in], pl.v[in], pl.k[out], pl.v[out], pl.n, ctx->sortHist + (kSortPasses - 1) * kRadix,
             ctx->sortTickets + pl.ticketSlot++, ctx->sortLookback, epoch, epochBase(ctx), redo);
         CS_LAUNCH_CHECK(ctx, "onesweepLastKernel");
@@ -805,7 +808,7 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
                                                        planFirstDigit(plan));
             CS_LAUNCH_CHECK(ctx, "sortHistKernel");
         }
-        sortScanHistKernel<<<kSortPasses, kRadix, 0, s>>>(ctx->sortHist);
+        launchChained(sortScanHistKernel, dim3(kSortPasses), dim3(kRadix), 0, s, ctx->sortHist);
         CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
     }
     ctx->evUsed[CS_STAGE_SORT_FIXUP] = false;
@@ -912,7 +915,7 @@ cs_status enqueueSort32(cs_context* ctx, u32* keys, u32* perm, u64 n, cudaStream
         if (need < grid) grid = need ? need : 1;
         sortHist32Kernel<<<grid, kHistBlock, 0, s>>>(keys, n, ctx->sortHist);
         CS_LAUNCH_CHECK(ctx, "sortHist32Kernel");
-        sortScanHistKernel<<<kSortPasses32, kRadix, 0, s>>>(ctx->sortHist);
+        launchChained(sortScanHistKernel, dim3(kSortPasses32), dim3(kRadix), 0, s, ctx->sortHist);
         CS_LAUNCH_CHECK(ctx, "sortScanHistKernel");
     }
     u32* const k[2] = {keys, reinterpret_cast<u32*>(ctx->keysAlt)};
