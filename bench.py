@@ -379,6 +379,43 @@ def run_ours(args):
     value = whole_job_value(n, world, ms_per_step)
     stages = {k: v / args.steps for k, v in stages.items()}
 
+    # ---- node properties on the finished tree (first row past the hot path; NOT part of the timed step); before the other
+    # legs: the gather's random 8-byte reads depend on where the allocator has put the arrays (5 ms here, up to 59 ms
+    # measured after the legs below had run) ------
+    props = None
+    if args.props:
+        def timed(fn, reps=5):
+            fn()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(reps):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); out = fn(); e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            return float(np.mean(ts)), out
+        nn = tree["numNodes"]
+        peak = _peaks()[0]
+        t_g, (xs, ys, zs) = timed(lambda: cs.gatherParticles(ctx, dx, dy, dz, tree["perm"]))
+        t_geo, (centers, half) = timed(lambda: cs.nodeGeometry(ctx, tree["prefixes"], tree["box6"]))
+        t_com, com = timed(lambda: cs.nodeMassCenters(ctx, xs, ys, zs, tree, centers))
+        box_h = tree["box6"].cpu().numpy()
+        focus = [box_h[0], box_h[0] + 0.25 * (box_h[1] - box_h[0]), box_h[2], box_h[2] + 0.25 * (box_h[3] - box_h[2]),
+                 box_h[4], box_h[4] + 0.25 * (box_h[5] - box_h[4])]
+        t_mac, mac = timed(lambda: cs.macMinDistance(ctx, centers, half, focus, 0.5))
+
+        def row(ms, nbytes):
+            return {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / (ms * 1e-3) / 1e9,
+                    "frac_of_measured_peak": nbytes / (ms * 1e-3) / 1e9 / peak}
+        props = {"gather": row(t_g, n * (4 + 24 + 24)),                       # perm + 3 gathered reads + 3 writes
+                 "geometry": row(t_geo, nn * (8 + 48)),
+                 "mass_centers": row(t_com, n * 24 + nn * (12 + 24 + 24)),  # sorted coordinates once + per-node arrays
+                 "mac": row(t_mac, nn * (48 + 1)),
+                 "mac_pass_fraction": float(mac.float().mean().item()), "nodes": nn,
+                 "note": "cs_gatherParticles, cs_nodeGeometry, cs_nodeMassCenters (2 launches), cs_macMinDistance; "
+                         "gather reads 8-byte words at random: 32-byte sectors make its DRAM traffic about 4x the useful bytes"}
+        del xs, ys, zs, centers, half, com, mac
+
     # ---- end to end: HOST buffers through cs_buildOctreeHost, copies inside the timed region ---
     e2e = None
     if not args.no_e2e:
@@ -549,40 +586,6 @@ def run_ours(args):
         incremental = {"rebuilds": len(times), "ms_per_rebuild": float(np.mean(times)), "ms_each": times,
                        "rounds": rounds, "mparticles_per_s": n / (float(np.mean(times)) * 1e-3) / 1e6,
                        "what": "box + keys + full re-sort + buildLeaves(previous leaves) + link + counts"}
-
-    # ---- node properties on the finished tree (first row past the hot path; NOT part of the timed step) ------
-    props = None
-    if args.props:
-        def timed(fn, reps=5):
-            fn()
-            torch.cuda.synchronize()
-            ts = []
-            for _ in range(reps):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(); out = fn(); e1.record()
-                torch.cuda.synchronize()
-                ts.append(e0.elapsed_time(e1))
-            return float(np.mean(ts)), out
-        nn = tree["numNodes"]
-        t_g, (xs, ys, zs) = timed(lambda: cs.gatherParticles(ctx, dx, dy, dz, tree["perm"]))
-        t_geo, (centers, half) = timed(lambda: cs.nodeGeometry(ctx, tree["prefixes"], tree["box6"]))
-        t_com, com = timed(lambda: cs.nodeMassCenters(ctx, xs, ys, zs, tree, centers))
-        box_h = tree["box6"].cpu().numpy()
-        focus = [box_h[0], box_h[0] + 0.25 * (box_h[1] - box_h[0]), box_h[2], box_h[2] + 0.25 * (box_h[3] - box_h[2]),
-                 box_h[4], box_h[4] + 0.25 * (box_h[5] - box_h[4])]
-        t_mac, mac = timed(lambda: cs.macMinDistance(ctx, centers, half, focus, 0.5))
-
-        def row(ms, nbytes):
-            return {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / (ms * 1e-3) / 1e9,
-                    "frac_of_measured_peak": nbytes / (ms * 1e-3) / 1e9 / peak}
-        props = {"gather": row(t_g, n * (4 + 24 + 24)),                       # perm + 3 gathered reads + 3 writes
-                 "geometry": row(t_geo, nn * (8 + 48)),
-                 "mass_centers": row(t_com, n * 24 + nn * (12 + 24 + 24)),  # sorted coordinates once + per-node arrays
-                 "mac": row(t_mac, nn * (48 + 1)),
-                 "mac_pass_fraction": float(mac.float().mean().item()), "nodes": nn,
-                 "note": "cs_gatherParticles, cs_nodeGeometry, cs_nodeMassCenters (2 launches), cs_macMinDistance; "
-                         "gather reads 8-byte words at random: 32-byte sectors make its DRAM traffic about 4x the useful bytes"}
-        del xs, ys, zs, centers, half, com, mac
 
     # ---- CPU baseline: the oracle as it stands, one core, bounded sample ---------------------
     cpu = None
