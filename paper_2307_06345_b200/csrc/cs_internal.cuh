@@ -148,7 +148,7 @@ struct cs_context {
     bool buildGraphSeen = false;
     cs::u32 buildGraphEpochs = 0;      // epochs one replay consumes
     uint64_t buildGraphLaunches = 0;   // kernels one replay launches
-    uint64_t graphMaxParticles = 1ull << 22;   // builds of at most this many particles are captured and replayed
+    uint64_t graphMaxParticles = 1ull << 32;   // builds of at most this many particles are captured and replayed (all)
     int sortMode = CS_SORT_AUTO;       // cs_setSortMode
     int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after the default plan needed the redo
     int shortLeft = 0;                 // CS_SORT_AUTO: sorts left before the short plan is tried again
