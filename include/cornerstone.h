@@ -56,8 +56,8 @@ typedef enum cs_status {
 enum {
     CS_STAGE_BOX = 0, CS_STAGE_KEYS = 1, CS_STAGE_SORT = 2, CS_STAGE_LEAVES = 3, CS_STAGE_LINK = 4,
     CS_STAGE_COUNTS = 5, CS_STAGE_SORT_HIST = 6,
-    CS_STAGE_SORT_PASSES = 7,    /* the plain radix passes: 3 or 4 (short / default plan) or 7 (plain plan) */
-    CS_STAGE_SORT_FIXUP = 8,     /* short / default plan: the last pass, which also orders the low bits, + the gated redo launch */
+    CS_STAGE_SORT_PASSES = 7,    /* the plain radix passes: 2, 3 or 4 (tiny / short / default plan) or 7 (plain plan) */
+    CS_STAGE_SORT_FIXUP = 8,     /* tiny / short / default plan: the last pass, which also orders the low bits, + the gated redo launch */
     CS_NUM_STAGES = 9
 };
 
@@ -132,18 +132,20 @@ cs_status cs_sortKeys(cs_context* ctx, uint64_t* keys, uint32_t* perm, uint64_t 
  *   bits below 9 F inside every run of equal leading digits.  If some run is longer than 257 elements, one more launch
  *   behind it redoes the sort with the 7 plain passes, decided on the device with no host round trip; the context
  *   learns of it (cs_buildOctree reads it with its sizes; after cs_sortKeys it follows the stream to the host).
- *   CS_SORT_AUTO (default): the short plan (F = 3: 4 passes; fits while no cell of octree level 12 holds more than 257
- *   particles); after it had to be redone, the default plan (F = 2: 5 passes; level 15) for the next 256 sorts, then
- *   the short plan is tried again (512, 1024, ... sorts after every further failure, at most 16384); after the default
- *   plan had to be redone, the 7 plain passes for 16 sorts.
- *   CS_SORT_DEFAULT: as CS_SORT_AUTO without the short plan.  CS_SORT_SHORT: always the short plan (redone when it does
- *   not fit).  CS_SORT_PLAIN: always the 7 plain LSD passes.
+ *   CS_SORT_AUTO (default): a ladder over the plans, finest first: the tiny plan (F = 4: 3 passes; fits while no cell
+ *   of octree level 9 holds more than 257 particles: uniform particles, up to billions of them), the short plan
+ *   (F = 3: 4 passes; level 12), the default plan (F = 2: 5 passes; level 15).  After a plan had to be redone the
+ *   context uses the next one for the next 256 sorts, then tries the finer one again (512, 1024, ... sorts after every
+ *   further failure, at most 16384; a plan is not retried while a coarser one still fails); after the default plan had
+ *   to be redone, the 7 plain passes for 16 sorts.
+ *   CS_SORT_DEFAULT: as CS_SORT_AUTO without the tiny and the short plan.  CS_SORT_SHORT, CS_SORT_TINY: always that plan
+ *   (redone when it does not fit).  CS_SORT_PLAIN: always the 7 plain LSD passes.
  *   Setting a mode also forgets earlier redos.  The sorted keys and perm are identical in all modes.
  *   Errors: INVALID_ARG. */
-enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1, CS_SORT_DEFAULT = 2, CS_SORT_SHORT = 3 };
+enum { CS_SORT_AUTO = 0, CS_SORT_PLAIN = 1, CS_SORT_DEFAULT = 2, CS_SORT_SHORT = 3, CS_SORT_TINY = 4 };
 cs_status cs_setSortMode(cs_context* ctx, int mode);
-/* Plain radix passes of the next sort on this context (the ones CS_STAGE_SORT_PASSES times): 3 or 4 (followed by the
- * fused last pass) or 7 (0 if ctx is NULL). */
+/* Plain radix passes of the next sort on this context (the ones CS_STAGE_SORT_PASSES times): 2, 3 or 4 (followed by
+ * the fused last pass) or 7 (0 if ctx is NULL). */
 int cs_sortPasses(const cs_context* ctx);
 
 /* cs_buildLeaves -- cornerstone leaf array by alternating f (Eq. 3) and g = g3 o g2 o g1

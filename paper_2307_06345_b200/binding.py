@@ -30,7 +30,7 @@ STAGE_NAMES = ("box", "keys", "sort", "leaves", "link", "counts", "sort_hist", "
 
 CURVE_MORTON, CURVE_HILBERT = 0, 1
 LEAVES_AUTO, LEAVES_ITERATIVE = 0, 1
-SORT_AUTO, SORT_PLAIN, SORT_DEFAULT, SORT_SHORT = 0, 1, 2, 3
+SORT_AUTO, SORT_PLAIN, SORT_DEFAULT, SORT_SHORT, SORT_TINY = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_NOT_CORNERSTONE, ERR_NOT_CONVERGED, ERR_CUDA = range(6)
 _STATUS_NAMES = {0: "CS_OK", 1: "CS_ERR_INVALID_ARG", 2: "CS_ERR_CAPACITY", 3: "CS_ERR_NOT_CORNERSTONE",
                  4: "CS_ERR_NOT_CONVERGED", 5: "CS_ERR_CUDA"}
@@ -207,8 +207,8 @@ class Context:
         self.check(lib().cs_setCurve(self.handle, int(curve)))
 
     def setSortMode(self, mode: int):
-        """SORT_AUTO (short plan, default plan, plain passes: whichever the input allows), SORT_DEFAULT (never the short
-        plan), SORT_SHORT (always the short plan) or SORT_PLAIN."""
+        """SORT_AUTO (tiny, short, default plan, plain passes: whichever the input allows), SORT_DEFAULT (never the tiny
+        or the short plan), SORT_SHORT / SORT_TINY (always that plan) or SORT_PLAIN."""
         self.check(lib().cs_setSortMode(self.handle, int(mode)))
 
     def setGraphLimit(self, max_particles: int):

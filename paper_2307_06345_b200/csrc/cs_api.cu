@@ -179,12 +179,14 @@ cs_status cs_buildLeaves(cs_context* ctx, const uint64_t* sortedKeys, uint64_t n
 cs_status cs_setSortMode(cs_context* ctx, int mode)
 {
     if (!ctx) return fail(nullptr, CS_ERR_INVALID_ARG, "cs_setSortMode: ctx is null");
-    if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN && mode != CS_SORT_DEFAULT && mode != CS_SORT_SHORT)
+    if (mode != CS_SORT_AUTO && mode != CS_SORT_PLAIN && mode != CS_SORT_DEFAULT && mode != CS_SORT_SHORT && mode != CS_SORT_TINY)
         return fail(ctx, CS_ERR_INVALID_ARG, "cs_setSortMode: unknown mode %d", mode);
     ctx->sortMode = mode;
     ctx->autoPlainLeft = 0;
-    ctx->shortLeft = 0;
-    ctx->shortHold = kShortHold;
+    for (int p = 0; p < kPlanDefault; ++p) {
+        ctx->planLeft[p] = 0;
+        ctx->planHold[p] = kShortHold;
+    }
     ctx->hostCtrl->sortRedoHint = 0;
     return CS_OK;
 }

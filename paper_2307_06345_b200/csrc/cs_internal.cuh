@@ -26,18 +26,20 @@ constexpr int kRoundSlots = kMaxRounds + 2;
 constexpr int kRadixBits = CS_RADIX_BITS;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = (63 + kRadixBits - 1) / kRadixBits;   // 63 key bits: 7 passes of 9 bits
-// Sort plans (cs_sort.cu): the plain plan sorts by all digits; the default plan by the digits kSortTopFirst .. (bits
-// 18..62) and orders the bits below inside runs of equal leading digits in its last pass; the short plan does the same
-// from digit kSortShortFirst (bits 27..62: one pass less), which works as long as no cell of octree level 12 holds more
-// than 257 particles.  A plan whose last pass finds a run too long is redone on the device and the context moves to the
-// next plan for a while.
-enum { kPlanShort = 0, kPlanDefault = 1, kPlanPlain = 2 };
+// Sort plans (cs_sort.cu): the plain plan sorts by all digits; a plan with first digit F sorts by the digits F .. 6 and
+// orders the bits below inside runs of equal leading digits in its last pass: the default plan (F = kSortTopFirst: bits
+// 18..62, 5 passes), the short plan (F = 3: bits 27..62, 4 passes: fits while no cell of octree level 12 holds more than
+// 257 particles) and the tiny plan (F = kSortMaxFirst = 4: bits 36..62, 3 passes: no such cell on level 9; what uniform
+// particles allow up to billions of them).  A plan whose last pass finds a run too long is redone on the device and the
+// context moves to the next plan for a while (the ladder of CS_SORT_AUTO).  Plans are numbered finest first.
+enum { kPlanTiny = 0, kPlanShort = 1, kPlanDefault = 2, kPlanPlain = 3 };
 constexpr int kSortTopFirst = 2;
 constexpr int kSortShortFirst = 3;
+constexpr int kSortMaxFirst = 4;
 constexpr int kPlainHold = 16;        // sorts on the plain plan after the default plan needed the redo, before it is tried again
-constexpr int kShortHold = 256;       // sorts on the default plan after the short plan needed the redo (doubles with every failure)
+constexpr int kShortHold = 256;       // sorts before a plan that needed the redo is tried again (doubles with every failure)
 constexpr int kShortHoldMax = 1 << 14;
-inline int planFirstDigit(int plan) { return plan == kPlanShort ? kSortShortFirst : plan == kPlanDefault ? kSortTopFirst : 0; }
+inline int planFirstDigit(int plan) { return plan == kPlanPlain ? 0 : kSortMaxFirst - plan; }
 inline int planPasses(int plan) { return kSortPasses - planFirstDigit(plan); }
 #ifndef CS_SORT_BLOCK
 #define CS_SORT_BLOCK 512
@@ -151,8 +153,8 @@ struct cs_context {
     uint64_t graphMaxParticles = 1ull << 32;   // builds of at most this many particles are captured and replayed (all)
     int sortMode = CS_SORT_AUTO;       // cs_setSortMode
     int autoPlainLeft = 0;             // CS_SORT_AUTO: sorts left on the plain plan after the default plan needed the redo
-    int shortLeft = 0;                 // CS_SORT_AUTO: sorts left before the short plan is tried again
-    int shortHold = cs::kShortHold;    // the next value of shortLeft (back-off)
+    int planLeft[cs::kPlanDefault] = {0, 0};                             // CS_SORT_AUTO: sorts left before the tiny / short plan is tried again
+    int planHold[cs::kPlanDefault] = {cs::kShortHold, cs::kShortHold};   // the next value of planLeft[] (back-off)
     int lastPlan = cs::kPlanDefault;   // plan of the last sort enqueued (whose redo flag may still arrive)
     cs::u32 redoGrid = 0;              // CTAs of onesweepRedoKernel that are resident together (cooperative launch)
 
@@ -303,7 +305,7 @@ cs_status leavesInit(cs_context*);
 cs_status enqueueSortReset(cs_context*, cudaStream_t);
 u64* sortSource(cs_context*, u64* keys, int plan);   // where the first radix pass reads the unsorted keys
 cs_status enqueueSort32(cs_context*, u32* keys, u32* perm, u64 n, cudaStream_t);   // 30-bit keys: 4 plain passes
-int sortDecidePlan(cs_context*);              // plan of the next sort (kPlanShort / kPlanDefault / kPlanPlain)
+int sortDecidePlan(cs_context*);              // plan of the next sort (kPlanTiny .. kPlanPlain)
 void sortPlanOutcome(cs_context*, int plan, bool redone);   // what the host learnt about a finished sort
 int sortPeekPlainPasses(const cs_context*);   // plain passes of the next sort (cs_sortPasses)
 cs_status enqueueSort(cs_context*, u64* keys, u32* perm, u64 n, bool fused, int plan, cudaStream_t);

@@ -438,6 +438,7 @@ cs_status enqueueKeys(cs_context* ctx, const double* x, const double* y, const d
     do {                                                          \
         if (histFrom < 0) CS_KEYS_LAUNCH(V, -1, C);               \
         else if (histFrom == 0) CS_KEYS_LAUNCH(V, 0, C);          \
+        else if (histFrom == kSortMaxFirst) CS_KEYS_LAUNCH(V, kSortMaxFirst, C); \
         else if (histFrom == kSortShortFirst) CS_KEYS_LAUNCH(V, kSortShortFirst, C); \
         else CS_KEYS_LAUNCH(V, kSortTopFirst, C);                 \
     } while (0)

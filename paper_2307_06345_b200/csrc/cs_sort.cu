@@ -427,6 +427,7 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headM
         const u32 H = headMask[i >> 5];
         const bool act = i < valid;
         const u32 mine = low[2 * (act ? i : cb)];
+        const u64 mineKey = keys[act ? i : cb];             // LOW > 32: the low word does not hold all the low bits
         const u32 dstBase = sm.globalBase[digitOf(keys[act ? i : cb], SHIFT)];
         u32 slot = i;
         if (H != kFull || !(headMask[(i >> 5) + 1] & 1u)) {  // not heads only, or the last slot's run goes on behind them
@@ -451,11 +452,19 @@ __device__ __forceinline__ void tileWriteOutFixup(const SortSmem& sm, u32* headM
                 runEnd = runStart;
             }
             u32 before = 0;                                  // members that precede: smaller low bits, or equal and earlier
-            if (act)
-                for (u32 m = runStart; m < runEnd; ++m) {
-                    const u32 v = low[2 * m];
-                    before += (v < mine || (v == mine && m < i)) ? 1u : 0u;
+            if (act) {
+                if constexpr (LOW <= 32) {
+                    for (u32 m = runStart; m < runEnd; ++m) {
+                        const u32 v = low[2 * m];
+                        before += (v < mine || (v == mine && m < i)) ? 1u : 0u;
+                    }
+                } else {                                     // the members of a run agree in the bits >= LOW: whole keys
+                    for (u32 m = runStart; m < runEnd; ++m) {
+                        const u64 v = keys[m];
+                        before += (v < mineKey || (v == mineKey && m < i)) ? 1u : 0u;
+                    }
                 }
+            }
             slot = runStart + before;
         }
         if (act && !tooLong) {
@@ -580,13 +589,13 @@ __global__ void __launch_bounds__(kSortBlock, 1) onesweepRedoKernel(const RedoAr
     const u32 tid = threadIdx.x;
     {   // digit counts of the passes the key kernel did not count (zero so far), then their exclusive scans
         u32* sh = reinterpret_cast<u32*>(smemRaw);
-        const int first = (int)a.first;                       // at most kSortShortFirst digits: 6 KB of counters
+        const int first = (int)a.first;                       // at most kSortMaxFirst digits: 8 KB of counters
         for (int i = tid; i < first * kRadix; i += kSortBlock) sh[i] = 0;
         __syncthreads();
         for (u64 i = (u64)blockIdx.x * kSortBlock + tid; i < a.n; i += (u64)gridDim.x * kSortBlock) {
             const u64 k = a.k[0][i];
 #pragma unroll
-            for (int p = 0; p < kSortShortFirst; ++p)
+            for (int p = 0; p < kSortMaxFirst; ++p)
                 if (p < first) atomicAdd(&sh[p * kRadix + digitOf(k, p * kRadixBits)], 1u);
         }
         __syncthreads();
@@ -622,11 +631,11 @@ cs_status enqueueSortReset(cs_context* ctx, cudaStream_t s)
 }
 
 // A plan with first digit F sorts by the digits F .. kSortPasses - 1, the last of them (the key's top digit) in the
-// fused pass that also orders the bits below F * kRadixBits inside runs of equal leading digits; F = kSortShortFirst
-// (short plan), kSortTopFirst (default plan).  The plain plan sorts by all kSortPasses digits.
+// fused pass that also orders the bits below F * kRadixBits inside runs of equal leading digits; F = kSortMaxFirst
+// (tiny plan), kSortShortFirst (short plan), kSortTopFirst (default plan).  The plain plan sorts by all kSortPasses digits.
 constexpr int kLastShift = (kSortPasses - 1) * kRadixBits;
-static_assert(kSortShortFirst * kRadixBits <= 32 && kSortShortFirst + 1 < kSortPasses && kSortShortFirst == kSortTopFirst + 1,
-              "the fix-up compares the keys' low words");
+static_assert(kSortMaxFirst + 1 < kSortPasses && kSortMaxFirst == kSortShortFirst + 1 && kSortShortFirst == kSortTopFirst + 1,
+              "plans of the sort: first digits 4, 3, 2");
 
 struct PassPlan {
     u64* k[2];
@@ -669,8 +678,10 @@ cs_status sortInit(cs_context* ctx)
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<0, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kSortTopFirst * kRadixBits, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kSortShortFirst * kRadixBits, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepKernel<kSortMaxFirst * kRadixBits, true, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kSortTopFirst * kRadixBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kSortShortFirst * kRadixBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    CS_CUDA(ctx, cudaFuncSetAttribute(onesweepLastKernel<kLastShift, kSortMaxFirst * kRadixBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     CS_CUDA(ctx, cudaFuncSetAttribute(onesweepRedoKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int perSM = 0;
     CS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSM, onesweepRedoKernel, kSortBlock, bytes));
@@ -697,33 +708,46 @@ static cs_status launchPasses(cs_context* ctx, PassPlan& pl, cudaStream_t s)
 u64* sortSource(cs_context* ctx, u64* keys, int plan) { return (planPasses(plan) & 1) ? ctx->keysAlt : keys; }
 
 // Which plan the next sort on this context runs (cs_setSortMode; include/cornerstone.h).  CS_SORT_AUTO climbs a
-// ladder: the short plan; after it had to be redone, the default plan for shortHold sorts (doubling with every failure,
-// so that inputs that never fit the short plan pay for ever fewer attempts); after the default plan had to be redone,
-// the plain plan for kPlainHold sorts.
+// ladder: the tiny plan; after a plan had to be redone, the next coarser one for planHold sorts (doubling with every
+// failure, so that inputs that never fit a plan pay for ever fewer attempts at it); after the default plan had to be
+// redone, the plain plan for kPlainHold sorts.
+static bool planForced(const cs_context* ctx)
+{
+    return ctx->sortMode == CS_SORT_PLAIN || ctx->sortMode == CS_SORT_SHORT || ctx->sortMode == CS_SORT_TINY;
+}
+
 static int peekPlan(const cs_context* ctx)
 {
     switch (ctx->sortMode) {
         case CS_SORT_PLAIN: return kPlanPlain;
         case CS_SORT_SHORT: return kPlanShort;
-        case CS_SORT_DEFAULT: return ctx->autoPlainLeft > 0 ? kPlanPlain : kPlanDefault;
-        default: return ctx->autoPlainLeft > 0 ? kPlanPlain : ctx->shortLeft > 0 ? kPlanDefault : kPlanShort;
+        case CS_SORT_TINY: return kPlanTiny;
+        default: break;
     }
+    if (ctx->autoPlainLeft > 0) return kPlanPlain;
+    if (ctx->sortMode == CS_SORT_AUTO)
+        for (int p = 0; p < kPlanDefault; ++p)
+            if (ctx->planLeft[p] == 0) return p;
+    return kPlanDefault;
 }
 
 void sortPlanOutcome(cs_context* ctx, int plan, bool redone)
 {
+    if (plan == kPlanPlain) return;
     if (!redone) {
-        if (plan == kPlanShort) ctx->shortHold = kShortHold;           // it fits: forget the back-off
+        if (plan < kPlanDefault) ctx->planHold[plan] = kShortHold;     // it fits: forget the back-off
         return;
     }
-    if (ctx->sortMode == CS_SORT_PLAIN || ctx->sortMode == CS_SORT_SHORT) return;   // forced plans do not adapt
-    if (plan == kPlanShort) {
-        ctx->shortLeft = ctx->shortHold;
-        ctx->shortHold = ctx->shortHold * 2 < kShortHoldMax ? ctx->shortHold * 2 : kShortHoldMax;
-    } else if (plan == kPlanDefault) {
+    if (planForced(ctx)) return;                                        // forced plans do not adapt
+    if (plan == kPlanDefault) {
         ctx->autoPlainLeft = kPlainHold;
-        if (ctx->shortLeft < ctx->shortHold) ctx->shortLeft = ctx->shortHold;   // what the default plan cannot do, the short one cannot
+    } else {
+        ctx->planLeft[plan] = ctx->planHold[plan];
+        ctx->planHold[plan] = ctx->planHold[plan] * 2 < kShortHoldMax ? ctx->planHold[plan] * 2 : kShortHoldMax;
     }
+    // a run too long for this plan lies inside a run of every finer plan: they wait at least their full hold again
+    for (int p = 0; p < plan && p < kPlanDefault; ++p)
+        if (ctx->planLeft[p] < ctx->planHold[p]) ctx->planLeft[p] = ctx->planHold[p];
 }
 
 int sortDecidePlan(cs_context* ctx)
@@ -733,16 +757,24 @@ int sortDecidePlan(cs_context* ctx)
         sortPlanOutcome(ctx, ctx->lastPlan, true);
     }
     const int plan = peekPlan(ctx);
-    if (plan == kPlanPlain && ctx->autoPlainLeft > 0) --ctx->autoPlainLeft;
-    else if (plan == kPlanDefault && ctx->sortMode == CS_SORT_AUTO && ctx->shortLeft > 0) --ctx->shortLeft;
+    if (plan == kPlanPlain) {
+        if (ctx->autoPlainLeft > 0) --ctx->autoPlainLeft;
+    } else if (ctx->sortMode == CS_SORT_AUTO) {             // a sort that does not try a finer plan counts towards its hold
+        for (int p = 0; p < plan && p < kPlanDefault; ++p)
+            if (ctx->planLeft[p] > 0) --ctx->planLeft[p];
+    }
     ctx->lastPlan = plan;
     return plan;
 }
 
 int sortPeekPlainPasses(const cs_context* ctx)
 {
-    const bool forced = ctx->sortMode == CS_SORT_PLAIN || ctx->sortMode == CS_SORT_SHORT;
-    const int plan = (ctx->hostCtrl->sortRedoHint && !forced) ? (ctx->lastPlan == kPlanShort ? kPlanDefault : kPlanPlain) : peekPlan(ctx);
+    int plan = peekPlan(ctx);
+    if (ctx->hostCtrl->sortRedoHint && !planForced(ctx) && ctx->lastPlan != kPlanPlain) {
+        // the last sort was redone: the next one takes the next coarser plan that is not on hold
+        plan = ctx->lastPlan + 1;
+        while (plan < kPlanDefault && (ctx->sortMode != CS_SORT_AUTO || ctx->planLeft[plan] > 0)) ++plan;
+    }
     return plan == kPlanPlain ? kSortPasses : planPasses(plan) - 1;
 }
 
@@ -825,8 +857,9 @@ cs_status enqueueSort(cs_context* ctx, u64* keys, u32* perm, u64 n, bool fused, 
         CS_TRY((launchPass<0, true>(ctx, pl, s)));
         return launchPasses<1, kSortPasses>(ctx, pl, s);
     }
-    return plan == kPlanShort ? enqueueShortCut<kSortShortFirst>(ctx, pl, fused, s)
-                              : enqueueShortCut<kSortTopFirst>(ctx, pl, fused, s);
+    return plan == kPlanTiny    ? enqueueShortCut<kSortMaxFirst>(ctx, pl, fused, s)
+           : plan == kPlanShort ? enqueueShortCut<kSortShortFirst>(ctx, pl, fused, s)
+                                : enqueueShortCut<kSortTopFirst>(ctx, pl, fused, s);
 }
 
 // ---- 30-bit keys (L = 10) -----------------------------------------------------------------------

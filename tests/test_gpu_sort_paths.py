@@ -1,7 +1,8 @@
 """GPU parity of cs_sortKeys on every path of cs_sort.cu against the oracle's stable sort (O3).
 
 Default plan: 5 radix passes over the leading 45 bits, the last of which also orders the low 18 bits inside runs of
-equal leading bits; short plan: 4 passes over the leading 36 bits, the low 27 ordered inside runs.  A run longer than
+equal leading bits; short plan: 4 passes over the leading 36 bits, the low 27 ordered inside runs; tiny plan: 3 passes
+over the leading 27 bits, the low 36 ordered inside runs.  A run longer than
 257 elements raises the device flag and the 7 gated plain passes redo the sort.  cs_setSortMode(PLAIN) runs the 7
 plain passes directly; AUTO moves between the three.  All of them must return the same (unique) keys and permutation,
 bit for bit.
@@ -33,11 +34,12 @@ def ctx(cs):
     c.close()
 
 
-@pytest.fixture(params=["default", "short"])
+@pytest.fixture(params=["default", "short", "tiny"])
 def plan(request, cs):
     """(sort mode, LOW): the plan whose last pass orders the low LOW bits inside runs of equal leading bits: the default
-    plan (5 passes over bits 18..62) and the short plan (4 passes over bits 27..62)."""
-    return (cs.SORT_DEFAULT, 18) if request.param == "default" else (cs.SORT_SHORT, 27)
+    plan (5 passes over bits 18..62), the short plan (4 passes over bits 27..62), the tiny plan (3 passes over bits
+    36..62)."""
+    return {"default": (cs.SORT_DEFAULT, 18), "short": (cs.SORT_SHORT, 27), "tiny": (cs.SORT_TINY, 36)}[request.param]
 
 
 def check(cs, ctx, k, mode=0):
@@ -54,7 +56,7 @@ def check(cs, ctx, k, mode=0):
 
 def keys_with_runs(rng, run_lengths, LOW, low_mode="random"):
     """Keys whose bits above LOW form runs of the given lengths, shuffled."""
-    tops = rng.choice(1 << 34, size=len(run_lengths), replace=False).astype(np.uint64)
+    tops = rng.choice(1 << min(34, 63 - LOW), size=len(run_lengths), replace=False).astype(np.uint64)
     parts = []
     for t, r in zip(tops, run_lengths):
         if low_mode == "random":
@@ -92,7 +94,7 @@ def test_runs_at_the_ends_and_across_blocks(cs, ctx, plan):
     mode, LOW = plan
     rng = np.random.default_rng(3)
     n_runs = 600
-    tops = np.sort(rng.choice(1 << 34, size=n_runs, replace=False).astype(np.uint64))
+    tops = np.sort(rng.choice(1 << min(34, 63 - LOW), size=n_runs, replace=False).astype(np.uint64))
     lens = rng.integers(100, MAX_RUN + 1, n_runs)            # long runs straddle every 256-thread block
     lens[0] = MAX_RUN
     lens[-1] = MAX_RUN
@@ -115,7 +117,7 @@ def test_plain_mode_equals_default(cs, ctx):
     rng = np.random.default_rng(8)
     for n in (1, 257, 6656, 6657, 123457):
         k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
-        for mode in (cs.SORT_PLAIN, cs.SORT_AUTO, cs.SORT_DEFAULT, cs.SORT_SHORT):
+        for mode in (cs.SORT_PLAIN, cs.SORT_AUTO, cs.SORT_DEFAULT, cs.SORT_SHORT, cs.SORT_TINY):
             check(cs, ctx, k, mode)
     with pytest.raises(cs.CornerstoneError):
         ctx.setSortMode(7)
@@ -140,13 +142,13 @@ def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
         assert np.array_equal(cs.u32(got["perm"]), ref["perm"])
         assert np.array_equal(cs.u64(got["leaves"]), ref["leaves"])
         assert np.array_equal(cs.u32(got["nodeCount"]), ref["nodeCount"])
-    # the ladder of CS_SORT_AUTO: the short plan (3 plain passes + the fused last one), redone on the device; the default
-    # plan (4 + 1), redone as well; then the 7 plain passes for 16 builds; then the default plan is tried again (and
-    # redone again): one pathological step does not cost every later one
-    short, default, plain = plans[0], plans[1], plans[2]        # 3, 4 and 7 with the 9-bit digits
-    assert short + 1 == default and plain > default + 1
-    assert plans == [short, default] + [plain] * 16 + [default, plain]
-    # CS_SORT_DEFAULT never tries the short plan
+    # the ladder of CS_SORT_AUTO: the tiny plan (2 plain passes + the fused last one), redone on the device; the short
+    # plan (3 + 1) and the default plan (4 + 1), redone as well; then the 7 plain passes for 16 builds; then the default
+    # plan is tried again (and redone again): one pathological step does not cost every later one
+    tiny, short, default, plain = plans[0], plans[1], plans[2], plans[3]        # 2, 3, 4 and 7 with the 9-bit digits
+    assert tiny + 1 == short and short + 1 == default and plain > default + 1
+    assert plans == [tiny, short, default] + [plain] * 16 + [default]
+    # CS_SORT_DEFAULT never tries the finer plans
     ctx.setSortMode(cs.SORT_DEFAULT)
     plans = []
     for _ in range(3):
@@ -157,28 +159,38 @@ def test_build_switches_to_plain_passes_after_a_redo(cs, ctx):
     ctx.setSortMode(cs.SORT_AUTO)
 
 
-def test_auto_backs_off_from_the_short_plan(cs, ctx):
-    """More than 257 particles in a level-12 cell but none in a level-15 cell: the short plan is redone once, then the
-    default plan serves (no redo, no plain passes); uniform particles stay on the short plan."""
+def test_auto_backs_off_from_the_finer_plans(cs, ctx):
+    """More than 257 particles in a level-12 cell but none in a level-15 cell: the tiny and the short plan are redone
+    once each, then the default plan serves (no redo, no plain passes).  More than 257 in a level-9 cell only: the short
+    plan serves.  Uniform particles stay on the tiny plan."""
     rng = np.random.default_rng(22)
     n = 50000
     k = np.concatenate([rng.integers(0, 1 << 63, n, dtype=np.uint64),
                         (np.uint64(0x765432101) << np.uint64(27)) | rng.integers(0, 1 << 27, 2000, dtype=np.uint64)])
     rng.shuffle(k)
     ctx.setSortMode(cs.SORT_AUTO)
-    short = ctx.sortPasses()
+    tiny = ctx.sortPasses()
     plans = []
-    for _ in range(6):
+    for _ in range(7):
         plans.append(ctx.sortPasses())
         check(cs, ctx, k, mode=None)
-    assert plans == [short] + [short + 1] * 5
+    assert plans == [tiny, tiny + 1] + [tiny + 2] * 5
+    k9 = np.concatenate([rng.integers(0, 1 << 63, n, dtype=np.uint64),
+                         (np.uint64(0x3654321) << np.uint64(36)) | rng.integers(0, 1 << 36, 2000, dtype=np.uint64)])
+    rng.shuffle(k9)
+    ctx.setSortMode(cs.SORT_AUTO)
+    plans = []
+    for _ in range(5):
+        plans.append(ctx.sortPasses())
+        check(cs, ctx, k9, mode=None)
+    assert plans == [tiny] + [tiny + 1] * 4
     ctx.setSortMode(cs.SORT_AUTO)
     u = rng.integers(0, 1 << 63, 200000, dtype=np.uint64)
     plans = []
     for _ in range(4):
         plans.append(ctx.sortPasses())
         check(cs, ctx, u, mode=None)
-    assert plans == [short] * 4
+    assert plans == [tiny] * 4
 
 
 def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
@@ -189,14 +201,16 @@ def test_sort_keys_alone_learns_of_the_redo(cs, ctx):
                         (np.uint64(0x1234567) << np.uint64(30)) | rng.integers(0, 1 << 18, 3000, dtype=np.uint64)])
     rng.shuffle(k)
     ctx.setSortMode(cs.SORT_AUTO)
-    short = ctx.sortPasses()                                    # 3 with the 9-bit digits
+    tiny = ctx.sortPasses()                                     # 2 with the 9-bit digits
     check(cs, ctx, k)                                           # check() synchronises when it copies the result back
-    assert ctx.sortPasses() == short + 1                        # the default plan
+    assert ctx.sortPasses() == tiny + 1                         # the short plan
     check(cs, ctx, k, mode=None)
-    assert ctx.sortPasses() > short + 2                         # 7: all digits
+    assert ctx.sortPasses() == tiny + 2                         # the default plan
+    check(cs, ctx, k, mode=None)
+    assert ctx.sortPasses() > tiny + 3                          # 7: all digits
     check(cs, ctx, k, mode=None)
     ctx.setSortMode(cs.SORT_AUTO)
-    assert ctx.sortPasses() == short
+    assert ctx.sortPasses() == tiny
 
 
 def test_workload_shapes(cs, ctx):
